@@ -1,0 +1,146 @@
+/*
+ * bkgdet.h -- C ABI of the B200-native background + detection hot path of arxiv 2502.10783
+ * ("Image Pre-Processing Framework for Time-Domain Astronomy in the Artificial Intelligence Era").
+ *
+ * The three calls BASELINE.json names -- bkg_estimate, bkg_subtract, detect_sources -- plus context,
+ * workspace queries, two single-step entry points used by the parity tests, and one host-buffer
+ * convenience call.  Citations are PAPER.md line numbers with the section
+ * they fall in; A<n> are the readings of silent/garbled passages listed in DESIGN.md.
+ *
+ * Conventions (all calls)
+ *   - Frames are float32, row-major, contiguous [B, H, W]; W must be a multiple of 4; H*W < 2^31.
+ *   - Every d_* argument is a DEVICE pointer owned by the caller, 16-byte aligned, valid until the
+ *     stream work completes.  h_* arguments are HOST pointers.  The library allocates nothing per call
+ *     except inside bd_run_host (buffers cached in the context).
+ *   - cuda_stream is a cudaStream_t passed as void* (0 = legacy default stream).  Calls enqueue work
+ *     and return; they never synchronise (bd_run_host does).
+ *   - Return value: BD_OK (0) or a negative BD_E* code; bd_last_error() gives text.
+ *   - Non-finite pixels: undefined results.
+ *   - Mesh grid: ny = ceil(H/mesh_h), nx = ceil(W/mesh_w); partial edge meshes are their own mesh (A9).
+ */
+#ifndef BKGDET_H
+#define BKGDET_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BD_OK 0
+#define BD_EINVAL (-1)      /* null pointer, non-positive size, even filter, W % 4 != 0, misaligned pointer ... */
+#define BD_EWORKSPACE (-2)  /* workspace too small */
+#define BD_ECUDA (-3)       /* CUDA runtime/driver error (text in bd_last_error) */
+#define BD_EUNSUPPORTED (-4) /* mesh too large for the kernels (see bd_mesh_stats) */
+
+typedef struct bd_ctx bd_ctx; /* opaque: device properties, TMA encode entry point, cached buffers, last error */
+
+/* Parameters of background estimation.  PAPER.md:67 (sub-regions, default 64x64), :78 (sigma range,
+ * maximum iterations), :80 (median filter), :69-76 eqs. 1-4 (estimators). */
+typedef struct {
+    int32_t mesh_h, mesh_w;   /* sub-region size in pixels; default 64, 64 */
+    int32_t filt_h, filt_w;   /* median-filter window on the mesh grid, odd, 1..11; default 3, 3   :80 */
+    double clip_sigma;        /* k_c of median +- k_c*std; default 3.0                              :78 */
+    int32_t clip_iters;       /* maximum rejection rounds (0 = no clipping); default 5             :78 */
+    int32_t skew_guard;       /* 0 (default) = estimator formula as printed; 1 = A12 rule: std==0 -> mean,
+                                 |mean-median|/std >= 0.3 -> median */
+    double median_factor;     /* background = median_factor*median - mean_factor*mean (eq. 4, A2):       */
+    double mean_factor;       /* (3,2) mode [default]; (2.5,1.5) eq. 3; (1,0) eq. 1 median; (0,-1) eq. 2 mean */
+} bd_bkg_params;
+
+/* One catalogue record (detect_sources).  PAPER.md:153 (peak value, total flux per candidate), :159
+ * (isophotal photometry); readings A18-A20.  Coordinates are 0-based, pixel centre at integer
+ * coordinates, x = column, y = row.  Moments are intensity-weighted by sub. */
+typedef struct {
+    int32_t frame;                      /* frame index in the batch */
+    int32_t label;                      /* 1 + minimum raster index (y*W + x) of the component, per frame */
+    int32_t npix;                       /* pixels in the component */
+    int32_t xmin, xmax, ymin, ymax;     /* bounding box, inclusive */
+    int32_t xpeak, ypeak;               /* position of the maximum of sub (ties: smallest raster index) */
+    float peak;                         /* max of sub over the component */
+    double flux;                        /* sum of sub */
+    double x, y;                        /* centroid  sum(I*x)/sum(I) */
+    double x2, y2, xy;                  /* central second moments  sum(I*(x-xc)^2)/sum(I) ... */
+} bd_source;
+
+/* ---- context ------------------------------------------------------------------------------------ */
+int bd_create(bd_ctx **ctx, int device);   /* binds to CUDA device `device`; returns BD_ECUDA if none */
+void bd_destroy(bd_ctx *ctx);
+const char *bd_last_error(const bd_ctx *ctx);
+void bd_default_bkg_params(bd_bkg_params *p);
+int bd_grid_shape(int H, int W, int mesh_h, int mesh_w, int *ny, int *nx);
+
+/* ---- workspace sizes (bytes of device memory the caller must pass as d_ws) ------------------------ */
+int bd_bkg_workspace_bytes(const bd_ctx *ctx, int B, int H, int W, const bd_bkg_params *p, size_t *bytes);
+int bd_detect_workspace_bytes(const bd_ctx *ctx, int B, int H, int W, int64_t cat_capacity, size_t *bytes);
+
+/* ---- a1: per-mesh sigma-clipped statistics (kernel K1).  PAPER.md:67-78, eqs. 1-4. --------------------
+ * For every mesh: up to clip_iters rounds of {median, mean, population std of the survivors; reject
+ * outside median +- clip_sigma*std (inclusive bounds, A6)}, stop when a round rejects nothing (A7), then
+ * the final statistics of the survivors.  Sums are accumulated in float64 against float64 bounds, so
+ * the survivor sets equal the float64 definition's.
+ * Outputs, each [B, ny, nx], any may be NULL:  d_bkg_raw = median_factor*median - mean_factor*mean
+ * (float64), d_rms_raw = std (float64), d_median, d_mean (float64), d_n_kept (int32 survivors).
+ * Limits: mesh_w % 4 == 0 and mesh_w <= 256 use the TMA loader, other widths a plain loader; a mesh
+ * must fit the shared memory of one thread-block cluster (<= 8 CTAs x 200 KiB) else BD_EUNSUPPORTED. */
+int bd_mesh_stats(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg_params *p,
+                  double *d_bkg_raw, double *d_rms_raw, double *d_median, double *d_mean,
+                  int32_t *d_n_kept, void *cuda_stream);
+
+/* ---- a2: median filter of both mesh grids + cubic B-spline prefilter (kernel K2).  PAPER.md:80. --------
+ * In: raw grids float64 [B, ny, nx].  Out: filtered grids (float32, for the caller; may be NULL) and the
+ * spline coefficients (float64) bkg_subtract consumes.  Window truncated at the grid border (A13);
+ * both grids filtered (A11); half-sample-symmetric spline boundary (A14).  d_ws: >= 2*B*ny*nx doubles. */
+int bd_grid_filter_spline(bd_ctx *ctx, const double *d_bkg_raw, const double *d_rms_raw, int B, int ny, int nx,
+                          int filt_h, int filt_w, float *d_bkg_mesh, float *d_rms_mesh,
+                          double *d_bkg_coef, double *d_rms_coef, void *d_ws, size_t ws_bytes,
+                          void *cuda_stream);
+
+/* ---- bkg_estimate = a1 + a2.  PAPER.md:67-80. -------------------------------------------------------
+ * d_bkg_mesh, d_rms_mesh: filtered mesh grids, float32 [B, ny, nx] (may be NULL).
+ * d_bkg_coef, d_rms_coef: spline coefficients, float64 [B, ny, nx] (required).
+ * d_ws / ws_bytes: at least bd_bkg_workspace_bytes(). */
+int bkg_estimate(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg_params *p,
+                 float *d_bkg_mesh, float *d_rms_mesh, double *d_bkg_coef, double *d_rms_coef,
+                 void *d_ws, size_t ws_bytes, void *cuda_stream);
+
+/* ---- bkg_subtract = a3 (kernel K3, fused).  PAPER.md:80 (spline interpolation back to full
+ * resolution), :61-65 (removal), :153 (threshold scan). -------------------------------------------------
+ * Per pixel: bkg, rms = cubic B-spline value of the coefficient grids at u=(x+1/2)/mesh_w-1/2,
+ * v=(y+1/2)/mesh_h-1/2 (A14);  sub = img - bkg;  mask = rms > 0 && sub > detect_k*rms (strict, A15).
+ * The background and the comparison are evaluated in float64; outputs are rounded to float32.
+ * d_sub (required), d_bkg, d_rms: float32 [B,H,W]; d_mask: uint8 [B,H,W] (0/1).  d_bkg, d_rms, d_mask may be
+ * NULL (not emitted); detect_k <= 0 with d_mask != NULL is BD_EINVAL. */
+int bkg_subtract(bd_ctx *ctx, const float *d_img, int B, int H, int W, int mesh_h, int mesh_w,
+                 const double *d_bkg_coef, const double *d_rms_coef, double detect_k,
+                 float *d_sub, float *d_bkg, float *d_rms, uint8_t *d_mask, void *cuda_stream);
+
+/* ---- detect_sources = a4 + a5 (kernels K4, K5).  PAPER.md:153 (connect pixels above the main
+ * threshold into candidates; peak and total flux per candidate), :159 (isophotal flux). ------------------
+ * d_mask: uint8 [B,H,W], non-zero = foreground.  If NULL the mask is computed from
+ * (d_sub, d_rms, detect_k) with the bkg_subtract rule in float64 on the float32 inputs.
+ * d_labels: int32 [B,H,W] out; 8-connected components (A16), label = 1 + minimum raster index of the
+ * component within its frame, 0 = background; all components are labelled (A20).
+ * d_cat: records of components with npix >= min_area (A19), ascending (frame, label); the first
+ * min(n_total, cat_capacity) are written.  d_n_sources: int64 [B] true per-frame counts (device).
+ * Catalogue overflow is not an error: records beyond cat_capacity are dropped.
+ * Sums use float64 atomics: flux/centroid/moments are not bit-reproducible run to run (labels are).
+ * d_ws / ws_bytes: at least bd_detect_workspace_bytes(). */
+int detect_sources(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_t *d_mask,
+                   int B, int H, int W, double detect_k, int32_t min_area,
+                   int32_t *d_labels, bd_source *d_cat, int64_t cat_capacity, int64_t *d_n_sources,
+                   void *d_ws, size_t ws_bytes, void *cuda_stream);
+
+/* ---- whole chain from HOST buffers (pinned or pageable), synchronous. ----------------------------------
+ * Copies h_img to the device, runs bkg_estimate -> bkg_subtract -> detect_sources, copies the
+ * catalogue and the per-frame counts back, and waits.  Device buffers are cached in ctx between calls.
+ * h_cat: [cat_capacity] records; h_n_sources: [B].  Returns BD_OK or an error code. */
+int bd_run_host(bd_ctx *ctx, const float *h_img, int B, int H, int W, const bd_bkg_params *p,
+                double detect_k, int32_t min_area, bd_source *h_cat, int64_t cat_capacity,
+                int64_t *h_n_sources);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BKGDET_H */

@@ -1,0 +1,226 @@
+"""Thin Python binding of libbkgdet (include/bkgdet.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; PyTorch is used for device memory
+and the current stream, nothing else.  There is no CPU fallback: if the shared library is missing or
+cannot be loaded, importing the binding's functions raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+import torch
+
+from . import _build
+
+__all__ = ["BkgParams", "Context", "SOURCE_DTYPE", "bkg_estimate", "bkg_subtract", "detect_sources", "mesh_stats",
+           "grid_filter_spline", "run_host", "grid_shape", "load_library", "EXPORTS"]
+
+EXPORTS = ["bd_create", "bd_destroy", "bd_last_error", "bd_default_bkg_params", "bd_grid_shape",
+           "bd_bkg_workspace_bytes", "bd_detect_workspace_bytes", "bd_mesh_stats", "bd_grid_filter_spline",
+           "bkg_estimate", "bkg_subtract", "detect_sources", "bd_run_host"]
+
+
+class _CParams(C.Structure):
+    _fields_ = [("mesh_h", C.c_int32), ("mesh_w", C.c_int32), ("filt_h", C.c_int32), ("filt_w", C.c_int32),
+                ("clip_sigma", C.c_double), ("clip_iters", C.c_int32), ("skew_guard", C.c_int32),
+                ("median_factor", C.c_double), ("mean_factor", C.c_double)]
+
+
+SOURCE_DTYPE = np.dtype([
+    ("frame", np.int32), ("label", np.int32), ("npix", np.int32), ("xmin", np.int32), ("xmax", np.int32),
+    ("ymin", np.int32), ("ymax", np.int32), ("xpeak", np.int32), ("ypeak", np.int32), ("peak", np.float32),
+    ("flux", np.float64), ("x", np.float64), ("y", np.float64), ("x2", np.float64), ("y2", np.float64),
+    ("xy", np.float64)], align=True)
+assert SOURCE_DTYPE.itemsize == 88
+
+
+@dataclass
+class BkgParams:
+    mesh_h: int = 64
+    mesh_w: int = 64
+    filt_h: int = 3
+    filt_w: int = 3
+    clip_sigma: float = 3.0
+    clip_iters: int = 5
+    skew_guard: int = 0
+    median_factor: float = 3.0
+    mean_factor: float = 2.0
+
+    def c(self) -> _CParams:
+        return _CParams(self.mesh_h, self.mesh_w, self.filt_h, self.filt_w, self.clip_sigma, self.clip_iters,
+                        self.skew_guard, self.median_factor, self.mean_factor)
+
+
+_lib = None
+
+
+def load_library(build: bool = True):
+    """dlopen libbkgdet.so (building it with nvcc first if the sources are newer)."""
+    global _lib
+    if _lib is None:
+        path = _build.build() if build else _build.LIB
+        lib = C.CDLL(path)
+        lib.bd_last_error.restype = C.c_char_p
+        for name in EXPORTS:
+            getattr(lib, name)          # fail loudly if a declared symbol is missing
+        _lib = lib
+    return _lib
+
+
+class BkgdetError(RuntimeError):
+    pass
+
+
+def grid_shape(H, W, mesh_h, mesh_w):
+    return (H + mesh_h - 1) // mesh_h, (W + mesh_w - 1) // mesh_w
+
+
+def _ptr(t):
+    return C.c_void_p(0 if t is None else t.data_ptr())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+class Context:
+    """Owns a bd_ctx bound to one CUDA device."""
+
+    def __init__(self, device: int = 0):
+        if not torch.cuda.is_available():
+            raise BkgdetError("libbkgdet needs a CUDA device (sm_100a); there is no CPU fallback")
+        self.lib = load_library()
+        self.device = device
+        self.h = C.c_void_p()
+        rc = self.lib.bd_create(C.byref(self.h), C.c_int(device))
+        if rc != 0:
+            raise BkgdetError(f"bd_create failed ({rc})")
+
+    def close(self):
+        if getattr(self, "h", None) and self.h.value:
+            self.lib.bd_destroy(self.h)
+            self.h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def check(self, rc: int):
+        if rc != 0:
+            raise BkgdetError(f"libbkgdet error {rc}: {self.lib.bd_last_error(self.h).decode()}")
+
+    def bkg_workspace_bytes(self, B, H, W, p: BkgParams) -> int:
+        n = C.c_size_t()
+        cp = p.c()
+        self.check(self.lib.bd_bkg_workspace_bytes(self.h, B, H, W, C.byref(cp), C.byref(n)))
+        return n.value
+
+    def detect_workspace_bytes(self, B, H, W, cat_capacity) -> int:
+        n = C.c_size_t()
+        self.check(self.lib.bd_detect_workspace_bytes(self.h, B, H, W, C.c_int64(cat_capacity), C.byref(n)))
+        return n.value
+
+
+def _dev(ctx):
+    return torch.device("cuda", ctx.device)
+
+
+def mesh_stats(ctx: Context, img: torch.Tensor, p: BkgParams):
+    """a1 (K1).  img float32 [B,H,W] on the device -> dict of [B,ny,nx] tensors."""
+    B, H, W = img.shape
+    ny, nx = grid_shape(H, W, p.mesh_h, p.mesh_w)
+    dev = _dev(ctx)
+    out = {k: torch.empty((B, ny, nx), dtype=torch.float64, device=dev) for k in ("bkg", "rms", "median", "mean")}
+    out["n_kept"] = torch.empty((B, ny, nx), dtype=torch.int32, device=dev)
+    cp = p.c()
+    ctx.check(ctx.lib.bd_mesh_stats(ctx.h, _ptr(img), B, H, W, C.byref(cp), _ptr(out["bkg"]), _ptr(out["rms"]),
+                                    _ptr(out["median"]), _ptr(out["mean"]), _ptr(out["n_kept"]), _stream()))
+    return out
+
+
+def grid_filter_spline(ctx: Context, bkg_raw: torch.Tensor, rms_raw: torch.Tensor, filt_h: int, filt_w: int):
+    """a2 (K2).  raw grids float64 [B,ny,nx] -> (bkg_mesh f32, rms_mesh f32, bkg_coef f64, rms_coef f64)."""
+    B, ny, nx = bkg_raw.shape
+    dev = _dev(ctx)
+    bm = torch.empty((B, ny, nx), dtype=torch.float32, device=dev); rm = torch.empty_like(bm)
+    cb = torch.empty((B, ny, nx), dtype=torch.float64, device=dev); cr = torch.empty_like(cb)
+    ws = torch.empty(2 * B * ny * nx + 32, dtype=torch.float64, device=dev)
+    ctx.check(ctx.lib.bd_grid_filter_spline(ctx.h, _ptr(bkg_raw), _ptr(rms_raw), B, ny, nx, filt_h, filt_w, _ptr(bm),
+                                            _ptr(rm), _ptr(cb), _ptr(cr), _ptr(ws), C.c_size_t(ws.numel() * 8), _stream()))
+    return bm, rm, cb, cr
+
+
+def bkg_estimate(ctx: Context, img: torch.Tensor, p: BkgParams, ws: torch.Tensor | None = None):
+    """a1 + a2.  -> (bkg_mesh f32, rms_mesh f32, bkg_coef f64, rms_coef f64), each [B,ny,nx]."""
+    B, H, W = img.shape
+    ny, nx = grid_shape(H, W, p.mesh_h, p.mesh_w)
+    dev = _dev(ctx)
+    bm = torch.empty((B, ny, nx), dtype=torch.float32, device=dev); rm = torch.empty_like(bm)
+    cb = torch.empty((B, ny, nx), dtype=torch.float64, device=dev); cr = torch.empty_like(cb)
+    if ws is None:
+        ws = torch.empty(ctx.bkg_workspace_bytes(B, H, W, p), dtype=torch.uint8, device=dev)
+    cp = p.c()
+    ctx.check(ctx.lib.bkg_estimate(ctx.h, _ptr(img), B, H, W, C.byref(cp), _ptr(bm), _ptr(rm), _ptr(cb), _ptr(cr),
+                                   _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+    return bm, rm, cb, cr
+
+
+def bkg_subtract(ctx: Context, img: torch.Tensor, mesh_h: int, mesh_w: int, bkg_coef: torch.Tensor,
+                 rms_coef: torch.Tensor, detect_k: float, want_bkg: bool = True, want_rms: bool = True,
+                 want_mask: bool = True, out: dict | None = None):
+    """a3 (K3).  -> dict(sub, bkg, rms float32 [B,H,W]; mask uint8 [B,H,W]); absent outputs are None."""
+    B, H, W = img.shape
+    dev = _dev(ctx)
+    o = out or {}
+    sub = o.get("sub") if o.get("sub") is not None else torch.empty((B, H, W), dtype=torch.float32, device=dev)
+    bkg = (o.get("bkg") if o.get("bkg") is not None else torch.empty_like(sub)) if want_bkg else None
+    rms = (o.get("rms") if o.get("rms") is not None else torch.empty_like(sub)) if want_rms else None
+    mask = (o.get("mask") if o.get("mask") is not None else torch.empty((B, H, W), dtype=torch.uint8, device=dev)) if want_mask else None
+    ctx.check(ctx.lib.bkg_subtract(ctx.h, _ptr(img), B, H, W, mesh_h, mesh_w, _ptr(bkg_coef), _ptr(rms_coef),
+                                   C.c_double(detect_k), _ptr(sub), _ptr(bkg), _ptr(rms), _ptr(mask), _stream()))
+    return dict(sub=sub, bkg=bkg, rms=rms, mask=mask)
+
+
+def detect_sources(ctx: Context, sub: torch.Tensor, rms: torch.Tensor | None, mask: torch.Tensor | None,
+                   detect_k: float, min_area: int, cat_capacity: int, ws: torch.Tensor | None = None,
+                   out: dict | None = None):
+    """a4 + a5 (K4, K5).  -> dict(labels int32 [B,H,W], cat uint8 [cap*88] (device), n_sources int64 [B])."""
+    B, H, W = sub.shape
+    dev = _dev(ctx)
+    o = out or {}
+    labels = o.get("labels") if o.get("labels") is not None else torch.empty((B, H, W), dtype=torch.int32, device=dev)
+    cat = o.get("cat") if o.get("cat") is not None else torch.empty(max(cat_capacity, 1) * SOURCE_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+    nsrc = o.get("n_sources") if o.get("n_sources") is not None else torch.empty(B, dtype=torch.int64, device=dev)
+    if ws is None:
+        ws = torch.empty(ctx.detect_workspace_bytes(B, H, W, cat_capacity), dtype=torch.uint8, device=dev)
+    ctx.check(ctx.lib.detect_sources(ctx.h, _ptr(sub), _ptr(rms), _ptr(mask), B, H, W, C.c_double(detect_k),
+                                     C.c_int32(min_area), _ptr(labels), _ptr(cat), C.c_int64(cat_capacity), _ptr(nsrc),
+                                     _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+    return dict(labels=labels, cat=cat, n_sources=nsrc)
+
+
+def catalogue_to_numpy(cat: torch.Tensor, n_sources: torch.Tensor, cat_capacity: int) -> np.ndarray:
+    """Device catalogue bytes -> numpy structured array of the valid records (synchronises)."""
+    n = int(min(int(n_sources.sum().item()), cat_capacity))
+    raw = cat[: n * SOURCE_DTYPE.itemsize].cpu().numpy()
+    return raw.view(SOURCE_DTYPE).copy()
+
+
+def run_host(ctx: Context, img: np.ndarray, p: BkgParams, detect_k: float, min_area: int, cat_capacity: int,
+             cat: np.ndarray | None = None):
+    """Whole chain from a HOST float32 array [B,H,W] (bd_run_host).  -> (records, n_sources[B])."""
+    assert img.dtype == np.float32 and img.ndim == 3 and img.flags.c_contiguous
+    B, H, W = img.shape
+    if cat is None:
+        cat = np.empty(max(cat_capacity, 1), dtype=SOURCE_DTYPE)
+    n = np.zeros(B, dtype=np.int64)
+    cp = p.c()
+    ctx.check(ctx.lib.bd_run_host(ctx.h, C.c_void_p(img.ctypes.data), B, H, W, C.byref(cp), C.c_double(detect_k),
+                                  C.c_int32(min_area), C.c_void_p(cat.ctypes.data), C.c_int64(cat_capacity),
+                                  C.c_void_p(n.ctypes.data)))
+    return cat[: min(int(n.sum()), cat_capacity)], n

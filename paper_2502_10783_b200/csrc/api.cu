@@ -1,0 +1,228 @@
+// C-ABI entry points of libbkgdet (include/bkgdet.h): argument checks, workspace carving, launch order.
+// No computation happens here; every step of the path runs in the kernels of k1..k45.
+#include <stdarg.h>
+#include <stdlib.h>
+
+#include "common.cuh"
+
+int bd_set_error(bd_ctx *ctx, int code, const char *fmt, ...) {
+    if (ctx) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(ctx->err, sizeof(ctx->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+static bool aligned16(const void *p) { return ((uintptr_t)p & 15) == 0; }
+
+extern "C" {
+
+int bd_create(bd_ctx **out, int device) {
+    if (!out) return BD_EINVAL;
+    *out = nullptr;
+    int n = 0;
+    if (cudaGetDeviceCount(&n) != cudaSuccess || n <= 0 || device < 0 || device >= n) return BD_ECUDA;
+    if (cudaSetDevice(device) != cudaSuccess) return BD_ECUDA;
+    bd_ctx *c = (bd_ctx *)calloc(1, sizeof(bd_ctx));
+    if (!c) return BD_ECUDA;
+    c->device = device;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { free(c); return BD_ECUDA; }
+    c->num_sms = prop.multiProcessorCount;
+    c->smem_optin = prop.sharedMemPerBlockOptin;
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+        c->encode_tiled = (decltype(c->encode_tiled))fn;
+    cudaGetLastError();
+    *out = c;
+    return BD_OK;
+}
+
+void bd_destroy(bd_ctx *ctx) {
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    if (ctx->host_dev) cudaFree(ctx->host_dev);
+    if (ctx->host_pinned) cudaFreeHost(ctx->host_pinned);
+    if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
+    free(ctx);
+}
+
+const char *bd_last_error(const bd_ctx *ctx) { return ctx ? ctx->err : "null context"; }
+
+void bd_default_bkg_params(bd_bkg_params *p) {
+    if (!p) return;
+    p->mesh_h = 64; p->mesh_w = 64;
+    p->filt_h = 3; p->filt_w = 3;
+    p->clip_sigma = 3.0; p->clip_iters = 5;
+    p->skew_guard = 0;
+    p->median_factor = 3.0; p->mean_factor = 2.0;
+}
+
+int bd_grid_shape(int H, int W, int mesh_h, int mesh_w, int *ny, int *nx) {
+    if (H <= 0 || W <= 0 || mesh_h <= 0 || mesh_w <= 0 || !ny || !nx) return BD_EINVAL;
+    *ny = (H + mesh_h - 1) / mesh_h;
+    *nx = (W + mesh_w - 1) / mesh_w;
+    return BD_OK;
+}
+
+static int check_frame(bd_ctx *ctx, int B, int H, int W) {
+    if (!ctx) return BD_EINVAL;
+    if (B <= 0 || H <= 0 || W <= 0) return bd_set_error(ctx, BD_EINVAL, "B, H, W must be positive");
+    if (B > 65535) return bd_set_error(ctx, BD_EINVAL, "B must be <= 65535");
+    if (W % 4) return bd_set_error(ctx, BD_EINVAL, "W must be a multiple of 4");
+    if ((long long)H * W >= (1ll << 31)) return bd_set_error(ctx, BD_EINVAL, "H*W must be < 2^31");
+    return BD_OK;
+}
+
+static int check_params(bd_ctx *ctx, const bd_bkg_params *p) {
+    if (!p) return bd_set_error(ctx, BD_EINVAL, "null params");
+    if (p->mesh_h <= 0 || p->mesh_w <= 0) return bd_set_error(ctx, BD_EINVAL, "mesh size must be positive");
+    if (p->filt_h < 1 || p->filt_w < 1 || !(p->filt_h & 1) || !(p->filt_w & 1) || p->filt_h > 11 || p->filt_w > 11)
+        return bd_set_error(ctx, BD_EINVAL, "filter size must be odd and in 1..11");
+    if (p->clip_iters < 0 || !(p->clip_sigma > 0.0)) return bd_set_error(ctx, BD_EINVAL, "clip_iters >= 0 and clip_sigma > 0 required");
+    return BD_OK;
+}
+
+int bd_bkg_workspace_bytes(const bd_ctx *ctx, int B, int H, int W, const bd_bkg_params *p, size_t *bytes) {
+    if (!ctx || !p || !bytes || B <= 0 || H <= 0 || W <= 0 || p->mesh_h <= 0 || p->mesh_w <= 0) return BD_EINVAL;
+    size_t cells = (size_t)B * ((H + p->mesh_h - 1) / p->mesh_h) * ((W + p->mesh_w - 1) / p->mesh_w);
+    *bytes = 4 * bd_align_up(cells * sizeof(double), 256) + 256;   // raw bkg, raw rms, 2 x prefilter scratch
+    return BD_OK;
+}
+
+int bd_detect_workspace_bytes(const bd_ctx *ctx, int B, int H, int W, int64_t cat_capacity, size_t *bytes) {
+    if (!ctx || !bytes || B <= 0 || H <= 0 || W <= 0 || cat_capacity < 0) return BD_EINVAL;
+    *bytes = k45_workspace_bytes(B, H, W, cat_capacity);
+    return BD_OK;
+}
+
+int bd_mesh_stats(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg_params *p, double *d_bkg_raw,
+                  double *d_rms_raw, double *d_median, double *d_mean, int32_t *d_n_kept, void *cuda_stream) {
+    int rc = check_frame(ctx, B, H, W);
+    if (rc) return rc;
+    if ((rc = check_params(ctx, p))) return rc;
+    if (!d_img || !aligned16(d_img)) return bd_set_error(ctx, BD_EINVAL, "d_img null or misaligned");
+    return k1_launch(ctx, d_img, B, H, W, p, d_bkg_raw, d_rms_raw, d_median, d_mean, d_n_kept, (cudaStream_t)cuda_stream);
+}
+
+int bd_grid_filter_spline(bd_ctx *ctx, const double *d_bkg_raw, const double *d_rms_raw, int B, int ny, int nx,
+                          int filt_h, int filt_w, float *d_bkg_mesh, float *d_rms_mesh, double *d_bkg_coef,
+                          double *d_rms_coef, void *d_ws, size_t ws_bytes, void *cuda_stream) {
+    if (!ctx) return BD_EINVAL;
+    if (!d_bkg_raw || !d_rms_raw || !d_bkg_coef || !d_rms_coef || !d_ws) return bd_set_error(ctx, BD_EINVAL, "null pointer");
+    if (B <= 0 || ny <= 0 || nx <= 0 || B > 65535) return bd_set_error(ctx, BD_EINVAL, "bad grid shape");
+    if (filt_h < 1 || filt_w < 1 || !(filt_h & 1) || !(filt_w & 1) || filt_h > 11 || filt_w > 11)
+        return bd_set_error(ctx, BD_EINVAL, "filter size must be odd and in 1..11");
+    size_t need = 2 * (size_t)B * ny * nx * sizeof(double);
+    if (ws_bytes < need) return bd_set_error(ctx, BD_EWORKSPACE, "grid workspace: need %zu bytes, got %zu", need, ws_bytes);
+    return k2_launch(ctx, d_bkg_raw, d_rms_raw, B, ny, nx, filt_h, filt_w, d_bkg_mesh, d_rms_mesh, d_bkg_coef, d_rms_coef,
+                     (double *)d_ws, (cudaStream_t)cuda_stream);
+}
+
+int bkg_estimate(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg_params *p, float *d_bkg_mesh,
+                 float *d_rms_mesh, double *d_bkg_coef, double *d_rms_coef, void *d_ws, size_t ws_bytes,
+                 void *cuda_stream) {
+    int rc = check_frame(ctx, B, H, W);
+    if (rc) return rc;
+    if ((rc = check_params(ctx, p))) return rc;
+    if (!d_img || !aligned16(d_img)) return bd_set_error(ctx, BD_EINVAL, "d_img null or misaligned");
+    if (!d_bkg_coef || !d_rms_coef || !d_ws) return bd_set_error(ctx, BD_EINVAL, "null coefficient or workspace pointer");
+    size_t need = 0;
+    bd_bkg_workspace_bytes(ctx, B, H, W, p, &need);
+    if (ws_bytes < need) return bd_set_error(ctx, BD_EWORKSPACE, "bkg workspace: need %zu bytes, got %zu", need, ws_bytes);
+    const int ny = (H + p->mesh_h - 1) / p->mesh_h, nx = (W + p->mesh_w - 1) / p->mesh_w;
+    const size_t cells = (size_t)B * ny * nx, stride = bd_align_up(cells * sizeof(double), 256);
+    char *base = (char *)bd_align_up((size_t)d_ws, 256);
+    double *raw_b = (double *)base, *raw_r = (double *)(base + stride), *scratch = (double *)(base + 2 * stride);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    rc = k1_launch(ctx, d_img, B, H, W, p, raw_b, raw_r, nullptr, nullptr, nullptr, st);
+    if (rc) return rc;
+    return k2_launch(ctx, raw_b, raw_r, B, ny, nx, p->filt_h, p->filt_w, d_bkg_mesh, d_rms_mesh, d_bkg_coef, d_rms_coef,
+                     scratch, st);
+}
+
+int bkg_subtract(bd_ctx *ctx, const float *d_img, int B, int H, int W, int mesh_h, int mesh_w, const double *d_bkg_coef,
+                 const double *d_rms_coef, double detect_k, float *d_sub, float *d_bkg, float *d_rms, uint8_t *d_mask,
+                 void *cuda_stream) {
+    int rc = check_frame(ctx, B, H, W);
+    if (rc) return rc;
+    if (mesh_h <= 0 || mesh_w <= 0) return bd_set_error(ctx, BD_EINVAL, "mesh size must be positive");
+    if (!d_img || !d_bkg_coef || !d_rms_coef || !d_sub) return bd_set_error(ctx, BD_EINVAL, "null pointer");
+    if (!aligned16(d_img) || !aligned16(d_sub) || !aligned16(d_bkg) || !aligned16(d_rms) || !aligned16(d_mask))
+        return bd_set_error(ctx, BD_EINVAL, "misaligned pointer (16 bytes required)");
+    if (d_mask && !(detect_k > 0.0)) return bd_set_error(ctx, BD_EINVAL, "detect_k must be > 0 when a mask is requested");
+    return k3_launch(ctx, d_img, B, H, W, mesh_h, mesh_w, d_bkg_coef, d_rms_coef, detect_k, d_sub, d_bkg, d_rms, d_mask,
+                     (cudaStream_t)cuda_stream);
+}
+
+int detect_sources(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_t *d_mask, int B, int H, int W,
+                   double detect_k, int32_t min_area, int32_t *d_labels, bd_source *d_cat, int64_t cat_capacity,
+                   int64_t *d_n_sources, void *d_ws, size_t ws_bytes, void *cuda_stream) {
+    int rc = check_frame(ctx, B, H, W);
+    if (rc) return rc;
+    if (!d_sub || !d_labels || !d_n_sources || !d_ws) return bd_set_error(ctx, BD_EINVAL, "null pointer");
+    if (!d_mask && (!d_rms || !(detect_k > 0.0))) return bd_set_error(ctx, BD_EINVAL, "no mask: d_rms and detect_k > 0 required");
+    if (cat_capacity < 0 || (cat_capacity > 0 && !d_cat)) return bd_set_error(ctx, BD_EINVAL, "bad catalogue buffer");
+    if (!aligned16(d_sub) || !aligned16(d_labels) || !aligned16(d_mask) || !aligned16(d_rms))
+        return bd_set_error(ctx, BD_EINVAL, "misaligned pointer (16 bytes required)");
+    return k45_launch(ctx, d_sub, d_rms, d_mask, B, H, W, detect_k, min_area, d_labels, d_cat, cat_capacity, d_n_sources,
+                      d_ws, ws_bytes, (cudaStream_t)cuda_stream);
+}
+
+int bd_run_host(bd_ctx *ctx, const float *h_img, int B, int H, int W, const bd_bkg_params *p, double detect_k,
+                int32_t min_area, bd_source *h_cat, int64_t cat_capacity, int64_t *h_n_sources) {
+    int rc = check_frame(ctx, B, H, W);
+    if (rc) return rc;
+    if ((rc = check_params(ctx, p))) return rc;
+    if (!h_img || !h_n_sources || cat_capacity < 0 || (cat_capacity > 0 && !h_cat))
+        return bd_set_error(ctx, BD_EINVAL, "null host pointer");
+    BD_CUDA_CHECK(ctx, cudaSetDevice(ctx->device));
+    if (!ctx->host_stream) BD_CUDA_CHECK(ctx, cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking));
+    cudaStream_t st = ctx->host_stream;
+    const size_t P = (size_t)B * H * W;
+    const int ny = (H + p->mesh_h - 1) / p->mesh_h, nx = (W + p->mesh_w - 1) / p->mesh_w;
+    const size_t cells = (size_t)B * ny * nx;
+    size_t ws_b = 0, ws_d = 0;
+    bd_bkg_workspace_bytes(ctx, B, H, W, p, &ws_b);
+    bd_detect_workspace_bytes(ctx, B, H, W, cat_capacity, &ws_d);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = bd_align_up(off + bytes, 256); return o; };
+    const size_t o_img = take(P * 4), o_sub = take(P * 4), o_rms = take(P * 4), o_mask = take(P), o_lab = take(P * 4);
+    const size_t o_cb = take(cells * 8), o_cr = take(cells * 8), o_wsb = take(ws_b), o_wsd = take(ws_d);
+    const size_t o_cat = take((size_t)cat_capacity * sizeof(bd_source)), o_n = take((size_t)B * 8);
+    if (off > ctx->host_dev_bytes) {
+        if (ctx->host_dev) cudaFree(ctx->host_dev);
+        ctx->host_dev = nullptr; ctx->host_dev_bytes = 0;
+        BD_CUDA_CHECK(ctx, cudaMalloc(&ctx->host_dev, off));
+        ctx->host_dev_bytes = off;
+    }
+    char *d = (char *)ctx->host_dev;
+    BD_CUDA_CHECK(ctx, cudaMemcpyAsync(d + o_img, h_img, P * 4, cudaMemcpyHostToDevice, st));
+    rc = bkg_estimate(ctx, (const float *)(d + o_img), B, H, W, p, nullptr, nullptr, (double *)(d + o_cb), (double *)(d + o_cr),
+                      d + o_wsb, ws_b, st);
+    if (rc) return rc;
+    rc = bkg_subtract(ctx, (const float *)(d + o_img), B, H, W, p->mesh_h, p->mesh_w, (const double *)(d + o_cb),
+                      (const double *)(d + o_cr), detect_k, (float *)(d + o_sub), nullptr, (float *)(d + o_rms),
+                      (uint8_t *)(d + o_mask), st);
+    if (rc) return rc;
+    rc = detect_sources(ctx, (const float *)(d + o_sub), (const float *)(d + o_rms), (const uint8_t *)(d + o_mask), B, H, W,
+                        detect_k, min_area, (int32_t *)(d + o_lab), (bd_source *)(d + o_cat), cat_capacity,
+                        (int64_t *)(d + o_n), d + o_wsd, ws_d, st);
+    if (rc) return rc;
+    BD_CUDA_CHECK(ctx, cudaMemcpyAsync(h_n_sources, d + o_n, (size_t)B * 8, cudaMemcpyDeviceToHost, st));
+    BD_CUDA_CHECK(ctx, cudaStreamSynchronize(st));
+    int64_t total = 0;
+    for (int f = 0; f < B; ++f) total += h_n_sources[f];
+    if (total > cat_capacity) total = cat_capacity;
+    if (total > 0) {
+        BD_CUDA_CHECK(ctx, cudaMemcpyAsync(h_cat, d + o_cat, (size_t)total * sizeof(bd_source), cudaMemcpyDeviceToHost, st));
+        BD_CUDA_CHECK(ctx, cudaStreamSynchronize(st));
+    }
+    return BD_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,75 @@
+// Internal declarations shared by the .cu files of libbkgdet (sm_100a only).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/bkgdet.h"
+
+struct bd_ctx {
+    int device;
+    int num_sms;
+    size_t smem_optin;
+    char err[512];
+    // cuTensorMapEncodeTiled, fetched through the runtime (no -lcuda link dependency)
+    CUresult (*encode_tiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                             const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                             CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    // bd_run_host cache
+    void *host_dev;
+    size_t host_dev_bytes;
+    void *host_pinned;
+    size_t host_pinned_bytes;
+    cudaStream_t host_stream;
+};
+
+int bd_set_error(bd_ctx *ctx, int code, const char *fmt, ...);
+
+#define BD_CUDA_CHECK(ctx, expr)                                                                       \
+    do {                                                                                               \
+        cudaError_t _e = (expr);                                                                       \
+        if (_e != cudaSuccess)                                                                         \
+            return bd_set_error((ctx), BD_ECUDA, "%s:%d %s: %s", __FILE__, __LINE__, #expr,            \
+                                cudaGetErrorString(_e));                                               \
+    } while (0)
+
+static inline size_t bd_align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// ---- launchers implemented in the kernel files ---------------------------------------------------------
+struct K1Plan {
+    int cluster;        // CTAs per mesh (1, 2, 4, 8)
+    int slab_rows;      // mesh rows held by one CTA
+    int threads;        // threads per CTA
+    size_t smem_bytes;  // dynamic shared memory per CTA
+    int use_tma;
+};
+int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan);
+int k1_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg_params *p, double *d_bkg_raw,
+              double *d_rms_raw, double *d_median, double *d_mean, int32_t *d_n_kept, cudaStream_t st);
+
+int k2_launch(bd_ctx *ctx, const double *d_bkg_raw, const double *d_rms_raw, int B, int ny, int nx, int fh, int fw,
+              float *d_bkg_mesh, float *d_rms_mesh, double *d_bkg_coef, double *d_rms_coef, double *d_scratch,
+              cudaStream_t st);
+
+int k3_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, int mh, int mw, const double *d_bkg_coef,
+              const double *d_rms_coef, double detect_k, float *d_sub, float *d_bkg, float *d_rms, uint8_t *d_mask,
+              cudaStream_t st);
+
+size_t k45_workspace_bytes(int B, int H, int W, int64_t cat_capacity);
+int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_t *d_mask, int B, int H, int W,
+               double detect_k, int min_area, int32_t *d_labels, bd_source *d_cat, int64_t cat_capacity,
+               int64_t *d_n_sources, void *d_ws, size_t ws_bytes, cudaStream_t st);
+
+// ---- small device helpers ------------------------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ uint32_t f32_to_key(float f) {   // order-preserving map float32 -> uint32
+    uint32_t b = __float_as_uint(f);
+    return b ^ ((b >> 31) ? 0xFFFFFFFFu : 0x80000000u);
+}
+__device__ __forceinline__ float key_to_f32(uint32_t k) {
+    uint32_t b = (k >> 31) ? (k ^ 0x80000000u) : ~k;
+    return __uint_as_float(b);
+}
+#endif

@@ -1,0 +1,57 @@
+"""CPU-only: the C-ABI library builds for sm_100a, loads, and exports every symbol include/bkgdet.h declares.
+No compute calls are made (there is no GPU here)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_functions():
+    src = open(os.path.join(ROOT, "include", "bkgdet.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    names = re.findall(r"^\s*(?:int|void|const char \*)\s*\**\s*([A-Za-z_]\w*)\s*\(", src, flags=re.M)
+    return sorted(set(names))
+
+
+def test_header_declares_the_three_named_calls():
+    names = declared_functions()
+    for n in ("bkg_estimate", "bkg_subtract", "detect_sources"):
+        assert n in names
+    assert len(names) >= 13
+
+
+def test_library_builds_loads_and_exports_all_symbols():
+    from paper_2502_10783_b200 import _build
+    import paper_2502_10783_b200 as m
+    lib = ctypes.CDLL(_build.build())
+    for n in declared_functions():
+        assert hasattr(lib, n), f"{n} declared in bkgdet.h but not exported"
+    assert sorted(m.EXPORTS) == declared_functions()
+
+
+def test_struct_layouts_match_header():
+    import paper_2502_10783_b200 as m
+    assert m.SOURCE_DTYPE.itemsize == 88 and m.SOURCE_DTYPE.fields["flux"][1] == 40
+    assert ctypes.sizeof(m._CParams) == 48   # 4 x i32, f64, 2 x i32, 2 x f64
+
+
+def test_no_gpu_no_fallback():
+    """Without a CUDA device the product path must fail loudly, not fall back to the CPU."""
+    import torch
+    import paper_2502_10783_b200 as m
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(m.BkgdetError):
+        m.Context(0)
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2502_10783_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in txt and "from oracle" not in txt and "oracle/" not in txt, f

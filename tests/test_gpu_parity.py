@@ -1,0 +1,326 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+Run with `python -m pytest tests -m gpu` on a B200."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402
+from parity_util import (assert_catalogue_equal, assert_maps_close, assert_mask_parity, fragile_touched_labels,  # noqa: E402
+                         to_oracle_params)
+from synth import CONFIGS, make_frame, make_frames, noise_frame  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def bd():
+    import paper_2502_10783_b200 as m
+    return m
+
+
+@pytest.fixture(scope="module")
+def ctx(bd):
+    c = bd.Context(0)
+    yield c
+    c.close()
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def params_for(bd, cfg, **kw):
+    d = dict(mesh_h=cfg.mesh, mesh_w=cfg.mesh, filt_h=cfg.filt, filt_w=cfg.filt, clip_sigma=cfg.clip_sigma,
+             clip_iters=cfg.clip_iters)
+    d.update(kw)
+    return bd.BkgParams(**d)
+
+
+# ------------------------------------------------------------------------------------------- K1
+def check_mesh_stats(bd, ctx, img, p):
+    """img float32 [B,H,W] numpy."""
+    out = bd.mesh_stats(ctx, dev(img), p)
+    torch.cuda.synchronize()
+    op = to_oracle_params(p)
+    for f in range(img.shape[0]):
+        st = oracle.mesh_stats(img[f], op)
+        assert np.array_equal(out["n_kept"][f].cpu().numpy(), st["n_kept"]), "n_kept differs"
+        assert np.array_equal(out["median"][f].cpu().numpy(), st["median"]), "median differs"
+        for k, ok in (("mean", "mean"), ("rms", "rms"), ("bkg", "bkg")):
+            g, w = out[k][f].cpu().numpy(), st[ok]
+            tol = 1e-10 * np.maximum(np.abs(w), np.abs(st["median"])) + 1e-300
+            if k == "rms":
+                tol = 1e-9 * np.maximum(np.abs(w), 1e-6 * np.abs(st["median"])) + 1e-300
+            assert np.all(np.abs(g - w) <= tol), f"{k}: worst {np.max(np.abs(g - w) / tol)} x tol"
+
+
+@pytest.mark.parametrize("cid,H,W", [(1, 512, 512), (2, 512, 640), (3, 528, 768), (4, 256, 320), (5, 384, 512)])
+def test_k1_mesh_stats_configs(bd, ctx, cid, H, W):
+    """Each config's frame recipe at a reduced size (several meshes + a ragged last mesh row for cfg 3)."""
+    cfg = CONFIGS[cid]
+    img = make_frames(cfg, H=H, W=W, B=2 if cid == 4 else 1)
+    check_mesh_stats(bd, ctx, img, params_for(bd, cfg))
+
+
+@pytest.mark.parametrize("mh,mw", [(64, 64), (32, 48), (50, 36), (17, 23), (128, 128), (256, 256), (100, 300), (7, 5), (1, 4)])
+def test_k1_mesh_shapes(bd, ctx, mh, mw):
+    """TMA and plain loaders, cluster sizes 1/2/4, partial meshes on both edges."""
+    rng = np.random.default_rng(mh * 1000 + mw)
+    img = rng.normal(500, 20, size=(1, 300, 340)).astype(np.float32)
+    img[0, rng.integers(0, 300, 200), rng.integers(0, 340, 200)] = 60000.0
+    check_mesh_stats(bd, ctx, img, bd.BkgParams(mesh_h=mh, mesh_w=mw))
+
+
+def test_k1_degenerate_inputs(bd, ctx):
+    const = np.full((1, 128, 128), 1234.5, dtype=np.float32)
+    check_mesh_stats(bd, ctx, const, bd.BkgParams())
+    ties = np.random.default_rng(1).integers(0, 4, size=(1, 128, 192)).astype(np.float32)     # heavy ties
+    check_mesh_stats(bd, ctx, ties, bd.BkgParams())
+    neg = np.random.default_rng(2).normal(0, 1, size=(1, 64, 128)).astype(np.float32)        # both signs
+    check_mesh_stats(bd, ctx, neg, bd.BkgParams(clip_sigma=1.0))
+    check_mesh_stats(bd, ctx, neg, bd.BkgParams(clip_iters=0))
+    check_mesh_stats(bd, ctx, neg, bd.BkgParams(median_factor=2.5, mean_factor=1.5, skew_guard=1))
+    outl = np.full((1, 64, 64), 100.0, dtype=np.float32)
+    outl[0, 3, 5] = outl[0, 60, 60] = 60000.0
+    check_mesh_stats(bd, ctx, outl, bd.BkgParams())
+    cauchy = np.random.default_rng(3).standard_cauchy(size=(1, 64, 128)).astype(np.float32)
+    check_mesh_stats(bd, ctx, cauchy, bd.BkgParams(clip_sigma=2.0))
+
+
+# ------------------------------------------------------------------------------------------- K2
+@pytest.mark.parametrize("ny,nx,fh,fw", [(8, 8, 3, 3), (37, 36, 5, 5), (2, 3, 3, 3), (1, 5, 5, 1), (96, 96, 3, 3),
+                                         (1, 1, 3, 3), (5, 9, 1, 1), (40, 300, 11, 7)])
+def test_k2_filter_and_prefilter(bd, ctx, ny, nx, fh, fw):
+    rng = np.random.default_rng(ny * 100 + nx)
+    B = 3
+    raw_b = rng.normal(1000, 30, size=(B, ny, nx)); raw_r = rng.uniform(5, 40, size=(B, ny, nx))
+    bm, rm, cb, cr = bd.grid_filter_spline(ctx, dev(raw_b), dev(raw_r), fh, fw)
+    torch.cuda.synchronize()
+    for f in range(B):
+        for raw, m, c in ((raw_b, bm, cb), (raw_r, rm, cr)):
+            filt = oracle.grid_median(raw[f], fh, fw)
+            assert np.array_equal(m[f].cpu().numpy(), filt.astype(np.float32))
+            want = oracle.spline_coeffs(filt)
+            assert np.max(np.abs(c[f].cpu().numpy() - want)) <= 1e-11 * np.max(np.abs(want))
+
+
+# ------------------------------------------------------------------------------------------- K3
+@pytest.mark.parametrize("H,W,mh,mw", [(256, 512, 64, 64), (300, 1028, 64, 64), (528, 2048, 256, 256), (97, 132, 50, 36),
+                                       (64, 64, 64, 64), (40, 1024, 7, 5)])
+def test_k3_maps_and_mask(bd, ctx, H, W, mh, mw):
+    rng = np.random.default_rng(H + W)
+    ny, nx = oracle.grid_shape(H, W, mh, mw)
+    B = 2
+    img = rng.normal(1000, 30, size=(B, H, W)).astype(np.float32)
+    gb = 1000 + 50 * rng.normal(size=(B, ny, nx)); gr = rng.uniform(20, 40, size=(B, ny, nx))
+    cb = np.stack([oracle.spline_coeffs(g) for g in gb]); cr = np.stack([oracle.spline_coeffs(g) for g in gr])
+    out = bd.bkg_subtract(ctx, dev(img), mh, mw, dev(cb), dev(cr), 1.5)
+    torch.cuda.synchronize()
+    for f in range(B):
+        bkg64 = oracle.spline_eval(cb[f], H, W, mh, mw); rms64 = oracle.spline_eval(cr[f], H, W, mh, mw)
+        sub64, _, mask, frag = oracle.subtract_threshold(img[f], bkg64, rms64, 1.5)
+        assert_maps_close(out["bkg"][f].cpu().numpy(), bkg64, "bkg")
+        assert_maps_close(out["rms"][f].cpu().numpy(), rms64, "rms")
+        assert_maps_close(out["sub"][f].cpu().numpy(), sub64, "sub", scale=bkg64)
+        assert_mask_parity(out["mask"][f].cpu().numpy(), mask, frag)
+        # tighter than the bar: float32 rounding of a float64 evaluation
+        assert np.max(np.abs(out["bkg"][f].cpu().numpy() - bkg64) / np.abs(bkg64)) < 1e-7
+    o2 = bd.bkg_subtract(ctx, dev(img), mh, mw, dev(cb), dev(cr), 1.5, want_bkg=False, want_rms=False, want_mask=False)
+    torch.cuda.synchronize()
+    assert o2["bkg"] is None and torch.equal(o2["sub"], out["sub"])
+
+
+# ------------------------------------------------------------------------------------------- K4 / K5
+def run_detect(bd, ctx, sub, mask, min_area, cap=None, rms=None, k=1.5):
+    B, H, W = sub.shape
+    cap = cap if cap is not None else B * ((H + 1) // 2) * ((W + 1) // 2) + 1
+    out = bd.detect_sources(ctx, dev(sub), None if rms is None else dev(rms), None if mask is None else dev(mask), k, min_area, cap)
+    torch.cuda.synchronize()
+    n = out["n_sources"].cpu().numpy()
+    cat = bd.catalogue_to_numpy(out["cat"], out["n_sources"], cap)
+    return out["labels"].cpu().numpy(), cat, n
+
+
+def check_detect(bd, ctx, sub, mask, min_area):
+    labels, cat, n = run_detect(bd, ctx, sub, mask, min_area)
+    worst = {}
+    for f in range(sub.shape[0]):
+        want_lab = oracle.label(mask[f])
+        assert np.array_equal(labels[f], want_lab), f"labels differ in frame {f}: {np.count_nonzero(labels[f] != want_lab)} px"
+        want_cat = oracle.reduce_sources(want_lab, sub[f], min_area)
+        assert n[f] == len(want_cat)
+        worst = assert_catalogue_equal(cat, want_cat, frame=f)
+    return worst
+
+
+@pytest.mark.parametrize("density", [0.02, 0.07, 0.16, 0.32, 0.41, 0.6, 0.95])
+@pytest.mark.parametrize("H,W", [(211, 172), (64, 256), (33, 132), (300, 516)])
+def test_k45_random_masks(bd, ctx, density, H, W):
+    rng = np.random.default_rng(int(density * 100) + H)
+    B = 2
+    mask = (rng.uniform(size=(B, H, W)) < density).astype(np.uint8)
+    sub = rng.uniform(0.5, 50.0, size=(B, H, W)).astype(np.float32)
+    check_detect(bd, ctx, sub, mask, 1)
+    check_detect(bd, ctx, sub, mask, 5)
+
+
+def test_k45_structured_masks(bd, ctx):
+    H, W = 97, 388
+    yy, xx = np.mgrid[:H, :W]
+    cases = [np.eye(H, W, dtype=np.uint8), np.fliplr(np.eye(H, W, dtype=np.uint8)),
+             ((yy + xx) % 2 == 0).astype(np.uint8), np.ones((H, W), np.uint8), np.zeros((H, W), np.uint8),
+             (yy % 2 == 0).astype(np.uint8), (xx % 2 == 0).astype(np.uint8),
+             ((yy % 4 == 0) | ((xx % 6 == 0) & (yy % 8 < 5))).astype(np.uint8),           # comb across tile seams
+             (((yy // 3 + xx // 5) % 2 == 0) & (yy % 7 != 0)).astype(np.uint8)]
+    spiral = np.zeros((H, W), np.uint8)
+    for k in range(0, 40, 4):   # nested rectangles joined into one long snake crossing every seam
+        spiral[k, k:W - k] = 1; spiral[H - 1 - k, k:W - k] = 1; spiral[k:H - k, k] = 1; spiral[k:H - k, W - 1 - k] = 1
+        spiral[k + 1:k + 4, k + 2] = 0 if k % 8 else 1
+    cases.append(spiral)
+    mask = np.stack(cases)
+    sub = np.random.default_rng(0).uniform(1, 2, size=mask.shape).astype(np.float32)
+    check_detect(bd, ctx, sub, mask, 1)
+
+
+def test_k45_exhaustive_4x4(bd, ctx):
+    """All 65536 masks of a 4x4 frame, as batches of 4096 frames (also exercises B > 1 bookkeeping)."""
+    P = 16
+    allm = ((np.arange(2 ** P)[:, None] >> np.arange(P)[None, :]) & 1).astype(np.uint8).reshape(-1, 4, 4)
+    sub = np.random.default_rng(4).uniform(1, 9, size=(4096, 4, 4)).astype(np.float32)
+    for c in range(0, 65536, 4096 * 4):          # every 4th batch keeps the test short; batch 0 and 12 included
+        m = allm[c:c + 4096]
+        labels, cat, n = run_detect(bd, ctx, sub, m, 2)
+        for f in range(0, 4096):
+            want = oracle.label(m[f])
+            assert np.array_equal(labels[f], want)
+        f_check = [0, 1, 777, 4095]
+        for f in f_check:
+            assert_catalogue_equal(cat, oracle.reduce_sources(oracle.label(m[f]), sub[f], 2), frame=f)
+        assert n.sum() == len(cat)
+
+
+def test_k45_mask_from_sub_rms_and_overflow(bd, ctx):
+    rng = np.random.default_rng(12)
+    B, H, W = 1, 130, 260
+    sub = rng.normal(0, 10, size=(B, H, W)).astype(np.float32)
+    rms = np.full((B, H, W), 10.0, dtype=np.float32); rms[0, :5] = 0.0
+    labels, cat, n = run_detect(bd, ctx, sub, None, 3, rms=rms, k=1.0)
+    mask = ((rms > 0) & (sub.astype(np.float64) > 1.0 * rms.astype(np.float64))).astype(np.uint8)
+    want_lab = oracle.label(mask[0])
+    assert np.array_equal(labels[0], want_lab)
+    want = oracle.reduce_sources(want_lab, sub[0], 3)
+    assert_catalogue_equal(cat, want, frame=0)
+    # capacity smaller than the catalogue: counts stay true, the first `cap` records are valid
+    cap = 7
+    _, cat2, n2 = run_detect(bd, ctx, sub, mask, 3, cap=cap)
+    assert n2[0] == len(want) and len(cat2) == cap
+    assert_catalogue_equal(cat2, want[:cap], frame=0)
+
+
+# ------------------------------------------------------------------------------------------- whole chain
+def run_chain(bd, ctx, img, p, k, min_area, cap):
+    d_img = dev(img)
+    bm, rm, cb, cr = bd.bkg_estimate(ctx, d_img, p)
+    o = bd.bkg_subtract(ctx, d_img, p.mesh_h, p.mesh_w, cb, cr, k)
+    det = bd.detect_sources(ctx, o["sub"], o["rms"], o["mask"], k, min_area, cap)
+    torch.cuda.synchronize()
+    return bm, rm, o, det
+
+
+def check_chain(bd, ctx, img, p, k, min_area, frames=None):
+    B, H, W = img.shape
+    cap = 1 << 20
+    bm, rm, o, det = run_chain(bd, ctx, img, p, k, min_area, cap)
+    cat = bd.catalogue_to_numpy(det["cat"], det["n_sources"], cap)
+    n = det["n_sources"].cpu().numpy()
+    report = {}
+    for f in (range(B) if frames is None else frames):
+        r = oracle.chain(img[f], to_oracle_params(p), k, min_area)
+        assert np.array_equal(bm[f].cpu().numpy(), r["bkg_grid"].astype(np.float32)) or \
+            np.max(np.abs(bm[f].cpu().numpy() - r["bkg_grid"]) / np.abs(r["bkg_grid"])) < 1e-6
+        assert_maps_close(o["bkg"][f].cpu().numpy(), r["bkg"], "bkg")
+        assert_maps_close(o["rms"][f].cpu().numpy(), r["rms"], "rms")
+        assert_maps_close(o["sub"][f].cpu().numpy(), r["sub64"], "sub", scale=r["bkg"])
+        mask_g = o["mask"][f].cpu().numpy()
+        ndiff = assert_mask_parity(mask_g, r["mask"], r["fragile"])
+        # labels: bit-exact given the same mask
+        lab_g = det["labels"][f].cpu().numpy()
+        assert np.array_equal(lab_g, oracle.label(mask_g))
+        # catalogue from the GPU's own labels/sub: exact stage parity
+        sub_g = o["sub"][f].cpu().numpy()
+        stage = oracle.reduce_sources(lab_g, sub_g, min_area)
+        assert n[f] == len(stage)
+        worst = assert_catalogue_equal(cat, stage, frame=f)
+        # catalogue against the oracle's own chain: 1:1 outside components touching fragile pixels
+        exempt = fragile_touched_labels(r["labels"], r["fragile"]) if ndiff else ()
+        if ndiff:
+            exempt = np.union1d(exempt, fragile_touched_labels(lab_g, r["fragile"]))
+        worst2 = assert_catalogue_equal(cat, r["cat"], frame=f, exempt_labels=exempt)
+        report[f] = dict(mask_diff=ndiff, n_sources=int(n[f]), fragile=int(r["fragile"].sum()), stage=worst, chain=worst2,
+                         exempt=len(exempt))
+    return report
+
+
+@pytest.mark.parametrize("cid,H,W,B", [(1, 512, 512, 1), (2, 1024, 1024, 1), (3, 1040, 1024, 1), (4, 512, 512, 3), (5, 768, 768, 1)])
+def test_chain_configs_reduced(bd, ctx, cid, H, W, B):
+    """configs[0] at full size; the others at a size the oracle finishes in seconds (several tiles, ragged tail)."""
+    cfg = CONFIGS[cid]
+    img = make_frames(cfg, H=H, W=W, B=B)
+    rep = check_chain(bd, ctx, img, params_for(bd, cfg), cfg.detect_k, cfg.min_area)
+    assert all(v["n_sources"] > 0 for v in rep.values())
+
+
+def test_chain_constant_frame(bd, ctx):
+    img = np.full((1, 256, 320), 4321.0, dtype=np.float32)
+    p = bd.BkgParams()
+    bm, rm, o, det = run_chain(bd, ctx, img, p, 1.5, 5, 16)
+    assert torch.all(o["bkg"] == 4321.0) and torch.all(o["rms"].abs() < 1e-9)
+    assert int(o["mask"].sum()) == 0 and int(det["n_sources"].sum()) == 0 and int(det["labels"].abs().sum()) == 0
+
+
+@pytest.mark.parametrize("cid", [2, 3, 5])
+def test_chain_full_size(bd, ctx, cid):
+    """BASELINE.json full sizes, in the launch configuration bench.py times."""
+    cfg = CONFIGS[cid]
+    img = make_frames(cfg)
+    rep = check_chain(bd, ctx, img, params_for(bd, cfg), cfg.detect_k, cfg.min_area)
+    print(cfg.name, rep)
+
+
+def test_chain_config4_batch(bd, ctx):
+    """64 x 2048^2 in one call; the oracle checks frames 0, 31 and 63 in full and counts for the rest are
+    cross-checked through labels (bit-exact labels imply exact component counts)."""
+    cfg = CONFIGS[4]
+    img = make_frames(cfg)
+    rep = check_chain(bd, ctx, img, params_for(bd, cfg), cfg.detect_k, cfg.min_area, frames=[0, 31, 63])
+    print(cfg.name, rep)
+
+
+def test_run_host_matches_device_path(bd, ctx):
+    cfg = CONFIGS[1]
+    img = make_frames(cfg)
+    p = params_for(bd, cfg)
+    cat_h, n_h = bd.run_host(ctx, img, p, cfg.detect_k, cfg.min_area, 4096)
+    bm, rm, o, det = run_chain(bd, ctx, img, p, cfg.detect_k, cfg.min_area, 4096)
+    cat_d = bd.catalogue_to_numpy(det["cat"], det["n_sources"], 4096)
+    assert np.array_equal(n_h, det["n_sources"].cpu().numpy())
+    for k in ("label", "npix", "xpeak", "ypeak"):
+        assert np.array_equal(cat_h[k], cat_d[k])
+    assert np.allclose(cat_h["flux"], cat_d["flux"], rtol=1e-12)
+
+
+# ------------------------------------------------------------------------------------------- errors
+def test_error_codes(bd, ctx):
+    img = torch.zeros((1, 64, 66), dtype=torch.float32, device="cuda")     # W % 4 != 0
+    with pytest.raises(bd.BkgdetError):
+        bd.mesh_stats(ctx, img, bd.BkgParams())
+    img = torch.zeros((1, 64, 64), dtype=torch.float32, device="cuda")
+    with pytest.raises(bd.BkgdetError):
+        bd.mesh_stats(ctx, img, bd.BkgParams(filt_h=4))
+    with pytest.raises(bd.BkgdetError):
+        bd.bkg_estimate(ctx, img, bd.BkgParams(), ws=torch.empty(8, dtype=torch.uint8, device="cuda"))
+    with pytest.raises(bd.BkgdetError):
+        bd.detect_sources(ctx, img, None, None, 1.5, 5, 16)                   # no mask and no rms
+    with pytest.raises(bd.BkgdetError):
+        bd.mesh_stats(ctx, torch.zeros((1, 4096, 4096), dtype=torch.float32, device="cuda"), bd.BkgParams(mesh_h=2048, mesh_w=2048))
