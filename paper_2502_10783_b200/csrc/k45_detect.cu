@@ -85,7 +85,7 @@ __device__ __forceinline__ uint32_t sm_find(volatile uint32_t *parent, uint32_t 
     while (p != x) { x = p; p = parent[x]; }
     return x;
 }
-__device__ __forceinline__ void sm_union(uint32_t *parent, uint32_t a, uint32_t b) {
+__device__ __noinline__ void sm_union(uint32_t *parent, uint32_t a, uint32_t b) {
     for (;;) {
         a = sm_find(parent, a);
         b = sm_find(parent, b);
@@ -126,12 +126,14 @@ __global__ void __launch_bounds__(K4_NT) k4a_tile_label(const uint8_t *mask, int
         if (ry < 0 || rx < 0 || rx >= TW) return 0u;
         return (sm_mask[ry][rx >> 2] >> (8 * (rx & 3))) & 1u;
     };
-#pragma unroll
+    // not unrolled on purpose: the unrolled body (16 pixels x 4 inlined union loops) was 85 KB of SASS and
+    // the kernel was instruction-fetch bound (ncu: 65% stall_no_inst)
+#pragma unroll 1
     for (int k = 0; k < TH / 8; ++k) {
         int ry = warp + 8 * k;
         uint32_t m = sm_mask[ry][lane];
         if (!m) continue;
-#pragma unroll
+#pragma unroll 1
         for (int q = 0; q < 4; ++q) {
             if (!((m >> (8 * q)) & 1u)) continue;
             int rx = rx0 + q;
@@ -147,7 +149,7 @@ __global__ void __launch_bounds__(K4_NT) k4a_tile_label(const uint8_t *mask, int
     }
     __syncthreads();
 
-#pragma unroll
+#pragma unroll 1
     for (int k = 0; k < TH / 8; ++k) {
         int ry = warp + 8 * k;
         bool row_ok = col_ok && (y0 + ry) < H;
