@@ -91,7 +91,7 @@ int bd_mesh_stats(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd
 /* ---- a2: median filter of both mesh grids + cubic B-spline prefilter (kernel K2).  PAPER.md:80. --------
  * In: raw grids float64 [B, ny, nx].  Out: filtered grids (float32, for the caller; may be NULL) and the
  * spline coefficients (float64) bkg_subtract consumes.  Window truncated at the grid border (A13);
- * both grids filtered (A11); half-sample-symmetric spline boundary (A14).  d_ws: >= 2*B*ny*nx doubles. */
+ * both grids filtered (A11); half-sample-symmetric spline boundary (A14).  d_ws: >= 4*B*(ny+nx) doubles. */
 int bd_grid_filter_spline(bd_ctx *ctx, const double *d_bkg_raw, const double *d_rms_raw, int B, int ny, int nx,
                           int filt_h, int filt_w, float *d_bkg_mesh, float *d_rms_mesh,
                           double *d_bkg_coef, double *d_rms_coef, void *d_ws, size_t ws_bytes,

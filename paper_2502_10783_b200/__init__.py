@@ -149,7 +149,7 @@ def grid_filter_spline(ctx: Context, bkg_raw: torch.Tensor, rms_raw: torch.Tenso
     dev = _dev(ctx)
     bm = torch.empty((B, ny, nx), dtype=torch.float32, device=dev); rm = torch.empty_like(bm)
     cb = torch.empty((B, ny, nx), dtype=torch.float64, device=dev); cr = torch.empty_like(cb)
-    ws = torch.empty(2 * B * ny * nx + 32, dtype=torch.float64, device=dev)
+    ws = torch.empty(4 * B * (ny + nx) + 32, dtype=torch.float64, device=dev)
     ctx.check(ctx.lib.bd_grid_filter_spline(ctx.h, _ptr(bkg_raw), _ptr(rms_raw), B, ny, nx, filt_h, filt_w, _ptr(bm),
                                             _ptr(rm), _ptr(cb), _ptr(cr), _ptr(ws), C.c_size_t(ws.numel() * 8), _stream()))
     return bm, rm, cb, cr

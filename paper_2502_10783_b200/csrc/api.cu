@@ -89,8 +89,10 @@ static int check_params(bd_ctx *ctx, const bd_bkg_params *p) {
 
 int bd_bkg_workspace_bytes(const bd_ctx *ctx, int B, int H, int W, const bd_bkg_params *p, size_t *bytes) {
     if (!ctx || !p || !bytes || B <= 0 || H <= 0 || W <= 0 || p->mesh_h <= 0 || p->mesh_w <= 0) return BD_EINVAL;
-    size_t cells = (size_t)B * ((H + p->mesh_h - 1) / p->mesh_h) * ((W + p->mesh_w - 1) / p->mesh_w);
-    *bytes = 4 * bd_align_up(cells * sizeof(double), 256) + 256;   // raw bkg, raw rms, 2 x prefilter scratch
+    const int ny = (H + p->mesh_h - 1) / p->mesh_h, nx = (W + p->mesh_w - 1) / p->mesh_w;
+    size_t cells = (size_t)B * ny * nx;
+    // raw bkg, raw rms, then K2's scratch
+    *bytes = 2 * bd_align_up(cells * sizeof(double), 256) + 2 * (size_t)B * k2_scratch_per_grid(ny, nx) * sizeof(double) + 512;
     return BD_OK;
 }
 
@@ -117,7 +119,7 @@ int bd_grid_filter_spline(bd_ctx *ctx, const double *d_bkg_raw, const double *d_
     if (B <= 0 || ny <= 0 || nx <= 0 || B > 65535) return bd_set_error(ctx, BD_EINVAL, "bad grid shape");
     if (filt_h < 1 || filt_w < 1 || !(filt_h & 1) || !(filt_w & 1) || filt_h > 11 || filt_w > 11)
         return bd_set_error(ctx, BD_EINVAL, "filter size must be odd and in 1..11");
-    size_t need = 2 * (size_t)B * ny * nx * sizeof(double);
+    size_t need = 2 * (size_t)B * k2_scratch_per_grid(ny, nx) * sizeof(double);
     if (ws_bytes < need) return bd_set_error(ctx, BD_EWORKSPACE, "grid workspace: need %zu bytes, got %zu", need, ws_bytes);
     return k2_launch(ctx, d_bkg_raw, d_rms_raw, B, ny, nx, filt_h, filt_w, d_bkg_mesh, d_rms_mesh, d_bkg_coef, d_rms_coef,
                      (double *)d_ws, (cudaStream_t)cuda_stream);

@@ -49,6 +49,8 @@ int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan);
 int k1_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg_params *p, double *d_bkg_raw,
               double *d_rms_raw, double *d_median, double *d_mean, int32_t *d_n_kept, cudaStream_t st);
 
+// doubles of scratch K2 needs per (frame, grid): the Thomas factors of both directions
+static inline __host__ __device__ size_t k2_scratch_per_grid(int ny, int nx) { return 2 * ((size_t)ny + (size_t)nx); }
 int k2_launch(bd_ctx *ctx, const double *d_bkg_raw, const double *d_rms_raw, int B, int ny, int nx, int fh, int fw,
               float *d_bkg_mesh, float *d_rms_mesh, double *d_bkg_coef, double *d_rms_coef, double *d_scratch,
               cudaStream_t st);

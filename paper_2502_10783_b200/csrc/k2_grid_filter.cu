@@ -8,59 +8,103 @@
 namespace {
 
 constexpr int K2_NT = 256;
-constexpr int K2_MAXWIN = 121;   // 11 x 11
 
-// Solve (c[k-1] + 4 c[k] + c[k+1]) / 6 = f[k], c[-1]=c[0], c[n]=c[n-1], along a strided line, in place.
-// Thomas algorithm; `cp` is scratch with the same stride.  The matrix is strictly diagonally dominant.
-__device__ void spline_line(double *f, double *cp, int n, int stride) {
+// Window median of cell (j, i) by rank counting (no per-thread array: a dynamically indexed local array
+// lives in local memory, which made the first version of this kernel 120 us for 1332 cells).
+// Rank of element a = #(v < v_a) + #(v == v_a with smaller window index); ranks are a permutation of 0..n-1.
+__device__ double window_median(const double *g, int ny, int nx, int j, int i, int fh, int fw) {
+    const int j0 = max(0, j - fh / 2), j1 = min(ny - 1, j + fh / 2);
+    const int i0 = max(0, i - fw / 2), i1 = min(nx - 1, i + fw / 2);
+    const int ww = i1 - i0 + 1, n = (j1 - j0 + 1) * ww;
+    const int k_lo = (n - 1) / 2, k_hi = n / 2;
+    double lo = 0.0, hi = 0.0;
+    for (int a = 0; a < n; ++a) {
+        const double va = g[(j0 + a / ww) * nx + i0 + a % ww];
+        int rank = 0;
+        for (int b = 0; b < n; ++b) {
+            const double vb = g[(j0 + b / ww) * nx + i0 + b % ww];
+            rank += (vb < va || (vb == va && b < a)) ? 1 : 0;
+        }
+        if (rank == k_lo) lo = va;
+        if (rank == k_hi) hi = va;
+    }
+    return (n & 1) ? lo : 0.5 * (lo + hi);
+}
+
+// Solve (c[k-1] + 4 c[k] + c[k+1]) / 6 = f[k], c[-1]=c[0], c[n]=c[n-1], along a strided line, in place
+// (Thomas algorithm; the matrix is strictly diagonally dominant).  cp[k], im[k] are the forward-sweep
+// factors, which depend on n only and are shared by every line of that length.
+__device__ void spline_factors(double *cp, double *im, int n) {
+    const double a = 1.0 / 6.0;
+    double m = 5.0 / 6.0;
+    im[0] = 1.0 / m;
+    cp[0] = a / m;
+    for (int k = 1; k < n; ++k) {
+        const double bk = (k == n - 1) ? 5.0 / 6.0 : 4.0 / 6.0;
+        m = bk - a * cp[k - 1];
+        cp[k] = a / m;
+        im[k] = 1.0 / m;
+    }
+}
+__device__ void spline_line(double *f, const double *cp, const double *im, int n, int stride) {
     if (n == 1) return;   // (c0 + 4 c0 + c0)/6 = f0
     const double a = 1.0 / 6.0;
-    double b0 = 5.0 / 6.0;
-    cp[0] = a / b0;
-    f[0] = f[0] / b0;
+    double prev = f[0] * im[0];
+    f[0] = prev;
     for (int k = 1; k < n; ++k) {
-        double bk = (k == n - 1) ? 5.0 / 6.0 : 4.0 / 6.0;
-        double m = bk - a * cp[(size_t)(k - 1) * stride];
-        cp[(size_t)k * stride] = a / m;
-        f[(size_t)k * stride] = (f[(size_t)k * stride] - a * f[(size_t)(k - 1) * stride]) / m;
+        prev = (f[(size_t)k * stride] - a * prev) * im[k];
+        f[(size_t)k * stride] = prev;
     }
-    for (int k = n - 2; k >= 0; --k)
-        f[(size_t)k * stride] -= cp[(size_t)k * stride] * f[(size_t)(k + 1) * stride];
+    for (int k = n - 2; k >= 0; --k) {
+        prev = f[(size_t)k * stride] - cp[k] * prev;
+        f[(size_t)k * stride] = prev;
+    }
 }
+
+// One CTA per (frame, grid).  The grid is staged in shared memory when it fits (K2_SMEM_CELLS cells);
+// otherwise the same code runs on global memory (scratch = 2 * ny * nx doubles per (frame, grid)... the
+// raw grid is read in place and the coefficient array is the working array).
+constexpr int K2_SMEM_CELLS = 2560;
 
 __global__ void __launch_bounds__(K2_NT) k2_filter_prefilter(const double *bkg_raw, const double *rms_raw, int ny,
                                                              int nx, int fh, int fw, float *bkg_mesh,
                                                              float *rms_mesh, double *bkg_coef, double *rms_coef,
                                                              double *scratch) {
+    __shared__ double s_raw[K2_SMEM_CELLS], s_work[K2_SMEM_CELLS];
+    __shared__ double s_cp[2][128], s_im[2][128];
     const int frame = blockIdx.x, which = blockIdx.y;
     const size_t goff = (size_t)frame * ny * nx;
     const double *raw = (which ? rms_raw : bkg_raw) + goff;
     float *mesh = which ? rms_mesh : bkg_mesh;
     double *coef = (which ? rms_coef : bkg_coef) + goff;
-    double *cp = scratch + ((size_t)frame * 2 + which) * ny * nx;
-
-    // median filter -> coef (used as the working array of the prefilter)
-    for (int c = threadIdx.x; c < ny * nx; c += K2_NT) {
-        int j = c / nx, i = c % nx;
-        double win[K2_MAXWIN];
-        int n = 0;
-        for (int dj = -(fh / 2); dj <= fh / 2; ++dj)
-            for (int di = -(fw / 2); di <= fw / 2; ++di) {
-                int jj = j + dj, ii = i + di;
-                if (jj < 0 || jj >= ny || ii < 0 || ii >= nx) continue;
-                double v = raw[jj * nx + ii];
-                int k = n++;
-                while (k > 0 && win[k - 1] > v) { win[k] = win[k - 1]; --k; }   // insertion sort
-                win[k] = v;
-            }
-        double med = (n & 1) ? win[(n - 1) / 2] : 0.5 * (win[n / 2 - 1] + win[n / 2]);
-        coef[c] = med;
+    const int cells = ny * nx;
+    const bool in_smem = cells <= K2_SMEM_CELLS && ny <= 128 && nx <= 128;
+    double *fac = scratch + ((size_t)frame * 2 + which) * k2_scratch_per_grid(ny, nx);   // global factors otherwise
+    double *cp_y = in_smem ? s_cp[0] : fac, *im_y = in_smem ? s_im[0] : fac + ny;
+    double *cp_x = in_smem ? s_cp[1] : fac + 2 * ny, *im_x = in_smem ? s_im[1] : fac + 2 * ny + nx;
+    const double *src = raw;
+    double *work = coef;
+    if (in_smem) {
+        for (int c = threadIdx.x; c < cells; c += K2_NT) s_raw[c] = raw[c];
+        src = s_raw;
+        work = s_work;
+    }
+    if (threadIdx.x == 0) spline_factors(cp_y, im_y, ny);
+    if (threadIdx.x == 32) spline_factors(cp_x, im_x, nx);
+    __syncthreads();
+    for (int c = threadIdx.x; c < cells; c += K2_NT) {
+        const double med = window_median(src, ny, nx, c / nx, c % nx, fh, fw);
+        work[c] = med;
         if (mesh) mesh[goff + c] = (float)med;
     }
     __syncthreads();
-    for (int i = threadIdx.x; i < nx; i += K2_NT) spline_line(coef + i, cp + i, ny, nx);   // along y
+    for (int i = threadIdx.x; i < nx; i += K2_NT) spline_line(work + i, cp_y, im_y, ny, nx);   // along y
     __syncthreads();
-    for (int j = threadIdx.x; j < ny; j += K2_NT) spline_line(coef + (size_t)j * nx, cp + (size_t)j * nx, nx, 1);
+    for (int j = threadIdx.x; j < ny; j += K2_NT) spline_line(work + (size_t)j * nx, cp_x, im_x, nx, 1);
+    if (in_smem) {
+        __syncthreads();
+        for (int c = threadIdx.x; c < cells; c += K2_NT) coef[c] = s_work[c];
+    }
 }
 
 }  // namespace

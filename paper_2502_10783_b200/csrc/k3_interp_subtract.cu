@@ -2,19 +2,39 @@
 // RMS-map emission and threshold-mask generation (step a3).  PAPER.md:80 ("we employ spline
 // interpolation to scale the refined background values back"), :61-65 (removal), :153 (threshold scan).
 //
-// HBM-bound streaming pass: 4 B/px read, up to 13 B/px written.  One thread owns 4 consecutive columns
-// and walks down a strip of rows.  For its columns it keeps, in registers, the four x-collapsed spline
-// coefficients g_r(x) = sum_di beta3(u - i0 - di) * c[R(j0-1+r)][R(i0+di)], r = 0..3, for both grids; a
-// pixel then costs 4 FMAs per map with the row's y-weights (uniform over the CTA, from shared memory).
-// The background and the threshold comparison are evaluated in float64 (the float32 ulp at ~1000 ADU is
-// comparable to the 1e-5*sigma agreement the catalogue needs); the RMS map in float32.
+// HBM-bound streaming pass: 4 B/px read, up to 13 B/px written.  A CTA owns a strip of 1024 columns x
+// `rows` rows; one thread owns 4 consecutive columns (one float4) and walks down the strip with K3_R row
+// loads in flight.
+//
+// Arithmetic.  With h_d(y) = sum_r beta3(v - j0 - r) c[R(j0+r)][R(i0+d)] (the y-collapsed coefficients of the
+// four grid columns i0-1..i0+2 that a pixel of grid cell i0 sees) the spline value is sum_d wx_d h_d, and
+// because the cubic B-spline weights are a partition of unity (sum_d wx_d = 1 exactly),
+//     bkg = h_0 + sum_{d != 0} wx_d (h_d - h_0).
+// The CTA first builds, in float64, a shared-memory table with one entry per (row, i0): h_0 split into a
+// float32 hi/lo pair, the three differences h_d - h_0 (a few ADU: float32 carries them to ~1e-6 ADU) and
+// the four y-collapsed RMS coefficients.  A pixel then costs 3 + 4 float32 FMAs with the x-weights its
+// thread keeps in registers, and sub = (img - hi) - (lo + sum) -- the first difference is exact for sky
+// pixels (Sterbenz), so the result agrees with the float64 definition to ~1e-6 ADU although no float64
+// instruction runs per pixel.  (The float32 ulp at ~1000 ADU, 6e-5, would not be good enough for the
+// 1e-5*sigma mask agreement if bkg itself were accumulated in float32.)
 #include "common.cuh"
 
 namespace {
 
 constexpr int K3_NT = 256;   // threads per CTA
 constexpr int K3_PX = 4;     // pixels per thread per row (one float4)
-constexpr int K3_R = 4;      // rows whose loads are in flight per thread
+#ifndef K3_ROWS_IN_FLIGHT
+#define K3_ROWS_IN_FLIGHT 8
+#endif
+#ifndef K3_MIN_CTAS
+#define K3_MIN_CTAS 2
+#endif
+#ifndef K3_STRIP_ROWS
+#define K3_STRIP_ROWS 32
+#endif
+constexpr int K3_R = K3_ROWS_IN_FLIGHT;   // rows whose loads are in flight per thread
+constexpr int K3_ENT = 12;   // floats per table entry (48 B: three 128-bit shared loads)
+constexpr int K3_TABLE_BYTES = 40 * 1024;
 
 __device__ __forceinline__ void bspline_weights(double t, double w[4]) {
     // beta3 at distances 1+t, t, 1-t, 2-t  (t in [0,1))
@@ -37,110 +57,122 @@ struct K3Args {
     const double *bcoef, *rcoef;
     float *sub, *bkg, *rms;
     uint8_t *mask;
-    int H, W, mh, mw, ny, nx, rows_per_cta;
-    double k_d;
+    int H, W, mh, mw, ny, nx, rows_per_cta, n_i0_max;
+    float k_d;
 };
 
-__global__ void __launch_bounds__(K3_NT, 2) k3_interp_subtract(K3Args a) {
-    extern __shared__ double smem_d[];
-    double *wy_tab = smem_d;                                   // [rows_per_cta][4]
-    int *j0_tab = (int *)(wy_tab + (size_t)a.rows_per_cta * 4);   // [rows_per_cta]
+// UNIFORM: mesh_w % 8 == 0, so the cell boundary (between columns mw*k + mw/2 - 1 and mw*k + mw/2) falls on a
+// multiple of 4 and the four columns of a thread lie in the same grid cell i0.
+template <bool UNIFORM>
+__global__ void __launch_bounds__(K3_NT, K3_MIN_CTAS) k3_interp_subtract(K3Args a) {
+    extern __shared__ __align__(16) float table[];   // [rows][n_i0][K3_ENT]
 
     const int frame = blockIdx.z;
     const int y_begin = blockIdx.y * a.rows_per_cta;
     const int y_end = min(y_begin + a.rows_per_cta, a.H);
-    const int x0 = (blockIdx.x * K3_NT + threadIdx.x) * K3_PX;
+    const int xc0 = blockIdx.x * K3_NT * K3_PX;
+    const int xc1 = min(xc0 + K3_NT * K3_PX, a.W) - 1;
+    const int x0 = xc0 + threadIdx.x * K3_PX;
     const size_t frame_off = (size_t)frame * a.H * a.W;
     const double *bc = a.bcoef + (size_t)frame * a.ny * a.nx;
     const double *rc = a.rcoef + (size_t)frame * a.ny * a.nx;
+    const double inv_mw = 1.0 / (double)a.mw, inv_mh = 1.0 / (double)a.mh;
+    // floor((x + 0.5)/mw - 0.5) with exact integer arithmetic: floor((2x + 1 - mw) / (2 mw))
+    auto cell_of = [](int x, int m) { int num = 2 * x + 1 - m, den = 2 * m; return num >= 0 ? num / den : -((-num + den - 1) / den); };
+    const int i0_first = cell_of(xc0, a.mw);
+    const int n_i0 = cell_of(xc1, a.mw) - i0_first + 1;
 
-    for (int r = threadIdx.x; r < y_end - y_begin; r += K3_NT) {
-        double v = ((double)(y_begin + r) + 0.5) / (double)a.mh - 0.5;
-        double fl = floor(v);
-        double w[4];
-        bspline_weights(v - fl, w);
-        wy_tab[r * 4 + 0] = w[0]; wy_tab[r * 4 + 1] = w[1]; wy_tab[r * 4 + 2] = w[2]; wy_tab[r * 4 + 3] = w[3];
-        j0_tab[r] = (int)fl;
+    // ---- table: one entry per (row, i0) --------------------------------------------------------------
+    const int n_ent = (y_end - y_begin) * n_i0;
+    for (int e = threadIdx.x; e < n_ent; e += K3_NT) {
+        const int r = e / n_i0, ii = e - r * n_i0;
+        const int y = y_begin + r, i0 = i0_first + ii;
+        const int j0 = cell_of(y, a.mh);
+        double wy[4];
+        bspline_weights(((double)y + 0.5) * inv_mh - 0.5 - (double)j0, wy);
+        double hb[4] = {0, 0, 0, 0}, hr[4] = {0, 0, 0, 0};
+#pragma unroll
+        for (int rr = 0; rr < 4; ++rr) {
+            const size_t row = (size_t)reflect_idx(j0 - 1 + rr, a.ny) * a.nx;
+#pragma unroll
+            for (int d = 0; d < 4; ++d) {
+                const int ci = reflect_idx(i0 - 1 + d, a.nx);
+                hb[d] = fma(wy[rr], __ldg(bc + row + ci), hb[d]);
+                hr[d] = fma(wy[rr], __ldg(rc + row + ci), hr[d]);
+            }
+        }
+        float *t = table + (size_t)e * K3_ENT;
+        const float hi = (float)hb[1];
+        t[0] = hi;
+        t[1] = (float)(hb[1] - (double)hi);
+        t[2] = (float)(hb[0] - hb[1]);
+        t[3] = (float)(hb[2] - hb[1]);
+        t[4] = (float)(hb[3] - hb[1]);
+        t[5] = (float)hr[0]; t[6] = (float)hr[1]; t[7] = (float)hr[2]; t[8] = (float)hr[3];
     }
     __syncthreads();
     if (x0 >= a.W) return;
 
-    // x-collapse of one grid row (reflected) for this thread's 4 columns, both grids
-    auto collapse = [&](int jrow, double gb_out[K3_PX], float gr_out[K3_PX]) {
-        const double *brow = bc + (size_t)reflect_idx(jrow, a.ny) * a.nx;
-        const double *rrow = rc + (size_t)reflect_idx(jrow, a.ny) * a.nx;
+    // ---- per-thread x weights (float64 -> float32) and table column ------------------------------------
+    float wx[K3_PX][4];
+    int ent_off[K3_PX];
 #pragma unroll
-        for (int q = 0; q < K3_PX; ++q) {
-            double u = ((double)(x0 + q) + 0.5) / (double)a.mw - 0.5;
-            double fl = floor(u);
-            int i0 = (int)fl;
-            double w[4];
-            bspline_weights(u - fl, w);
-            double sb = 0.0, sr = 0.0;
-#pragma unroll
-            for (int d = 0; d < 4; ++d) {
-                int ci = reflect_idx(i0 - 1 + d, a.nx);
-                sb = fma(w[d], __ldg(brow + ci), sb);
-                sr = fma(w[d], __ldg(rrow + ci), sr);
-            }
-            gb_out[q] = sb;
-            gr_out[q] = (float)sr;
-        }
-    };
+    for (int q = 0; q < K3_PX; ++q) {
+        const int i0 = cell_of(x0 + q, a.mw);
+        double w[4];
+        bspline_weights(((double)(x0 + q) + 0.5) * inv_mw - 0.5 - (double)i0, w);
+        wx[q][0] = (float)w[0]; wx[q][1] = (float)w[1]; wx[q][2] = (float)w[2]; wx[q][3] = (float)w[3];
+        ent_off[q] = (i0 - i0_first) * K3_ENT;
+    }
+    const int row_stride = n_i0 * K3_ENT;
 
-    double gb[4][K3_PX];
-    float gr[4][K3_PX];
-    int cur_j0 = j0_tab[0];
-#pragma unroll
-    for (int r = 0; r < 4; ++r) collapse(cur_j0 - 1 + r, gb[r], gr[r]);
-
-    const float kdf_guard = 0.0f;
+    const float *img = a.img + frame_off + x0;
     for (int yb = y_begin; yb < y_end; yb += K3_R) {
         float4 pix[K3_R];
 #pragma unroll
-        for (int r = 0; r < K3_R; ++r) {
-            int y = yb + r;
-            if (y < y_end)
-                pix[r] = __ldcs(reinterpret_cast<const float4 *>(a.img + frame_off + (size_t)y * a.W + x0));
-        }
+        for (int r = 0; r < K3_R; ++r)
+            if (yb + r < y_end) pix[r] = __ldcs(reinterpret_cast<const float4 *>(img + (size_t)(yb + r) * a.W));
 #pragma unroll
         for (int r = 0; r < K3_R; ++r) {
-            int y = yb + r;
+            const int y = yb + r;
             if (y >= y_end) break;
-            int j0 = j0_tab[y - y_begin];
-            if (j0 != cur_j0) {   // uniform over the CTA: entered a new mesh row, slide the 4-row window
-#pragma unroll
-                for (int q = 0; q < K3_PX; ++q) {
-                    gb[0][q] = gb[1][q]; gb[1][q] = gb[2][q]; gb[2][q] = gb[3][q];
-                    gr[0][q] = gr[1][q]; gr[1][q] = gr[2][q]; gr[2][q] = gr[3][q];
-                }
-                cur_j0 = j0;
-                collapse(cur_j0 + 2, gb[3], gr[3]);
-            }
-            const double4 wy01 = *reinterpret_cast<const double4 *>(wy_tab + (size_t)(y - y_begin) * 4);
-            const double wy[4] = {wy01.x, wy01.y, wy01.z, wy01.w};
-            const float wyf[4] = {(float)wy01.x, (float)wy01.y, (float)wy01.z, (float)wy01.w};
+            const float *trow = table + (size_t)(y - y_begin) * row_stride;
             const float in[4] = {pix[r].x, pix[r].y, pix[r].z, pix[r].w};
             float o_sub[4], o_bkg[4], o_rms[4];
             uint32_t mbits = 0;
+            float4 t0, t1;
+            float t8;
+            if (UNIFORM) {
+                const float *t = trow + ent_off[0];
+                t0 = *reinterpret_cast<const float4 *>(t);
+                t1 = *reinterpret_cast<const float4 *>(t + 4);
+                t8 = t[8];
+            }
 #pragma unroll
             for (int q = 0; q < K3_PX; ++q) {
-                double b = wy[0] * gb[0][q];
-                b = fma(wy[1], gb[1][q], b);
-                b = fma(wy[2], gb[2][q], b);
-                b = fma(wy[3], gb[3][q], b);
-                float s = wyf[0] * gr[0][q];
-                s = fmaf(wyf[1], gr[1][q], s);
-                s = fmaf(wyf[2], gr[2][q], s);
-                s = fmaf(wyf[3], gr[3][q], s);
-                double d = (double)in[q] - b;
-                o_sub[q] = (float)d;
-                o_bkg[q] = (float)b;
+                if (!UNIFORM) {
+                    const float *t = trow + ent_off[q];
+                    t0 = *reinterpret_cast<const float4 *>(t);
+                    t1 = *reinterpret_cast<const float4 *>(t + 4);
+                    t8 = t[8];
+                }
+                // t0 = {hi, lo, e_-1, e_+1}, t1 = {e_+2, r_-1, r_0, r_+1}, t8 = r_+2
+                float rel = wx[q][0] * t0.z;
+                rel = fmaf(wx[q][2], t0.w, rel);
+                rel = fmaf(wx[q][3], t1.x, rel);
+                rel += t0.y;
+                float s = wx[q][0] * t1.y;
+                s = fmaf(wx[q][1], t1.z, s);
+                s = fmaf(wx[q][2], t1.w, s);
+                s = fmaf(wx[q][3], t8, s);
+                const float d = (in[q] - t0.x) - rel;
+                o_sub[q] = d;
+                o_bkg[q] = t0.x + rel;
                 o_rms[q] = s;
-                bool fg = (s > kdf_guard) && (d > a.k_d * (double)s);
+                const bool fg = (s > 0.0f) && (d > a.k_d * s);
                 mbits |= (fg ? 1u : 0u) << (8 * q);
             }
-            size_t off = frame_off + (size_t)y * a.W + x0;
+            const size_t off = frame_off + (size_t)y * a.W + x0;
             __stcs(reinterpret_cast<float4 *>(a.sub + off), make_float4(o_sub[0], o_sub[1], o_sub[2], o_sub[3]));
             if (a.bkg) __stcs(reinterpret_cast<float4 *>(a.bkg + off), make_float4(o_bkg[0], o_bkg[1], o_bkg[2], o_bkg[3]));
             if (a.rms) __stcs(reinterpret_cast<float4 *>(a.rms + off), make_float4(o_rms[0], o_rms[1], o_rms[2], o_rms[3]));
@@ -159,19 +191,21 @@ int k3_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, int mh, int 
     a.sub = d_sub; a.bkg = d_bkg; a.rms = d_rms; a.mask = d_mask;
     a.H = H; a.W = W; a.mh = mh; a.mw = mw;
     a.ny = (H + mh - 1) / mh; a.nx = (W + mw - 1) / mw;
-    a.k_d = detect_k;
-    // rows per CTA: aim for >= 8 CTAs per SM over the launch so the tail is short, but keep strips long
-    // enough (>= 16 rows) that the 16 collapse FMAs/px at the strip start are amortised.
-    int col_blocks = (W + K3_NT * K3_PX - 1) / (K3_NT * K3_PX);
-    long want_ctas = (long)ctx->num_sms * 16;
-    int rows = (int)(((long)H * col_blocks * B + want_ctas - 1) / want_ctas);
-    rows = (rows + K3_R - 1) / K3_R * K3_R;
-    if (rows < 16) rows = 16;
-    if (rows > 128) rows = 128;
+    a.k_d = (float)detect_k;
+    const int cols = K3_NT * K3_PX;
+    const int col_blocks = (W + cols - 1) / cols;
+    // grid cells a 1024-column strip can touch; the table (rows x cells x 48 B) bounds the strip height
+    a.n_i0_max = (cols < W ? cols : W) / mw + 2;
+    int rows = K3_TABLE_BYTES / (a.n_i0_max * K3_ENT * (int)sizeof(float));
+    if (rows > K3_STRIP_ROWS) rows = K3_STRIP_ROWS;
+    if (rows >= K3_R) rows = rows / K3_R * K3_R;
+    if (rows < 1) return bd_set_error(ctx, BD_EUNSUPPORTED, "mesh width %d too small for the interpolation kernel", mw);
+    if (rows > H) rows = H;
     a.rows_per_cta = rows;
     dim3 grid(col_blocks, (H + rows - 1) / rows, B);
-    size_t smem = (size_t)rows * 4 * sizeof(double) + (size_t)rows * sizeof(int);
-    k3_interp_subtract<<<grid, K3_NT, smem, st>>>(a);
+    size_t smem = (size_t)rows * a.n_i0_max * K3_ENT * sizeof(float);
+    if (mw % 8 == 0) k3_interp_subtract<true><<<grid, K3_NT, smem, st>>>(a);
+    else k3_interp_subtract<false><<<grid, K3_NT, smem, st>>>(a);
     BD_CUDA_CHECK(ctx, cudaGetLastError());
     return BD_OK;
 }
