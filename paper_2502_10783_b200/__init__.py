@@ -126,6 +126,19 @@ class Context:
         return n.value
 
 
+def k1_slow_meshes(ctx: "Context", reset: bool = True) -> int:
+    """Diagnostics: meshes that went through K1's general (slow) path since the last reset (synchronises)."""
+    n = C.c_ulonglong()
+    torch.cuda.synchronize()
+    ctx.check(ctx.lib.bd_debug_k1_slow_meshes(C.byref(n), C.c_int(1 if reset else 0)))
+    return n.value
+
+
+def k1_force_slow(ctx: "Context", on: bool) -> None:
+    """Diagnostics: make K1 skip its fast path (the tests exercise both paths)."""
+    ctx.check(ctx.lib.bd_debug_k1_force_slow(ctx.h, C.c_int(1 if on else 0)))
+
+
 def _dev(ctx):
     return torch.device("cuda", ctx.device)
 

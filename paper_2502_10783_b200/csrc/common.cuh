@@ -13,6 +13,7 @@ struct bd_ctx {
     int num_sms;
     size_t smem_optin;
     char err[512];
+    int k1_force_slow;   // diagnostics: K1 skips its fast path
     // cuTensorMapEncodeTiled, fetched through the runtime (no -lcuda link dependency)
     CUresult (*encode_tiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                              const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
@@ -44,6 +45,7 @@ struct K1Plan {
     int threads;        // threads per CTA
     size_t smem_bytes;  // dynamic shared memory per CTA
     int use_tma;
+    int tailcap;        // capacity of the tail-pixel list (team total)
 };
 int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan);
 int k1_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg_params *p, double *d_bkg_raw,

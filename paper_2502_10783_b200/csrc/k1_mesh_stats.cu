@@ -5,25 +5,29 @@
 //
 // The paper gives one GPU *thread* per sub-region.  Here a mesh is owned by a team of C CTAs (a
 // thread-block cluster; C = 1 when the mesh fits one CTA's shared memory): each CTA stages a slab of the
-// mesh's rows in shared memory with one TMA bulk-tensor load, and every later sweep reads shared memory
-// only, so HBM sees each pixel once (4 B/px).
+// mesh's rows in shared memory with one TMA bulk-tensor load, so HBM sees each pixel once (4 B/px).
 //
-// Structure of the clipping loop.  The survivors of every round are the pixels in a value interval
-// [LO, HI] (LO = max of the lower bounds so far, HI = min of the upper bounds).  A round therefore needs
-//   (1) one sweep for n, sum(x-p), sum((x-p)^2) over [LO, HI] and the count below LO -- float64 sums
-//       against float64 bounds, so the survivor set is the float64 definition's; and
-//   (2) the order statistics n_below + (n-1)/2 and n_below + n/2 of the WHOLE mesh.
-// (2) is a radix select on order-preserving uint32 keys that avoids per-pixel shared-memory atomics
-// (measured: ~1 atomic/clk/SM, which made the first version of this kernel 2.1 ms on a 9216x9232 frame):
-//   * the median of a set lies within one (population) standard deviation of its mean, so the search
-//     starts from the key range of [mean - sd, mean + sd];
-//   * each refinement level histograms that range into <= 64 bins with PER-THREAD byte counters in shared
-//     memory (plain load/add/store, bank-conflict free), reduced with dp4a; it descends into the bin that
-//     holds the wanted rank until that bin has <= 512 pixels (or is a single key);
-//   * the pixels of a window of bins around it (<= 1024 pixels) are gathered, shared by the team, and
-//     counting-sorted once; every later round's median is then a table lookup, because later medians move
-//     by a fraction of sigma.  A rank that falls outside the window rebuilds the window.
-// Team-wide values go through distributed shared memory; with C = 1 everything is CTA-local.
+// What the clipping loop needs.  The survivors of every round are the pixels in a value interval [LO, HI]
+// (LO = max of the lower bounds so far, HI = min of the upper bounds).  A round needs (1) n, sum(x-p),
+// sum((x-p)^2) over [LO, HI] and the count below LO -- float64 sums against float64 bounds, so the survivor
+// set is the float64 definition's -- and (2) two order statistics of the WHOLE mesh.
+//
+// Fast path (two sweeps of the slab, whatever the number of rounds).  While the TMA load is in flight every
+// CTA reads the same small lattice sample of the mesh from global memory and sorts it (bitonic).  Sample
+// quantiles give a key bracket [ka, kb] that contains the median rank and a conservative core interval
+// [A, B] = q50 -+ c*(q50 - q16) that every clipping bound of the paper's loop stays outside of.
+//   sweep 1: float64 core sums over [A, B]; count of "tail" pixels outside it; a 64-bin histogram of the
+//            bracket with PER-THREAD byte counters (plain load/add/store: no shared-memory atomics, which
+//            run at ~1/clk/SM), reduced with dp4a; team-wide totals through distributed shared memory;
+//   sweep 2: gather the pixels of a window of bins around the median rank (<= 2048) and the tail pixels.
+// Rank 0 of the team collects both lists through DSMEM, the other CTAs exit.  It sorts the window once
+// (every round's median is then a table lookup) and runs the rounds on the tail list alone:
+//   n = n_core + #tail in [lo, hi],  sums = core sums + tail sums.
+// Any assumption that fails (bound enters the core, median rank leaves the window, tail list overflow,
+// degenerate sample) sends the mesh to the
+// Slow path (general, one CTA): a sweep per round plus a radix select that descends 64-bin histograms from
+// the key range of [mean - sd, mean + sd] (the median lies within one standard deviation of the mean).
+// It reads the slab from shared memory when C = 1 and the mesh from global memory (L2) otherwise.
 #include <cooperative_groups.h>
 
 #include "common.cuh"
@@ -32,17 +36,21 @@ namespace cg = cooperative_groups;
 
 namespace {
 
-constexpr int K1_NBIN = 64;        // bins per refinement level
-constexpr int K1_T1 = 512;         // stop refining when the target bin holds <= this many pixels
-constexpr int K1_LISTCAP = 1024;   // candidate window capacity (team total)
-constexpr int K1_FB = 1024;        // fine bins of the candidate counting sort
+constexpr int K1_NBIN = 64;        // histogram bins per level
+constexpr int K1_T1 = 512;         // slow path: stop refining when the target bin holds <= this many pixels
+constexpr int K1_LISTCAP = 2048;   // candidate window capacity (team total)
 constexpr int K1_MAXWARPS = 16;
 constexpr int K1_MAXC = 8;
+constexpr int K1_FAST_MIN_PX = 8192;   // below this the fixed costs of the fast path exceed the sweeps it saves
+                                       // (and the dead slab must hold the 12 KiB of sort arrays)
+
+__device__ unsigned long long g_k1_slow_meshes;   // diagnostic: meshes that took the slow path
+__device__ unsigned long long g_k1_reason[8];     // diagnostic: why (1 sample, 2 tails, 3 rank/bin, 4 window, 5 round window, 6 bound)
 
 struct K1Args {
     const float *img;
     int B, H, W, mh, mw, ny, nx;
-    int slab_rows, use_tma;
+    int slab_rows, use_tma, tailcap, allow_fast;
     double k_c;
     int iters, skew_guard;
     double median_factor, mean_factor;
@@ -50,30 +58,31 @@ struct K1Args {
     int32_t *n_kept;
 };
 
-struct Xch {   // one CTA's contribution to a team-wide reduction
+struct Xch {   // one CTA's contribution to the team-wide totals (peers read it through DSMEM)
     double s1, s2;
-    int n_in, n_below;
-    uint32_t below, m, nextkey, pad;
+    int n_core, n_tail;
+    uint32_t below, m_cand, m_tail, pad;
     uint32_t cnt[K1_NBIN];
+};
+
+struct SampleX {   // one CTA's sample statistics (peers read them through DSMEM)
+    double q50, q16;
+    double lo3, hi3;     // sample quantiles 3 standard deviations either side of 0.5 (averaged over a team of >= 4)
+    uint32_t ka, kb;     // keys of the quantiles 6 standard deviations either side (used as they are otherwise)
+    int valid, pad;
 };
 
 struct Smem {   // fixed-size part of shared memory; follows the slab
     alignas(16) unsigned long long mbar;
-    Xch xch[2];
+    SampleX sx;
+    Xch xch;
     Xch tot;
     double red_d[2][K1_MAXWARPS];
     int red_i[2][K1_MAXWARPS];
     uint32_t red_u[K1_MAXWARPS];
     uint32_t win_b0, win_b1;
-    uint32_t cand_local[K1_LISTCAP];   // this CTA's candidates (peers read it through DSMEM)
-    uint32_t list[K1_LISTCAP];         // the team's candidates
-    // the union area (per-thread byte histograms during refinement; sort arrays afterwards) follows
-};
-
-struct SortArea {
-    uint32_t sorted[K1_LISTCAP];
-    uint32_t fcur[K1_FB];
-    uint32_t fstart[K1_FB + 1];
+    uint32_t list[K1_LISTCAP];   // candidate keys: this CTA's during the gather; the team's (sorted) at rank 0
+    // the work area follows: sample keys -> per-thread byte histograms -> tail pixels
 };
 
 template <int C>
@@ -107,8 +116,20 @@ __device__ void block_reduce_stats(Smem &s, double &s1, double &s2, int &n_in, i
     }
     if (lane == 0) { s.red_d[0][warp] = s1; s.red_d[1][warp] = s2; s.red_i[0][warp] = n_in; s.red_i[1][warp] = n_below; }
     __syncthreads();
-    s1 = 0; s2 = 0; n_in = 0; n_below = 0;
-    for (int w = 0; w < nw; ++w) { s1 += s.red_d[0][w]; s2 += s.red_d[1][w]; n_in += s.red_i[0][w]; n_below += s.red_i[1][w]; }
+    if (warp == 0) {   // nw <= 16 partials: one more shuffle tree, in a fixed order
+        s1 = lane < nw ? s.red_d[0][lane] : 0.0; s2 = lane < nw ? s.red_d[1][lane] : 0.0;
+        n_in = lane < nw ? s.red_i[0][lane] : 0; n_below = lane < nw ? s.red_i[1][lane] : 0;
+#pragma unroll
+        for (int o = 8; o; o >>= 1) {
+            s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+            s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+            n_in += __shfl_xor_sync(0xffffffffu, n_in, o);
+            n_below += __shfl_xor_sync(0xffffffffu, n_below, o);
+        }
+        if (lane == 0) { s.red_d[0][0] = s1; s.red_d[1][0] = s2; s.red_i[0][0] = n_in; s.red_i[1][0] = n_below; }
+    }
+    __syncthreads();
+    s1 = s.red_d[0][0]; s2 = s.red_d[1][0]; n_in = s.red_i[0][0]; n_below = s.red_i[1][0];
     __syncthreads();
 }
 
@@ -128,155 +149,221 @@ __device__ uint32_t block_reduce_u32(Smem &s, uint32_t v) {   // MIN ? min : sum
     return v;
 }
 
-// Team-wide combine.  `mine` holds this CTA's block-reduced scalars (same value in all threads); cnt[] is
-// taken from s.xch[slot].cnt, which the caller filled before (when with_cnt).  Sums everything over the team
-// in rank order (every CTA computes the same bits), min for nextkey.  Result in s.tot (valid after return).
-// phase alternates the exchange slot so a fast CTA's next write cannot overtake a slow CTA's read.
-template <int C>
-__device__ void team_combine(Smem &s, const Xch &mine, int &phase, bool with_cnt) {
-    Xch *slot = &s.xch[phase & 1];
-    if constexpr (C == 1) {
-        __syncthreads();   // every thread is done with the previous s.tot
-        if (threadIdx.x == 0) {
-            s.tot.s1 = mine.s1; s.tot.s2 = mine.s2; s.tot.n_in = mine.n_in; s.tot.n_below = mine.n_below;
-            s.tot.below = mine.below; s.tot.m = mine.m; s.tot.nextkey = mine.nextkey;
-        }
-        if (with_cnt && threadIdx.x < K1_NBIN) s.tot.cnt[threadIdx.x] = slot->cnt[threadIdx.x];
-        __syncthreads();
-        ++phase;
-        return;
+// exclusive block scan of v; returns this thread's offset, total in `total`
+__device__ uint32_t block_scan_excl(Smem &s, uint32_t v, uint32_t &total) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    uint32_t incl = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
     }
-    if (threadIdx.x == 0) {
-        slot->s1 = mine.s1; slot->s2 = mine.s2; slot->n_in = mine.n_in; slot->n_below = mine.n_below;
-        slot->below = mine.below; slot->m = mine.m; slot->nextkey = mine.nextkey;
-    }
-    Team<C>::sync();
-    if (threadIdx.x == 0) {
-        double s1 = 0, s2 = 0;
-        int n_in = 0, n_below = 0;
-        uint32_t below = 0, m = 0, nk = 0xFFFFFFFFu;
-        for (unsigned r = 0; r < (unsigned)C; ++r) {
-            const Xch *o = Team<C>::remote(slot, r);
-            s1 += o->s1; s2 += o->s2; n_in += o->n_in; n_below += o->n_below;
-            below += o->below; m += o->m; nk = min(nk, o->nextkey);
-        }
-        s.tot.s1 = s1; s.tot.s2 = s2; s.tot.n_in = n_in; s.tot.n_below = n_below;
-        s.tot.below = below; s.tot.m = m; s.tot.nextkey = nk;
-    }
-    if (with_cnt && threadIdx.x >= 32 && threadIdx.x < 32 + K1_NBIN) {
-        const int b = threadIdx.x - 32;
-        uint32_t t = 0;
-        for (unsigned r = 0; r < (unsigned)C; ++r) t += Team<C>::remote(slot, r)->cnt[b];
-        s.tot.cnt[b] = t;
-    }
+    if (lane == 31) s.red_u[warp] = incl;
     __syncthreads();
-    ++phase;
+    uint32_t base = 0;
+    total = 0;
+    for (int w = 0; w < nw; ++w) { if (w < warp) base += s.red_u[w]; total += s.red_u[w]; }
+    __syncthreads();
+    return base + incl - v;
 }
 
-template <int C>
-__global__ void k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a) {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    float *slab = reinterpret_cast<float *>(smem_raw);   // [slab_rows * mw], 128-B aligned for TMA
-    const size_t slab_bytes = ((size_t)a.slab_rows * a.mw * sizeof(float) + 127) & ~(size_t)127;
-    Smem &s = *reinterpret_cast<Smem *>(smem_raw + slab_bytes);
-    unsigned char *area = smem_raw + slab_bytes + ((sizeof(Smem) + 127) & ~(size_t)127);
-    uint8_t *hist8 = area;                                   // [K1_NBIN][nt] byte counters
-    SortArea &srt = *reinterpret_cast<SortArea *>(area);     // aliases hist8 (used after the gather)
-
-    const unsigned rank = Team<C>::rank();
-    const int mesh = blockIdx.x / C;
-    const int frame = mesh / (a.ny * a.nx);
-    const int mj = (mesh / a.nx) % a.ny, mi = mesh % a.nx;
-    const int y0 = mj * a.mh, x0 = mi * a.mw;
-    const int vh = min(a.mh, a.H - y0), vw = min(a.mw, a.W - x0);       // valid part of the mesh
-    const int row0 = (int)rank * a.slab_rows;                           // first mesh row of this CTA's slab
-    const int my_rows = max(0, min(a.slab_rows, vh - row0));
-    const int n_c = my_rows * vw;                                       // valid pixels in this slab, a prefix
-    const int n_tot = vh * vw;
-    const float *frame_ptr = a.img + (size_t)frame * a.H * a.W;
-    const int tid = threadIdx.x, nt = blockDim.x;
-    const int lane = tid & 31;
-
-    // ---- stage the slab ---------------------------------------------------------------------------------
-    const bool tma = a.use_tma && vw == a.mw;
-    if (tma && tid == 0) {
-        uint32_t bar = smem_u32(&s.mbar);
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        uint32_t bytes = (uint32_t)((size_t)a.slab_rows * a.mw * sizeof(float));
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-        // rows past H are zero-filled by TMA; they lie beyond the n_c prefix and are never read
-        asm volatile(
-            "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes"
-            " [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(smem_u32(slab)),
-            "l"(&tmap), "r"(x0), "r"(y0 + row0), "r"(frame), "r"(bar)
-            : "memory");
+// in-place ascending bitonic sort of a[0..n), n a power of two; all threads of the CTA call it
+__device__ void bitonic_sort(uint32_t *a, int n) {
+    for (int k = 2; k <= n; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int t = threadIdx.x; t < (n >> 1); t += blockDim.x) {
+                const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));   // index with bit j clear
+                const int p = i | j;
+                const uint32_t x = a[i], y = a[p];
+                const bool up = (i & k) == 0;
+                if ((x > y) == up) { a[i] = y; a[p] = x; }
+            }
+            __syncthreads();
+        }
     }
-    // pivot of the round-0 sums: median of five pixels of the mesh (uniform over the team; a robust centre
-    // keeps the one-pass variance accurate even when some of the five are outliers)
+}
+
+// reduce the per-thread byte columns hist8[bin][thread] to per-bin totals out[bin] (needs nt % 64 == 0)
+__device__ void reduce_byte_hist(const uint8_t *hist8, int nt, uint32_t *out) {
+    const int tid = threadIdx.x;
+    const int G = nt / K1_NBIN, b = tid / G, g = tid - b * G;   // G threads per bin, nt/4 words per bin
+    const uint32_t *row = reinterpret_cast<const uint32_t *>(hist8) + (size_t)b * (nt / 4);
+    uint32_t acc = 0;
+#pragma unroll
+    for (int j = 0; j < 16; ++j) acc = __dp4a(row[j * G + g], 0x01010101u, acc);
+    for (int o = G >> 1; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (g == 0) out[b] = acc;
+}
+
+// Which bin of cnt[0..64) holds 0-based rank r (r < sum cnt)?  Every warp computes it redundantly (lane l owns
+// bins 2l, 2l+1).  Returns false if r is not covered.  `excl0`/`c0`/`c1` are left for prefix queries.
+struct BinHit { uint32_t b, pre, cnt; uint32_t excl, c0, c1; };
+__device__ bool locate_bin(const uint32_t *cnt, uint32_t r, BinHit &h) {
+    const int lane = threadIdx.x & 31;
+    const uint32_t c0 = cnt[2 * lane], c1 = cnt[2 * lane + 1];
+    uint32_t incl = c0 + c1;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    const uint32_t excl = incl - c0 - c1;
+    const bool mine0 = r >= excl && r < excl + c0, mine1 = r >= excl + c0 && r < incl;
+    const uint32_t bal = __ballot_sync(0xffffffffu, mine0 || mine1);
+    h.excl = excl; h.c0 = c0; h.c1 = c1;
+    if (bal == 0) return false;
+    const int src = __ffs(bal) - 1;
+    h.b = __shfl_sync(0xffffffffu, 2 * lane + (mine1 ? 1 : 0), src);
+    h.pre = __shfl_sync(0xffffffffu, mine1 ? excl + c0 : excl, src);
+    h.cnt = __shfl_sync(0xffffffffu, mine1 ? c1 : c0, src);
+    return true;
+}
+// exclusive prefix of bin b, from the registers locate_bin left
+__device__ __forceinline__ uint32_t bin_prefix(const BinHit &h, uint32_t b) {
+    const int lane = threadIdx.x & 31;
+    return __shfl_sync(0xffffffffu, (b & 1) ? h.excl + h.c0 : h.excl, (int)(b >> 1));
+}
+
+// thread 0: grow a window of bins around b while it holds <= K1_LISTCAP pixels
+__device__ void grow_window(Smem &s, const uint32_t *cnt, int nb, uint32_t b, uint32_t cntb) {
+    int b0 = (int)b, b1 = (int)b;
+    uint32_t tot = cntb;
+    // later rounds clip mostly positive outliers (sources, hot pixels), which moves the median rank DOWN:
+    // two bins on the low side for every bin on the high side
+    for (int g = 0; g < K1_NBIN; ++g) {
+        bool grew = false;
+        for (int rep = 0; rep < 2; ++rep)
+            if (b0 - 1 >= 0 && tot + cnt[b0 - 1] <= (uint32_t)K1_LISTCAP) { --b0; tot += cnt[b0]; grew = true; }
+        if (b1 + 1 < nb && tot + cnt[b1 + 1] <= (uint32_t)K1_LISTCAP) { ++b1; tot += cnt[b1]; grew = true; }
+        if (!grew) break;
+    }
+    s.win_b0 = b0; s.win_b1 = b1;
+}
+
+// Counting sort of the candidate keys list[0..m) (all in [kga, kga + gspan]) into sorted[0..m): K1_FB fine bins
+// by key, shared-memory atomics on m <= 2048 elements only, then an insertion sort inside the (tiny) bins that
+// hold more than one key.  fcur is scratch [K1_FB].
+constexpr int K1_FB = 1024;
+struct SortArea {
+    uint32_t sorted[K1_LISTCAP];
+    uint32_t fcur[K1_FB];
+};
+__device__ void sort_candidates(Smem &s, const uint32_t *list, uint32_t m, uint32_t kga, uint32_t gspan, SortArea &srt) {
+    const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31;
+    int fshift = 0;
+    while ((gspan >> fshift) >= (uint32_t)K1_FB) ++fshift;
+    const int nfb = (int)(gspan >> fshift) + 1;
+    for (int i = tid; i < nfb; i += nt) srt.fcur[i] = 0;
+    __syncthreads();
+    for (uint32_t i = tid; i < m; i += nt) atomicAdd(&srt.fcur[(list[i] - kga) >> fshift], 1u);
+    __syncthreads();
+    {   // exclusive scan of fcur[0..nfb), in place
+        const int per = (nfb + nt - 1) / nt, f0 = tid * per;
+        uint32_t local = 0;
+        for (int k = 0; k < per; ++k) if (f0 + k < nfb) local += srt.fcur[f0 + k];
+        uint32_t inc = local;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) s.red_u[tid >> 5] = inc;
+        __syncthreads();
+        uint32_t run = inc - local;
+        for (int w = 0; w < (tid >> 5); ++w) run += s.red_u[w];
+        for (int k = 0; k < per; ++k) {
+            if (f0 + k >= nfb) break;
+            const uint32_t c = srt.fcur[f0 + k];
+            srt.fcur[f0 + k] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+    for (uint32_t i = tid; i < m; i += nt) {
+        const uint32_t k = list[i];
+        srt.sorted[atomicAdd(&srt.fcur[(k - kga) >> fshift], 1u)] = k;
+    }
+    __syncthreads();
+    if (fshift > 0) {   // fcur[f] is now the end of bin f = the start of bin f + 1
+        for (int f = tid; f < nfb; f += nt) {
+            const uint32_t lo = f ? srt.fcur[f - 1] : 0u, hi = srt.fcur[f];
+            for (uint32_t i = lo + 1; i < hi; ++i) {
+                const uint32_t k = srt.sorted[i];
+                uint32_t j = i;
+                while (j > lo && srt.sorted[j - 1] > k) { srt.sorted[j] = srt.sorted[j - 1]; --j; }
+                srt.sorted[j] = k;
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// ---- pixel source of the slow path: the slab in shared memory (C = 1) or the mesh in global memory ---------
+struct MeshSrc {
+    const float *slab;   // non-null: n_slab valid pixels packed (TMA rows are full width, so packed) in shared memory
+    int n_slab;
+    const float *g;      // else: top-left pixel of the mesh in global memory, row pitch W
+    int W, vh, vw;
+    bool vec4;           // rows of g are 16-byte aligned and vw % 4 == 0
+};
+
+// Apply f(float) to every pixel of the mesh.  The assignment of pixels to threads is the same on every call
+// (the per-thread byte histograms rely on that).
+template <typename F>
+__device__ __forceinline__ void for_each_px(const MeshSrc &m, F f) {
+    const int tid = threadIdx.x, nt = blockDim.x;
+    if (m.slab) {
+        const float4 *s4 = reinterpret_cast<const float4 *>(m.slab);
+        const int n4 = m.n_slab >> 2, n_tail = m.n_slab & 3;
+        for (int i = tid; i < n4; i += nt) {
+            const float4 v = s4[i];
+            f(v.x); f(v.y); f(v.z); f(v.w);
+        }
+        if (tid < n_tail) f(m.slab[(n4 << 2) + tid]);
+    } else {
+        const int lane = tid & 31, warp = tid >> 5, nw = nt >> 5;
+        for (int r = warp; r < m.vh; r += nw) {
+            const float *row = m.g + (size_t)r * m.W;
+            if (m.vec4) {
+                for (int c = lane * 4; c < m.vw; c += 128) {
+                    const float4 v = __ldg(reinterpret_cast<const float4 *>(row + c));
+                    f(v.x); f(v.y); f(v.z); f(v.w);
+                }
+            } else {
+                for (int c = lane; c < m.vw; c += 32) f(__ldg(row + c));
+            }
+        }
+    }
+}
+
+// ---- slow path: one CTA, general -------------------------------------------------------------------------
+// Leaves the final statistics of the survivors in med/mu/sd/n.
+__device__ __noinline__ void k1_slow_path(const MeshSrc &src, Smem &s, uint8_t *hist8, int n_tot, double k_c, int iters,
+                                          double &med, double &mu, double &sd, int &n_out) {
+    const int tid = threadIdx.x, nt = blockDim.x;
+    SortArea &srt = *reinterpret_cast<SortArea *>(hist8);
+    // pivot of the round-0 sums: any pixel of the mesh would do for correctness; take the mean of a few
     double pivot;
     {
-        const int ys[5] = {0, 0, vh - 1, vh - 1, vh / 2}, xs[5] = {0, vw - 1, 0, vw - 1, vw / 2};
-        float v[5];
-#pragma unroll
-        for (int k = 0; k < 5; ++k) v[k] = __ldg(frame_ptr + (size_t)(y0 + ys[k]) * a.W + x0 + xs[k]);
-#define K1_CE(i, j) { float lo_ = fminf(v[i], v[j]), hi_ = fmaxf(v[i], v[j]); v[i] = lo_; v[j] = hi_; }
-        K1_CE(0, 1) K1_CE(3, 4) K1_CE(2, 4) K1_CE(2, 3) K1_CE(0, 3) K1_CE(0, 2) K1_CE(1, 4) K1_CE(1, 3) K1_CE(1, 2)
-#undef K1_CE
-        pivot = (double)v[2];
+        double t1 = 0;
+        int c = 0, z = 0;
+        double z2 = 0;
+        for_each_px(src, [&](float e) { t1 += (double)e; ++c; });
+        block_reduce_stats(s, t1, z2, c, z);
+        pivot = t1 / (double)n_tot;
     }
-    if (tma) {
-        __syncthreads();
-        uint32_t bar = smem_u32(&s.mbar), done = 0;
-        while (!done) {
-            asm volatile(
-                "{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
-                : "=r"(done)
-                : "r"(bar)
-                : "memory");
-        }
-    } else {   // plain loader: valid pixels packed row-major
-        for (int i = tid; i < n_c; i += nt) {
-            int r = i / vw, c = i - r * vw;
-            slab[i] = frame_ptr[(size_t)(y0 + row0 + r) * a.W + x0 + c];
-        }
-        __syncthreads();
-    }
-
-    const float4 *slab4 = reinterpret_cast<const float4 *>(slab);
-    const int n4 = n_c >> 2, n_tail = n_c & 3;
-    int phase = 0;
-
-    // every sweep: whole float4s without per-element bounds checks, then the <= 3 tail pixels
-#define K1_SWEEP(BODY)                                                   \
-    {                                                                    \
-        for (int i_ = tid; i_ < n4; i_ += nt) {                          \
-            const float4 v_ = slab4[i_];                                 \
-            { const float e = v_.x; BODY }                               \
-            { const float e = v_.y; BODY }                               \
-            { const float e = v_.z; BODY }                               \
-            { const float e = v_.w; BODY }                               \
-        }                                                                \
-        if (tid < n_tail) { const float e = slab[(n4 << 2) + tid]; BODY }\
-    }
-
-    // ---- sweep A: round-0 sums about the pivot -------------------------------------------------------------
     double s1, s2;
     {
         double t1 = 0, t2 = 0;
-        K1_SWEEP({ const double d = (double)e - pivot; t1 += d; t2 = fma(d, d, t2); })
         int z0 = 0, z1 = 0;
+        for_each_px(src, [&](float e) { const double d = (double)e - pivot; t1 += d; t2 = fma(d, d, t2); });
         block_reduce_stats(s, t1, t2, z0, z1);
-        Xch mine; mine.s1 = t1; mine.s2 = t2; mine.n_in = 0; mine.n_below = 0; mine.below = 0; mine.m = 0; mine.nextkey = 0;
-        team_combine<C>(s, mine, phase, false);
-        s1 = s.tot.s1; s2 = s.tot.s2;
-        __syncthreads();
+        s1 = t1; s2 = t2;
     }
 
-    // ---- candidate window state (uniform over the team) ---------------------------------------------------
-    int mode = 0;                 // 0 none, 1 sorted list, 2 single key
-    uint32_t list_off = 0, list_m = 0;             // mode 1: ranks [list_off, list_off + list_m) are srt.sorted[]
-    uint32_t sel_key = 0, sel_lo = 0, sel_hi = 0;  // mode 2: ranks [sel_lo, sel_hi) all have key sel_key
+    int mode = 0;                                   // 0 none, 1 sorted list, 2 single key
+    uint32_t list_off = 0, list_m = 0;              // mode 1: ranks [list_off, list_off + list_m) are srt.sorted[]
+    uint32_t sel_key = 0, sel_lo = 0, sel_hi = 0;   // mode 2: ranks [sel_lo, sel_hi) all have key sel_key
 
     // Build the window for 0-based rank `want` of the whole mesh, searching keys [ka, kb] (must contain it).
     auto build = [&](uint32_t want, uint32_t ka, uint32_t kb) {
@@ -286,171 +373,56 @@ __global__ void k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a
             const uint32_t span = kb - ka;
             int shift = 0;
             while ((span >> shift) >= (uint32_t)K1_NBIN) ++shift;
-            // -- per-thread byte histogram of the keys in [ka, kb]
             for (int i = tid; i < (K1_NBIN * nt) / 16; i += nt) reinterpret_cast<uint4 *>(hist8)[i] = make_uint4(0, 0, 0, 0);
             __syncthreads();
             uint32_t below = 0;
             uint8_t *col = hist8 + tid;
-            K1_SWEEP({
+            for_each_px(src, [&](float e) {
                 const uint32_t k = f32_to_key(e);
                 const uint32_t t = k - ka;
                 if (t <= span) col[(t >> shift) * nt] += 1;
                 else if (top && k < ka) ++below;
-            })
+            });
             __syncthreads();
-            // -- reduce the byte columns: G = nt/64 threads per bin, 16 words each, dp4a
-            {
-                const int G = nt / K1_NBIN, b = tid / G, g = tid - b * G;
-                const uint32_t *row = reinterpret_cast<const uint32_t *>(hist8) + (size_t)b * (nt / 4);
-                uint32_t acc = 0;
-#pragma unroll
-                for (int j = 0; j < 16; ++j) acc = __dp4a(row[j * G + g], 0x01010101u, acc);
-                for (int o = G >> 1; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-                if (g == 0) s.xch[phase & 1].cnt[b] = acc;
-            }
-            if (top) below = block_reduce_u32<false>(s, below);
+            reduce_byte_hist(hist8, nt, s.tot.cnt);
+            if (top) { below = block_reduce_u32<false>(s, below); off = below; }
             else __syncthreads();
-            Xch mine; mine.s1 = 0; mine.s2 = 0; mine.n_in = 0; mine.n_below = 0; mine.below = below; mine.m = 0; mine.nextkey = 0;
-            team_combine<C>(s, mine, phase, true);
-            if (top) off = s.tot.below;
             top = false;
-            // -- locate the bin of `want` (every warp redundantly: lane l owns bins 2l, 2l+1)
-            const uint32_t c0 = s.tot.cnt[2 * lane], c1 = s.tot.cnt[2 * lane + 1];
-            uint32_t incl = c0 + c1;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
-                if (lane >= o) incl += t;
-            }
-            const uint32_t excl = incl - c0 - c1;
-            const uint32_t r = want - off;
-            const bool mine0 = r >= excl && r < excl + c0, mine1 = r >= excl + c0 && r < incl;
-            const uint32_t bal = __ballot_sync(0xffffffffu, mine0 || mine1);
-            if (bal == 0) {   // cannot happen for a range that brackets the rank; be safe: search all keys
+            BinHit h;
+            if (!locate_bin(s.tot.cnt, want - off, h)) {   // cannot happen for a range that brackets the rank
                 ka = 0; kb = 0xFFFFFFFFu; off = 0; top = true;
                 __syncthreads();
                 continue;
             }
-            const int src = __ffs(bal) - 1;
-            const uint32_t b = __shfl_sync(0xffffffffu, 2 * lane + (mine1 ? 1 : 0), src);
-            const uint32_t pre = __shfl_sync(0xffffffffu, mine1 ? excl + c0 : excl, src);
-            const uint32_t cntb = __shfl_sync(0xffffffffu, mine1 ? c1 : c0, src);
             if (shift == 0) {   // the bin is a single key
-                mode = 2; sel_key = ka + b; sel_lo = off + pre; sel_hi = sel_lo + cntb;
+                mode = 2; sel_key = ka + h.b; sel_lo = off + h.pre; sel_hi = sel_lo + h.cnt;
                 __syncthreads();
                 return;
             }
-            if (cntb > (uint32_t)K1_T1) {   // descend
-                off += pre;
-                ka = ka + (b << shift);
+            if (h.cnt > (uint32_t)K1_T1) {   // descend
+                off += h.pre;
+                ka = ka + (h.b << shift);
                 kb = min(kb, ka + ((1u << shift) - 1u));
-                __syncthreads();   // everyone has read s.tot.cnt before the next level rewrites it
+                __syncthreads();
                 continue;
             }
-            // -- window of bins around b with <= K1_LISTCAP pixels (thread 0 decides; same inputs on every CTA)
-            if (tid == 0) {
-                const int nb = (int)(span >> shift) + 1;
-                int b0 = (int)b, b1 = (int)b;
-                uint32_t tot = cntb;
-                for (int g = 0; g < 8; ++g) {
-                    bool grew = false;
-                    if (b1 + 1 < nb && tot + s.tot.cnt[b1 + 1] <= (uint32_t)K1_LISTCAP) { ++b1; tot += s.tot.cnt[b1]; grew = true; }
-                    if (b0 - 1 >= 0 && tot + s.tot.cnt[b0 - 1] <= (uint32_t)K1_LISTCAP) { --b0; tot += s.tot.cnt[b0]; grew = true; }
-                    if (!grew) break;
-                }
-                s.win_b0 = b0; s.win_b1 = b1;
-            }
+            if (tid == 0) grow_window(s, s.tot.cnt, (int)(span >> shift) + 1, h.b, h.cnt);
             __syncthreads();
             const uint32_t b0 = s.win_b0, b1 = s.win_b1;
-            // exclusive prefix of bin b0 (lane b0/2 knows it)
-            const uint32_t pre0 = __shfl_sync(0xffffffffu, (b0 & 1) ? excl + c0 : excl, (int)(b0 >> 1));
+            const uint32_t pre0 = bin_prefix(h, b0);
             const uint32_t kga = ka + (b0 << shift);
             const uint32_t kgb = min(kb, ka + (((b1 + 1) << shift) - 1u));
-            // -- gather: this thread's count is in its byte column; block scan -> private offset; write pass
             uint32_t mycnt = 0;
             for (uint32_t bb = b0; bb <= b1; ++bb) mycnt += col[bb * nt];
-            uint32_t incl2 = mycnt;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                uint32_t t = __shfl_up_sync(0xffffffffu, incl2, o);
-                if (lane >= o) incl2 += t;
-            }
-            if (lane == 31) s.red_u[tid >> 5] = incl2;
-            __syncthreads();
-            uint32_t wbase = 0, m_c = 0;
-            for (int w = 0; w < (nt >> 5); ++w) { if (w < (tid >> 5)) wbase += s.red_u[w]; m_c += s.red_u[w]; }
-            uint32_t pos = wbase + incl2 - mycnt;
+            uint32_t m;
+            uint32_t pos = block_scan_excl(s, mycnt, m);
             const uint32_t gspan = kgb - kga;
-            K1_SWEEP({
+            for_each_px(src, [&](float e) {
                 const uint32_t k = f32_to_key(e);
-                if (k - kga <= gspan) s.cand_local[pos++] = k;
-            })
-            // -- share the candidates over the team
-            Xch mine2; mine2.s1 = 0; mine2.s2 = 0; mine2.n_in = 0; mine2.n_below = 0; mine2.below = 0; mine2.m = m_c; mine2.nextkey = 0;
-            const int slot = phase & 1;
-            team_combine<C>(s, mine2, phase, false);   // includes the barrier that publishes cand_local
-            const uint32_t m = s.tot.m;
-            if constexpr (C == 1) {
-                for (uint32_t i = tid; i < m; i += nt) s.list[i] = s.cand_local[i];
-            } else {
-                uint32_t base = 0;
-                for (unsigned r = 0; r < (unsigned)C; ++r) {
-                    const uint32_t mr = Team<C>::remote(&s.xch[slot], r)->m;
-                    const uint32_t *src2 = Team<C>::remote(s.cand_local, r);
-                    for (uint32_t i = tid; i < mr; i += nt) s.list[base + i] = src2[i];
-                    base += mr;
-                }
-                Team<C>::sync();   // peers are done reading my cand_local and exchange slot
-            }
-            // -- counting sort of the list on fine bins (hist8 is dead now; the sort arrays alias it)
-            int fshift = 0;
-            while ((gspan >> fshift) >= (uint32_t)K1_FB) ++fshift;
-            const int nfb = (int)(gspan >> fshift) + 1;
+                if (k - kga <= gspan) s.list[pos++] = k;
+            });
             __syncthreads();
-            for (int i = tid; i < nfb; i += nt) srt.fcur[i] = 0;
-            __syncthreads();
-            for (uint32_t i = tid; i < m; i += nt) atomicAdd(&srt.fcur[(s.list[i] - kga) >> fshift], 1u);
-            __syncthreads();
-            {   // exclusive scan of fcur[0..nfb) -> fstart, fcur
-                const int per = (nfb + nt - 1) / nt, f0 = tid * per;
-                uint32_t local = 0;
-                for (int k = 0; k < per; ++k) if (f0 + k < nfb) local += srt.fcur[f0 + k];
-                uint32_t inc = local;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-                    if (lane >= o) inc += t;
-                }
-                if (lane == 31) s.red_u[tid >> 5] = inc;
-                __syncthreads();
-                uint32_t run = inc - local;
-                for (int w = 0; w < (tid >> 5); ++w) run += s.red_u[w];
-                for (int k = 0; k < per; ++k) {
-                    if (f0 + k >= nfb) break;
-                    const uint32_t c = srt.fcur[f0 + k];
-                    srt.fstart[f0 + k] = run;
-                    srt.fcur[f0 + k] = run;
-                    run += c;
-                }
-            }
-            __syncthreads();
-            for (uint32_t i = tid; i < m; i += nt) {
-                const uint32_t k = s.list[i];
-                srt.sorted[atomicAdd(&srt.fcur[(k - kga) >> fshift], 1u)] = k;
-            }
-            __syncthreads();
-            if (fshift > 0) {   // a fine bin may hold several keys: order it (bins are tiny)
-                for (int f = tid; f < nfb; f += nt) {
-                    const uint32_t lo = srt.fstart[f], hi = srt.fcur[f];
-                    for (uint32_t i = lo + 1; i < hi; ++i) {
-                        const uint32_t k = srt.sorted[i];
-                        uint32_t j = i;
-                        while (j > lo && srt.sorted[j - 1] > k) { srt.sorted[j] = srt.sorted[j - 1]; --j; }
-                        srt.sorted[j] = k;
-                    }
-                }
-                __syncthreads();
-            }
+            sort_candidates(s, s.list, m, kga, gspan, srt);   // the histogram is dead: the sort arrays alias it
             mode = 1; list_off = off + pre0; list_m = m;
             return;
         }
@@ -459,26 +431,18 @@ __global__ void k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a
     // smallest key strictly greater than `key` in the mesh (only asked when one exists)
     auto next_key = [&](uint32_t key) -> uint32_t {
         uint32_t best = 0xFFFFFFFFu;
-        K1_SWEEP({ const uint32_t k = f32_to_key(e); if (k > key) best = min(best, k); })
-        best = block_reduce_u32<true>(s, best);
-        Xch mine; mine.s1 = 0; mine.s2 = 0; mine.n_in = 0; mine.n_below = 0; mine.below = 0; mine.m = 0; mine.nextkey = best;
-        team_combine<C>(s, mine, phase, false);
-        const uint32_t r = s.tot.nextkey;
-        __syncthreads();
-        return r;
+        for_each_px(src, [&](float e) { const uint32_t k = f32_to_key(e); if (k > key) best = min(best, k); });
+        return block_reduce_u32<true>(s, best);
     };
 
-    // ---- clipping rounds -----------------------------------------------------------------------------------
     double LO = -INFINITY, HI = INFINITY;
     int n = n_tot, n_below = 0;
-    double med = 0, mu = 0, sd = 0;
     for (int round = 0;; ++round) {
         const double inv_n = 1.0 / (double)n;
         const double m1 = s1 * inv_n;
         mu = pivot + m1;
-        double var = s2 * inv_n - m1 * m1;
+        const double var = s2 * inv_n - m1 * m1;
         sd = var > 0.0 ? sqrt(var) : 0.0;
-        // median: ranks k0 = n_below + (n-1)/2 and (n even) k0 + 1 of the whole mesh
         const uint32_t k0 = (uint32_t)(n_below + (n - 1) / 2);
         const bool two = (n & 1) == 0;
         uint32_t key_a, key_b;
@@ -501,14 +465,13 @@ __global__ void k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a
             build(k0, ka, kb);
         }
         med = 0.5 * ((double)key_to_f32(key_a) + (double)key_to_f32(key_b));
-        if (round >= a.iters) break;
-        const double lo = fmax(LO, med - a.k_c * sd), hi = fmin(HI, med + a.k_c * sd);
-        // sweep: survivors of [lo, hi], sums about the new pivot (= current median: a robust centre that lies
-        // inside the surviving interval, so the one-pass variance loses no digits -- and is exactly 0 when all
-        // survivors are equal)
+        if (round >= iters) break;
+        const double lo = fmax(LO, med - k_c * sd), hi = fmin(HI, med + k_c * sd);
+        // survivors of [lo, hi]; sums about the new pivot (= current median: inside the surviving interval, so
+        // the one-pass variance loses no digits -- and is exactly 0 when all survivors are equal)
         double t1 = 0, t2 = 0;
         int c_in = 0, c_below = 0;
-        K1_SWEEP({
+        for_each_px(src, [&](float e) {
             const double x = (double)e;
             if (x < lo) ++c_below;
             else if (x <= hi) {
@@ -517,22 +480,332 @@ __global__ void k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a
                 t1 += d;
                 t2 = fma(d, d, t2);
             }
-        })
+        });
         block_reduce_stats(s, t1, t2, c_in, c_below);
-        Xch mine; mine.s1 = t1; mine.s2 = t2; mine.n_in = c_in; mine.n_below = c_below; mine.below = 0; mine.m = 0; mine.nextkey = 0;
-        team_combine<C>(s, mine, phase, false);
-        const int n_new = s.tot.n_in;
-        const int nb_new = s.tot.n_below;
-        const double s1_new = s.tot.s1, s2_new = s.tot.s2;
-        __syncthreads();   // s.tot is rewritten by the next combine
-        if (n_new == n || n_new == 0) break;   // stable (A7) or would empty the set: keep the current statistics
+        if (c_in == n || c_in == 0) break;   // stable (A7) or would empty the set: keep the current statistics
         LO = lo; HI = hi;
-        n = n_new; n_below = nb_new; s1 = s1_new; s2 = s2_new;
+        n = c_in; n_below = c_below; s1 = t1; s2 = t2;
         pivot = med;
     }
-#undef K1_SWEEP
+    n_out = n;
+}
 
-    if (rank == 0 && tid == 0) {
+// ---- the kernel ------------------------------------------------------------------------------------------
+template <int C>
+__global__ void k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float *slab = reinterpret_cast<float *>(smem_raw);   // [slab_rows * mw], 128-B aligned for TMA
+    const size_t slab_bytes = ((size_t)a.slab_rows * a.mw * sizeof(float) + 127) & ~(size_t)127;
+    Smem &s = *reinterpret_cast<Smem *>(smem_raw + slab_bytes);
+    unsigned char *area = smem_raw + slab_bytes + ((sizeof(Smem) + 127) & ~(size_t)127);
+    uint8_t *hist8 = area;                                  // [K1_NBIN][nt] byte counters
+    uint32_t *samp = reinterpret_cast<uint32_t *>(area);    // sample keys (before the histogram)
+    float *tail = reinterpret_cast<float *>(area);          // tail pixels (after the histogram)
+
+    const unsigned rank = Team<C>::rank();
+    const int mesh = blockIdx.x / C;
+    const int frame = mesh / (a.ny * a.nx);
+    const int mj = (mesh / a.nx) % a.ny, mi = mesh % a.nx;
+    const int y0 = mj * a.mh, x0 = mi * a.mw;
+    const int vh = min(a.mh, a.H - y0), vw = min(a.mw, a.W - x0);       // valid part of the mesh
+    const int row0 = (int)rank * a.slab_rows;                           // first mesh row of this CTA's slab
+    const int my_rows = max(0, min(a.slab_rows, vh - row0));
+    const int n_c = my_rows * vw;                                       // valid pixels in this slab, a prefix
+    const int n_tot = vh * vw;
+    const float *mesh_ptr = a.img + (size_t)frame * a.H * a.W + (size_t)y0 * a.W + x0;
+    const int tid = threadIdx.x, nt = blockDim.x;
+
+    // ---- stage the slab ---------------------------------------------------------------------------------
+    const bool tma = a.use_tma && vw == a.mw;
+    if (tma && tid == 0) {
+        uint32_t bar = smem_u32(&s.mbar);
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        uint32_t bytes = (uint32_t)((size_t)a.slab_rows * a.mw * sizeof(float));
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+        // rows past H are zero-filled by TMA; they lie beyond the n_c prefix and are never read
+        asm volatile(
+            "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes"
+            " [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(smem_u32(slab)),
+            "l"(&tmap), "r"(x0), "r"(y0 + row0), "r"(frame), "r"(bar)
+            : "memory");
+    }
+
+    // ---- lattice sample of this CTA's slab rows (read from global while the TMA load is in flight), sorted ---
+    bool fast = a.allow_fast && n_tot >= K1_FAST_MIN_PX && vw >= 16;
+    constexpr int M_S = 256, G_S = 8;   // 8 x 8 lattice points x 4 consecutive pixels
+    if (fast && my_rows > 0) {
+        for (int e = tid; e < M_S; e += nt) {
+            const int pt = e >> 2, q = e & 3;
+            const int i = pt / G_S, j = pt - i * G_S;
+            const int y = row0 + ((2 * i + 1) * my_rows) / (2 * G_S);
+            const int x = min((((2 * j + 1) * vw) / (2 * G_S)) & ~3, vw - 4) + q;
+            samp[e] = f32_to_key(__ldg(mesh_ptr + (size_t)y * a.W + x));
+        }
+        __syncthreads();
+        bitonic_sort(samp, M_S);
+    }
+    // sample quantiles, averaged over the team -> pivot, core interval [A, B], median bracket [ka, kb]
+    double pivot = 0.0;
+    float A_f = 0.f, B_f = 0.f;
+    uint32_t ka = 0, kb = 0;
+    if (fast) {
+        if (tid == 0) {
+            s.sx.valid = my_rows > 0 ? 1 : 0;
+            if (my_rows > 0) {
+                s.sx.q50 = (double)key_to_f32(samp[M_S / 2]);
+                s.sx.q16 = (double)key_to_f32(samp[(M_S * 16) / 100]);
+                s.sx.ka = samp[M_S / 2 - 48];   // +-6 standard deviations of a 256-sample quantile near 0.5
+                s.sx.kb = samp[M_S / 2 + 48];
+                s.sx.lo3 = (double)key_to_f32(samp[M_S / 2 - 24]);
+                s.sx.hi3 = (double)key_to_f32(samp[M_S / 2 + 24]);
+            }
+        }
+        Team<C>::sync();   // #0 (a plain barrier when C = 1)
+        double q50 = 0, q16 = 0, lo3 = 0, hi3 = 0;
+        int nv = 0;
+        ka = 0xFFFFFFFFu; kb = 0;
+        for (unsigned r = 0; r < (unsigned)C; ++r) {   // rank order: the same bits on every CTA
+            const SampleX *o = Team<C>::remote(&s.sx, r);
+            if (!o->valid) continue;
+            ++nv; q50 += o->q50; q16 += o->q16; lo3 += o->lo3; hi3 += o->hi3; ka = min(ka, o->ka); kb = max(kb, o->kb);
+        }
+        q50 /= (double)nv; q16 /= (double)nv;
+        if (nv >= 4) {   // the average of >= 4 independent 3-sigma quantiles is a 6-sigma bracket, half as wide
+            ka = f32_to_key(__double2float_rd(lo3 / (double)nv));
+            kb = f32_to_key(__double2float_ru(hi3 / (double)nv));
+        }
+        const double sig = q50 - q16;                 // lower side: sources and hot pixels are positive
+        const double c = nv >= 4 ? 2.2 : 2.0;         // the averaged estimate is less noisy
+        pivot = q50;
+        A_f = (float)(pivot - c * sig);
+        B_f = (float)(pivot + c * sig);
+        if (!(sig > 0.0) || ka >= kb || !((double)A_f < pivot) || !((double)B_f > pivot)) {
+            fast = false;
+            if (tid == 0 && rank == 0) atomicAdd(&g_k1_reason[1], 1ull);
+        }
+    }
+    __syncthreads();   // the sample is dead: the work area becomes the byte histogram
+
+    if (tma) {
+        uint32_t bar = smem_u32(&s.mbar), done = 0;
+        while (!done) {
+            asm volatile(
+                "{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
+                : "=r"(done)
+                : "r"(bar)
+                : "memory");
+        }
+    } else if (C == 1 || fast) {   // plain loader: valid pixels packed row-major
+        for (int i = tid; i < n_c; i += nt) {
+            int r = i / vw, c = i - r * vw;
+            slab[i] = mesh_ptr[(size_t)(row0 + r) * a.W + c];
+        }
+        __syncthreads();
+    }
+
+    const float4 *slab4 = reinterpret_cast<const float4 *>(slab);
+    const int n4 = n_c >> 2, n_tail4 = n_c & 3;
+#define K1_SWEEP(BODY)                                                    \
+    {                                                                     \
+        for (int i_ = tid; i_ < n4; i_ += nt) {                           \
+            const float4 v_ = slab4[i_];                                  \
+            { const float e = v_.x; BODY }                                \
+            { const float e = v_.y; BODY }                                \
+            { const float e = v_.z; BODY }                                \
+            { const float e = v_.w; BODY }                                \
+        }                                                                 \
+        if (tid < n_tail4) { const float e = slab[(n4 << 2) + tid]; BODY }\
+    }
+
+    double med = 0, mu = 0, sd = 0;
+    int n_final = n_tot;
+    bool done_fast = false;
+    bool slab_dirty = false;   // the fast path reuses the slab for its sort arrays
+
+    if (fast) {
+        // ---- sweep 1: core sums, tail count, bracket histogram ---------------------------------------------
+        const uint32_t span = kb - ka;
+        int shift = 0;
+        while ((span >> shift) >= (uint32_t)K1_NBIN) ++shift;
+        for (int i = tid; i < (K1_NBIN * nt) / 16; i += nt) reinterpret_cast<uint4 *>(hist8)[i] = make_uint4(0, 0, 0, 0);
+        __syncthreads();
+        double t1 = 0, t2 = 0;
+        int c_core = 0, c_tail = 0;
+        uint32_t below = 0;
+        uint8_t *col = hist8 + tid;
+        K1_SWEEP({
+            const uint32_t k = f32_to_key(e);
+            const uint32_t t = k - ka;
+            if (t <= span) col[(t >> shift) * nt] += 1;
+            else if (k < ka) ++below;
+            if (e >= A_f && e <= B_f) {
+                const double d = (double)e - pivot;
+                t1 += d;
+                t2 = fma(d, d, t2);
+                ++c_core;
+            } else ++c_tail;
+        })
+        __syncthreads();
+        reduce_byte_hist(hist8, nt, s.xch.cnt);
+        below = block_reduce_u32<false>(s, below);
+        {
+            int ct = c_tail;
+            block_reduce_stats(s, t1, t2, c_core, ct);
+            if (tid == 0) { s.xch.s1 = t1; s.xch.s2 = t2; s.xch.n_core = c_core; s.xch.n_tail = ct; s.xch.below = below; }
+        }
+        Team<C>::sync();   // #1: every CTA's xch is published
+        if (tid == 0) {
+            double q1 = 0, q2 = 0;
+            int nc = 0, ntl = 0;
+            uint32_t bl = 0;
+            for (unsigned r = 0; r < (unsigned)C; ++r) {   // rank order: every CTA computes the same bits
+                const Xch *o = Team<C>::remote(&s.xch, r);
+                q1 += o->s1; q2 += o->s2; nc += o->n_core; ntl += o->n_tail; bl += o->below;
+            }
+            s.tot.s1 = q1; s.tot.s2 = q2; s.tot.n_core = nc; s.tot.n_tail = ntl; s.tot.below = bl;
+        }
+        if (tid >= 32 && tid < 32 + K1_NBIN) {
+            const int b = tid - 32;
+            uint32_t t = 0;
+            for (unsigned r = 0; r < (unsigned)C; ++r) t += Team<C>::remote(&s.xch, r)->cnt[b];
+            s.tot.cnt[b] = t;
+        }
+        __syncthreads();
+        const double s1c = s.tot.s1, s2c = s.tot.s2;
+        const int n_core = s.tot.n_core, n_tail_tot = s.tot.n_tail;
+        const uint32_t off = s.tot.below;
+        // ---- window of bins around the round-0 median rank ----------------------------------------------
+        const uint32_t k_first = (uint32_t)((n_tot - 1) / 2);
+        BinHit h;
+        bool ok = n_tail_tot <= a.tailcap && n_core > 0 && k_first >= off;
+        ok = locate_bin(s.tot.cnt, k_first - off, h) && ok;   // (all lanes run the shuffles)
+        if (tid == 0 && rank == 0) {
+            if (!(n_tail_tot <= a.tailcap)) atomicAdd(&g_k1_reason[2], 1ull);
+            else if (!ok) atomicAdd(&g_k1_reason[3], 1ull);
+            else if (h.cnt > (uint32_t)K1_LISTCAP) atomicAdd(&g_k1_reason[4], 1ull);
+        }
+        ok = ok && h.cnt <= (uint32_t)K1_LISTCAP;
+        uint32_t m_tot = 0, list_off = 0, kga = 0, gspan = 0;
+        if (ok) {
+            if (tid == 0) grow_window(s, s.tot.cnt, (int)(span >> shift) + 1, h.b, h.cnt);
+            __syncthreads();
+            const uint32_t b0 = s.win_b0, b1 = s.win_b1;
+            list_off = off + bin_prefix(h, b0);
+            kga = ka + (b0 << shift);
+            const uint32_t kgb = min(kb, ka + (((b1 + 1) << shift) - 1u));
+            gspan = kgb - kga;
+            // ---- sweep 2: gather window candidates and tail pixels ---------------------------------------
+            uint32_t mycnt = 0;
+            for (uint32_t bb = b0; bb <= b1; ++bb) mycnt += col[bb * nt];
+            uint32_t packed_tot;
+            const uint32_t packed = block_scan_excl(s, mycnt | ((uint32_t)c_tail << 16), packed_tot);
+            uint32_t pos_c = packed & 0xFFFFu, pos_t = packed >> 16;   // (the scan's barriers: histogram is dead)
+            K1_SWEEP({
+                const uint32_t k = f32_to_key(e);
+                if (k - kga <= gspan) s.list[pos_c++] = k;
+                if (!(e >= A_f && e <= B_f)) tail[pos_t++] = e;
+            })
+            if (tid == 0) { s.xch.m_cand = packed_tot & 0xFFFFu; s.xch.m_tail = packed_tot >> 16; }
+        }
+        Team<C>::sync();   // #2: lists published (or: everybody is done reading the peers' xch)
+        if (!ok) {
+            fast = false;
+        } else {
+            m_tot = s.xch.m_cand;
+            uint32_t mt_tot = s.xch.m_tail;
+            if constexpr (C > 1) {
+                if (rank == 0) {
+                    for (unsigned r = 1; r < (unsigned)C; ++r) {
+                        const Xch *o = Team<C>::remote(&s.xch, r);
+                        const uint32_t mr = o->m_cand, tr = o->m_tail;
+                        const uint32_t *lsrc = Team<C>::remote(s.list, r);
+                        const float *tsrc = Team<C>::remote(tail, r);
+                        for (uint32_t i = tid; i < mr; i += nt) s.list[m_tot + i] = lsrc[i];
+                        for (uint32_t i = tid; i < tr; i += nt) tail[mt_tot + i] = tsrc[i];
+                        m_tot += mr; mt_tot += tr;
+                    }
+                }
+                Team<C>::sync();   // #3: rank 0 has copied; peers may leave
+                if (rank != 0) return;
+            }
+            __syncthreads();
+            SortArea &srt = *reinterpret_cast<SortArea *>(slab);   // the slab is dead from here on
+            slab_dirty = true;
+            sort_candidates(s, s.list, m_tot, kga, gspan, srt);
+            // ---- clipping rounds on the tail list --------------------------------------------------------
+            const double A_d = (double)A_f, B_d = (double)B_f;
+            auto tail_stats = [&](double lo, double hi, double &q1, double &q2, int &c_in, int &c_below) {
+                q1 = 0; q2 = 0; c_in = 0; c_below = 0;
+                for (uint32_t i = tid; i < mt_tot; i += nt) {
+                    const double x = (double)tail[i];
+                    if (x < lo) ++c_below;
+                    else if (x <= hi) {
+                        const double d = x - pivot;
+                        ++c_in;
+                        q1 += d;
+                        q2 = fma(d, d, q2);
+                    }
+                }
+                block_reduce_stats(s, q1, q2, c_in, c_below);
+            };
+            double LO = -INFINITY, HI = INFINITY, q1, q2;
+            int c_in, c_below;
+            tail_stats(LO, HI, q1, q2, c_in, c_below);
+            int n = n_core + c_in, n_below = c_below;
+            double s1 = s1c + q1, s2 = s2c + q2;
+            done_fast = true;
+            for (int round = 0;; ++round) {
+                const double inv_n = 1.0 / (double)n;
+                const double m1 = s1 * inv_n;
+                mu = pivot + m1;
+                const double var = s2 * inv_n - m1 * m1;
+                sd = var > 0.0 ? sqrt(var) : 0.0;
+                const uint32_t k0 = (uint32_t)(n_below + (n - 1) / 2);
+                const bool two = (n & 1) == 0;
+                if (k0 < list_off || k0 + (two ? 1u : 0u) >= list_off + m_tot) {
+                    done_fast = false;
+                    if (tid == 0) atomicAdd(&g_k1_reason[5], 1ull);
+                    break;
+                }
+                const uint32_t j = k0 - list_off;
+                const uint32_t key_a = srt.sorted[j], key_b = two ? srt.sorted[j + 1] : key_a;
+                med = 0.5 * ((double)key_to_f32(key_a) + (double)key_to_f32(key_b));
+                n_final = n;
+                if (round >= a.iters) break;
+                const double lo = fmax(LO, med - a.k_c * sd), hi = fmin(HI, med + a.k_c * sd);
+                if (!(lo <= A_d && hi >= B_d)) {   // a bound entered the core
+                    done_fast = false;
+                    if (tid == 0) atomicAdd(&g_k1_reason[6], 1ull);
+                    break;
+                }
+                tail_stats(lo, hi, q1, q2, c_in, c_below);
+                const int n_new = n_core + c_in;
+                if (n_new == n) break;   // stable (A7); n_new > 0 because the core survives
+                LO = lo; HI = hi;
+                n = n_new; n_below = c_below; s1 = s1c + q1; s2 = s2c + q2;
+            }
+        }
+    }
+#undef K1_SWEEP
+    if constexpr (C > 1) {
+        if (!fast) {   // nothing was exchanged yet (or everybody passed #2): the peers have no further part
+            if (rank != 0) return;
+        }
+    }
+
+    if (!done_fast) {
+        if (tid == 0) atomicAdd(&g_k1_slow_meshes, 1ull);
+        MeshSrc src;
+        src.slab = (C == 1 && !slab_dirty) ? slab : nullptr;
+        src.n_slab = n_c;
+        src.g = mesh_ptr; src.W = a.W; src.vh = vh; src.vw = vw;
+        src.vec4 = (vw % 4 == 0) && (a.mw % 4 == 0) && (a.W % 4 == 0);
+        __syncthreads();
+        k1_slow_path(src, s, hist8, n_tot, a.k_c, a.iters, med, mu, sd, n_final);
+    }
+
+    if (tid == 0) {
         double bkg = a.median_factor * med - a.mean_factor * mu;
         if (a.skew_guard) {
             if (sd == 0.0) bkg = mu;
@@ -542,17 +815,15 @@ __global__ void k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a
         if (a.rms_raw) a.rms_raw[mesh] = sd;
         if (a.median) a.median[mesh] = med;
         if (a.mean) a.mean[mesh] = mu;
-        if (a.n_kept) a.n_kept[mesh] = n;
+        if (a.n_kept) a.n_kept[mesh] = n_final;
     }
-    if constexpr (C > 1) Team<C>::sync();   // nobody leaves while a peer may still read its shared memory
 }
 
 }  // namespace
 
 // ---- host side ------------------------------------------------------------------------------------------
 static size_t k1_smem_bytes(int slab_rows, int mw, int threads) {
-    size_t area = (size_t)K1_NBIN * threads;
-    if (area < sizeof(SortArea)) area = sizeof(SortArea);
+    size_t area = (size_t)K1_NBIN * threads;   // byte histograms; also holds the sample (<= 4 KiB) and the tails
     return bd_align_up((size_t)slab_rows * mw * sizeof(float), 128) + bd_align_up(sizeof(Smem), 128) + area + 128;
 }
 
@@ -568,12 +839,21 @@ int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan) {
             int threads = px >= 16384 ? 512 : 256;
             size_t smem = k1_smem_bytes(rows, mesh_w, threads);
             bool ok = pass == 0 ? slab <= soft : true;
-            // byte counters: a thread sees at most ceil(px/threads) + 4 pixels of the slab
-            if (ok && smem <= ctx->smem_optin && px / threads + 5 <= 255) {
+            // byte counters: what one thread can see of (a) its slab, (b) the whole mesh read from global
+            // memory by a lone CTA (slow path of a team), must stay <= 255 per bin
+            size_t per_thread = px / threads + 5;
+            {
+                int nw = threads / 32;
+                size_t rows_w = (size_t)(mesh_h + nw - 1) / nw;
+                size_t per_row = mesh_w % 4 == 0 ? (size_t)((mesh_w + 127) / 128) * 4 : (size_t)(mesh_w + 31) / 32;
+                if (rows_w * per_row > per_thread) per_thread = rows_w * per_row;
+            }
+            if (ok && smem <= ctx->smem_optin && per_thread <= 255) {
                 plan->cluster = c;
                 plan->slab_rows = rows;
                 plan->smem_bytes = smem;
                 plan->threads = threads;
+                plan->tailcap = K1_NBIN * threads / 4;
                 plan->use_tma = (mesh_w % 4 == 0 && mesh_w <= 256 && rows <= 256) ? 1 : 0;
                 return BD_OK;
             }
@@ -605,11 +885,12 @@ int k1_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg
               double *d_rms_raw, double *d_median, double *d_mean, int32_t *d_n_kept, cudaStream_t st) {
     K1Plan plan;
     int rc = k1_plan(ctx, p->mesh_h, p->mesh_w, &plan);
-    if (rc != BD_OK) return bd_set_error(ctx, rc, "mesh %dx%d does not fit a thread-block cluster's shared memory", p->mesh_h, p->mesh_w);
+    if (rc != BD_OK) return bd_set_error(ctx, rc, "mesh %dx%d is too large for the statistics kernel", p->mesh_h, p->mesh_w);
     K1Args a;
     a.img = d_img; a.B = B; a.H = H; a.W = W; a.mh = p->mesh_h; a.mw = p->mesh_w;
     a.ny = (H + a.mh - 1) / a.mh; a.nx = (W + a.mw - 1) / a.mw;
-    a.slab_rows = plan.slab_rows; a.use_tma = plan.use_tma;
+    a.slab_rows = plan.slab_rows; a.use_tma = plan.use_tma; a.tailcap = plan.tailcap;
+    a.allow_fast = ctx->k1_force_slow ? 0 : 1;
     a.k_c = p->clip_sigma; a.iters = p->clip_iters; a.skew_guard = p->skew_guard;
     a.median_factor = p->median_factor; a.mean_factor = p->mean_factor;
     a.bkg_raw = d_bkg_raw; a.rms_raw = d_rms_raw; a.median = d_median; a.mean = d_mean; a.n_kept = d_n_kept;
@@ -636,5 +917,26 @@ int k1_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg
         default: e = k1_launch_c<8>(tmap, a, plan, n_mesh, st); break;
     }
     BD_CUDA_CHECK(ctx, e);
+    return BD_OK;
+}
+
+// diagnostics (not part of include/bkgdet.h): number of meshes that took the slow path since the last reset
+extern "C" int bd_debug_k1_slow_meshes(unsigned long long *out, int reset) {
+    unsigned long long v = 0, z = 0;
+    if (cudaMemcpyFromSymbol(&v, g_k1_slow_meshes, sizeof(v)) != cudaSuccess) return BD_ECUDA;
+    if (reset && cudaMemcpyToSymbol(g_k1_slow_meshes, &z, sizeof(z)) != cudaSuccess) return BD_ECUDA;
+    if (out) *out = v;
+    return BD_OK;
+}
+extern "C" int bd_debug_k1_reasons(unsigned long long *out8, int reset) {
+    unsigned long long z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    if (cudaMemcpyFromSymbol(out8, g_k1_reason, sizeof(z)) != cudaSuccess) return BD_ECUDA;
+    if (reset && cudaMemcpyToSymbol(g_k1_reason, z, sizeof(z)) != cudaSuccess) return BD_ECUDA;
+    return BD_OK;
+}
+// diagnostics: force every mesh through the slow path (tests exercise both)
+extern "C" int bd_debug_k1_force_slow(bd_ctx *ctx, int on) {
+    if (!ctx) return BD_EINVAL;
+    ctx->k1_force_slow = on ? 1 : 0;
     return BD_OK;
 }

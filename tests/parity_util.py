@@ -7,8 +7,9 @@ Tolerances, written out:
   * sub: |d| <= 1e-4 * |bkg_oracle| (a relative test on a zero-mean quantity is meaningless);
   * mask: may differ only where the oracle's |sub - k*rms| <= 1e-5 * rms ("fragile" pixels);
   * labels: bit-exact against the oracle's labelling of the SAME mask;
-  * catalogue: 1:1 on (frame, label); npix, bbox, peak position exact; flux, x, y 1e-4 relative
-    (x, y additionally 1e-3 px absolute is reported); x2, y2, xy 1e-3 relative with an absolute floor.
+  * catalogue: 1:1 on (frame, label); npix, bbox, peak position exact; peak value 1e-6 relative (float32 rounding of sub);
+    flux, x, y 1e-4 relative
+    (x, y additionally 1e-3 px absolute is reported); x2, y2, xy 1e-3 relative to max(|moment|, 1e-3*(x2+y2)).
 """
 from __future__ import annotations
 
@@ -19,6 +20,7 @@ import oracle
 REL_MAP = 1e-4
 REL_CAT = 1e-4
 REL_MOM = 1e-3
+REL_PEAK = 1e-6
 
 
 def to_oracle_params(p):
@@ -42,7 +44,7 @@ def assert_mask_parity(mask_gpu, mask_or, fragile):
     return int(diff.sum())
 
 
-def assert_catalogue_equal(got, want, frame=None, exempt_labels=()):
+def assert_catalogue_equal(got, want, frame=None, exempt_labels=(), peak_pos_exact=True):
     """got: GPU records (bd_source dtype) of one frame; want: oracle records of the same labels/sub."""
     if frame is not None:
         got = got[got["frame"] == frame]
@@ -54,9 +56,20 @@ def assert_catalogue_equal(got, want, frame=None, exempt_labels=()):
     if len(want) == 0:
         return dict(n=0)
     assert np.array_equal(got["label"], want["label"]), "labels / order differ"
-    for k in ("npix", "xmin", "xmax", "ymin", "ymax", "xpeak", "ypeak"):
+    for k in ("npix", "xmin", "xmax", "ymin", "ymax"):
         assert np.array_equal(got[k], want[k]), f"{k} differs at {np.flatnonzero(got[k] != want[k])[:5]}"
-    assert np.array_equal(got["peak"].astype(np.float32), want["peak"].astype(np.float32)), "peak differs"
+    moved = (got["xpeak"] != want["xpeak"]) | (got["ypeak"] != want["ypeak"])
+    if peak_pos_exact:
+        # same sub map on both sides: the peak pixel (ties -> smallest raster index) is unique
+        assert not moved.any(), f"peak position differs at {np.flatnonzero(moved)[:5]}"
+    else:
+        # each side takes the maximum of its OWN float32 sub map; the maps agree to ~1e-6 ADU, so where two
+        # pixels of a component are equal to the last bit (adjacent saturated / hot pixels) the winner may
+        # differ.  The peak VALUE is still compared below; such near-ties must stay rare.
+        assert moved.sum() <= max(2, len(want) // 100), f"{moved.sum()} of {len(want)} peak positions differ"
+    # peak is a float32 value of sub: both sides round a value that agrees to ~1e-6 ADU, so the last bit may differ
+    perr = np.abs(got["peak"].astype(np.float64) - want["peak"]) / np.maximum(np.abs(want["peak"]), 1e-300)
+    assert np.all(perr <= REL_PEAK), f"peak: worst rel {perr.max():.3e}"
     worst = {}
     for k in ("flux", "x", "y"):
         err = np.abs(got[k] - want[k]) / np.maximum(np.abs(want[k]), 1e-300)
@@ -64,7 +77,9 @@ def assert_catalogue_equal(got, want, frame=None, exempt_labels=()):
         worst[k] = float(err.max())
     worst["centroid_abs_px"] = float(max(np.abs(got["x"] - want["x"]).max(), np.abs(got["y"] - want["y"]).max()))
     for k in ("x2", "y2", "xy"):
-        scale = np.maximum(np.abs(want[k]), 1e-6 * (1.0 + want["x2"] + want["y2"]))
+        # a moment can be ~0 by symmetry (xy, or x2 of a one-column component): the error it inherits from a
+        # relative perturbation eps of the pixel values is <= eps * (x2 + y2), so the scale has that floor
+        scale = np.maximum(np.abs(want[k]), 1e-3 * (want["x2"] + want["y2"]) + 1e-9)
         err = np.abs(got[k] - want[k]) / scale
         assert np.all(err <= REL_MOM), f"{k}: worst rel {err.max():.3e}"
         worst[k] = float(err.max())

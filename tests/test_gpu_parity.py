@@ -39,9 +39,18 @@ def params_for(bd, cfg, **kw):
 
 # ------------------------------------------------------------------------------------------- K1
 def check_mesh_stats(bd, ctx, img, p):
-    """img float32 [B,H,W] numpy."""
-    out = bd.mesh_stats(ctx, dev(img), p)
-    torch.cuda.synchronize()
+    """img float32 [B,H,W] numpy.  Both the fast path (where it applies) and the forced general path."""
+    for force_slow in (False, True):
+        bd.k1_force_slow(ctx, force_slow)
+        try:
+            out = bd.mesh_stats(ctx, dev(img), p)
+            torch.cuda.synchronize()
+        finally:
+            bd.k1_force_slow(ctx, False)
+        _compare_mesh_stats(out, img, p)
+
+
+def _compare_mesh_stats(out, img, p):
     op = to_oracle_params(p)
     for f in range(img.shape[0]):
         st = oracle.mesh_stats(img[f], op)
@@ -86,6 +95,18 @@ def test_k1_degenerate_inputs(bd, ctx):
     check_mesh_stats(bd, ctx, outl, bd.BkgParams())
     cauchy = np.random.default_rng(3).standard_cauchy(size=(1, 64, 128)).astype(np.float32)
     check_mesh_stats(bd, ctx, cauchy, bd.BkgParams(clip_sigma=2.0))
+    # meshes large enough for the fast path, built so that it gives up half-way (a clipping bound enters the
+    # core interval; the median rank leaves the candidate window) and the general path takes over
+    big = np.random.default_rng(4).normal(0, 1, size=(1, 256, 384)).astype(np.float32)
+    for mesh in (128, 256):
+        check_mesh_stats(bd, ctx, big, bd.BkgParams(mesh_h=mesh, mesh_w=mesh, clip_sigma=1.0))
+        check_mesh_stats(bd, ctx, big, bd.BkgParams(mesh_h=mesh, mesh_w=mesh, clip_sigma=2.0, clip_iters=20))
+    bigc = np.random.default_rng(5).standard_cauchy(size=(1, 256, 384)).astype(np.float32)
+    skew = np.random.default_rng(6).exponential(50.0, size=(1, 256, 384)).astype(np.float32) + 100.0
+    tie2 = np.random.default_rng(7).integers(0, 4, size=(1, 256, 384)).astype(np.float32)
+    for mesh in (128, 256):
+        for im in (bigc, skew, tie2):
+            check_mesh_stats(bd, ctx, im, bd.BkgParams(mesh_h=mesh, mesh_w=mesh))
 
 
 # ------------------------------------------------------------------------------------------- K2
@@ -256,7 +277,7 @@ def check_chain(bd, ctx, img, p, k, min_area, frames=None):
         exempt = fragile_touched_labels(r["labels"], r["fragile"]) if ndiff else ()
         if ndiff:
             exempt = np.union1d(exempt, fragile_touched_labels(lab_g, r["fragile"]))
-        worst2 = assert_catalogue_equal(cat, r["cat"], frame=f, exempt_labels=exempt)
+        worst2 = assert_catalogue_equal(cat, r["cat"], frame=f, exempt_labels=exempt, peak_pos_exact=False)
         report[f] = dict(mask_diff=ndiff, n_sources=int(n[f]), fragile=int(r["fragile"].sum()), stage=worst, chain=worst2,
                          exempt=len(exempt))
     return report
