@@ -33,7 +33,7 @@ from synth import CONFIGS, make_frames  # noqa: E402
 METRIC = "Mpix/s background+detection per frame"
 K3_BYTES_PER_PX = 17.0          # img 4 read; sub 4 + bkg 4 + rms 4 + mask 1 written
 CHAIN_BYTES_PER_PX = 30.0       # K1 4 + K3 17 + K4 5 + K5 4
-LAUNCHES_PER_STEP = 18          # K1, K2, K3, then detect_sources: k4a, 2 seams, 2x3 scans, zero, k4c, counts, init, k5b, k5c
+LAUNCHES_PER_STEP = 10          # K1, K2a, K2b, K3, then detect_sources: k4a, k4b, k5m, k5k, k5s, k5f (+2 memsets, not counted)
 FALLBACK_HBM_GBS = 6650.0       # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 
 

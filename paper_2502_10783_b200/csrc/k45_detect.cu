@@ -3,65 +3,91 @@
 // connected to form source candidates ... calculate peak values and total flux for each candidate"),
 // :159 (isophotal photometry).  Readings A16 (8-connectivity), A18-A20 (moments, min_area, label map).
 //
-// The paper scans with one thread per pixel and reduces with Thrust.  Here:
-//   K4a  tile-local union-find in shared memory (128x32-pixel tiles, union by minimum index with
-//        atomicMin), written out as parent pointers = 1 + raster index, plus a root bitmap;
-//   K4b  seam merge: the pixel pairs that straddle tile borders are united in global memory
-//        (atomicMin on the label array); a root that gets linked clears its bit;
-//   scan of the root bitmap -> every root's rank in raster order (the catalogue order);
-//   K4c  flatten every pixel to its root (= minimum raster index of the component) and count areas
-//        by root rank;
-//   scan of (area >= min_area) -> catalogue slot of every kept root;
-//   K5b  accumulate flux, first and second moments (float64 atomics, coordinates relative to the root
-//        pixel), peak (64-bit atomicMax on value|~index) and bounding box of kept components only;
-//   K5c  finalise records in slot order = ascending (frame, label).
-// Labels are bit-exact by construction; the float sums depend on atomic order (not bit-reproducible).
+// The paper scans with one thread per pixel and reduces with Thrust.  Here the frame is cut into 128x64-pixel
+// tiles and labelling and reduction are ONE pass over the tile (the first version labelled, flattened and then
+// re-read labels and sub twice more: 1.38 ms on 9216x9232; ncu showed the tile kernel instruction-bound on
+// divergent per-pixel loops and the re-read passes latency-bound):
+//   K4a  per tile: mask bytes -> bit rows (+1-pixel halo) in shared memory; a COMPACT list of the tile's
+//        foreground pixels, so every later phase runs dense; union-find on the list (parent = start of the
+//        horizontal run, vertical/diagonal links with the usual pruning, union by minimum index); per-component
+//        pixel counts; components that can matter (count >= min_area, or touching a foreground pixel of
+//        another tile) get partial sums (npix, flux, first/second moments about the tile-local root, peak,
+//        bbox) reduced in shared memory with warp-segmented shuffles, and are written as one 96-byte record
+//        each; the label tile (1 + raster index of the tile-local root, 0 = background) is assembled in
+//        shared memory and leaves with one TMA bulk-tensor store; the tile's border bit rows/columns are
+//        exported (48 B per tile).
+//   K4b  seam merge from the exported border bits alone: only real cross-tile links touch the label array
+//        (union by atomicMin on the root's label word).
+//   K5m  for every record whose tile-local root is no longer a root: add it to the final root's record
+//        (float64 atomics, moments shifted to the new origin) and relabel the pixels of its bounding box.
+//   K5k  records that are final roots with npix >= min_area set their bit in a per-pixel bitmap and count into
+//        1024-pixel blocks;  K5s scans the block counts;  K5f ranks every kept root (= catalogue slot in
+//        ascending (frame, label) order) and writes its record.
+// Records live in a direct-mapped table indexed by the 2x2-pixel block of the root (two roots can never share
+// one: they would be 8-adjacent), so no allocation can overflow; only the touched entries cost traffic.
+// Labels are bit-exact by construction; float sums depend on atomic order (not bit-reproducible).
 #include "common.cuh"
 
 namespace {
 
 typedef unsigned long long u64;
 
-constexpr int TW = 128, TH = 32, K4_NT = 256;
-constexpr int SCAN_NT = 256, SCAN_PER = 16, SCAN_ELEMS = SCAN_NT * SCAN_PER;
+constexpr int TW = 128, TH = 64, K4_NT = 512;
+constexpr int TPX = TW * TH;             // 8192 pixels per tile
+constexpr int BROWS = TH + 2;            // bit rows incl. halo rows y0-1 and y0+TH
+constexpr int BWORDS = 6;                // [0] bit 31 = column x0-1, [1..4] the tile, [5] bit 0 = column x0+TW
+constexpr int NS = 64;                   // shared-memory stat slots per batch
+constexpr int EDGE_WORDS = 12;           // per tile: top[4], bottom[4], left[2], right[2]
 
-struct Acc {
+constexpr uint32_t F_ROOT = 0x80000000u; // root word: F_ROOT | F_REC | F_RING | slot << 14 | count
+constexpr uint32_t F_REC = 0x40000000u;
+constexpr uint32_t F_RING = 0x20000000u;
+constexpr uint32_t CNT_MASK = 0x3FFFu;   // count <= 8192
+constexpr int SLOT_SHIFT = 14;           // slot < 2048 (at most one root per 2x2 block)
+
+struct Rec {   // 96 bytes; sums are about the record's own root pixel
     double f, sx, sy, sxx, syy, sxy;
-    u64 peak;   // (ordered key of sub << 32) | (0xFFFFFFFF - raster index): atomicMax -> max value, ties -> min index
-    u64 root;   // global pixel index of the root
-    int xmin, xmax, ymin, ymax;
+    u64 peak;          // (ordered key of sub << 32) | (0xFFFFFFFF - raster index in frame): max -> max value, ties -> min index
+    int32_t root;      // raster index of the root within its frame
+    int32_t frame;
+    int32_t npix;
+    int32_t xmin, xmax, ymin, ymax;
+    int32_t pad[3];
 };
+static_assert(sizeof(Rec) == 96, "Rec must be 96 bytes");
 
 struct Ws {
-    uint32_t *counters;     // [0] n_roots, [1] n_kept
-    uint8_t *maskbuf;       // [P] (only when the caller gave no mask)
-    uint32_t *rootbits;     // [NW+1]
-    uint32_t *rootprefix;   // [NW+1]
-    uint32_t *scanpart;     // [..]
-    int32_t *area;          // [maxroots]
-    uint32_t *keptprefix;   // [maxroots+1]
-    Acc *acc;               // [cap]
-    size_t P, NW, maxroots, npart;
+    uint32_t *counters;     // [0] n_rec, [1] n_kept
+    uint8_t *maskbuf;       // [P] (only used when the caller gave no mask)
+    uint32_t *edges;        // [ntiles * EDGE_WORDS]
+    uint32_t *reclist;      // [nblk2] 2x2-block ids of the records written by K4a
+    uint32_t *keptbits;     // [NWk] one bit per pixel  |
+    uint32_t *blkcnt;       // [NB + 1] per 4096 px     |  zeroed together every call
+    uint32_t *blkprefix;    // [NB + 2]
+    Rec *rec;               // [nblk2] direct-mapped by 2x2 block
+    size_t P, nblk2, NWk, NB, ntiles;
+    size_t zero_bytes;      // bytes from keptbits to the end of blkcnt
     size_t total;
 };
 
-size_t carve(Ws &w, void *base, int B, int H, int W, int64_t cap) {
-    size_t P = (size_t)B * H * W;
+size_t carve(Ws &w, void *base, int B, int H, int W) {
+    const size_t P = (size_t)B * H * W;
     w.P = P;
-    w.NW = (P + 31) / 32;
-    w.maxroots = (size_t)B * ((H + 1) / 2) * ((W + 1) / 2);
-    size_t nscan = (w.NW + 1 > w.maxroots ? w.NW + 1 : w.maxroots);
-    w.npart = (nscan + SCAN_ELEMS - 1) / SCAN_ELEMS + 2;
+    w.nblk2 = (size_t)B * ((H + 1) / 2) * (W / 2);
+    w.NWk = (P + 31) / 32 + 32;
+    w.NB = (P + 4095) / 4096;            // ranking blocks of 4096 pixels (RB_SHIFT)
+    w.ntiles = (size_t)B * ((H + TH - 1) / TH) * ((W + TW - 1) / TW);
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = bd_align_up(off + bytes, 256); return (char *)base + o; };
     w.counters = (uint32_t *)take(64 * sizeof(uint32_t));
     w.maskbuf = (uint8_t *)take(P);
-    w.rootbits = (uint32_t *)take((w.NW + 1) * sizeof(uint32_t));
-    w.rootprefix = (uint32_t *)take((w.NW + 2) * sizeof(uint32_t));
-    w.scanpart = (uint32_t *)take(w.npart * sizeof(uint32_t));
-    w.area = (int32_t *)take(w.maxroots * sizeof(int32_t));
-    w.keptprefix = (uint32_t *)take((w.maxroots + 1) * sizeof(uint32_t));
-    w.acc = (Acc *)take((size_t)(cap > 0 ? cap : 1) * sizeof(Acc));
+    w.edges = (uint32_t *)take(w.ntiles * EDGE_WORDS * sizeof(uint32_t));
+    w.reclist = (uint32_t *)take(w.nblk2 * sizeof(uint32_t));
+    w.keptbits = (uint32_t *)take(w.NWk * sizeof(uint32_t));
+    w.blkcnt = (uint32_t *)take((w.NB + 1) * sizeof(uint32_t));
+    w.zero_bytes = (size_t)((char *)w.blkcnt - (char *)w.keptbits) + (w.NB + 1) * sizeof(uint32_t);
+    w.blkprefix = (uint32_t *)take((w.NB + 2) * sizeof(uint32_t));
+    w.rec = (Rec *)take(w.nblk2 * sizeof(Rec));
     w.total = off;
     return off;
 }
@@ -79,108 +105,351 @@ __global__ void k_make_mask(const float *sub, const float *rms, size_t n4, doubl
     reinterpret_cast<uint32_t *>(mask)[i] = m;
 }
 
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// 4 mask bytes (non-zero = foreground) -> 4 bits
+__device__ __forceinline__ uint32_t bytes_to_nibble(uint32_t v) {
+    const uint32_t nz = ((((v & 0x7F7F7F7Fu) + 0x7F7F7F7Fu) | v) & 0x80808080u) >> 7;   // bits 0, 8, 16, 24
+    return (nz * 0x00204081u >> 21) & 0xFu;
+}
+
 // ------------------------------------------------------------------------------------------------ K4a
-__device__ __forceinline__ uint32_t sm_find(volatile uint32_t *parent, uint32_t x) {
-    uint32_t p = parent[x];
-    while (p != x) { x = p; p = parent[x]; }
+// shared-memory union-find on lab[]: a root points to itself, union by minimum index
+__device__ __forceinline__ uint32_t sm_find(volatile uint32_t *par, uint32_t x) {
+    uint32_t p = par[x];
+    while (p != x) { x = p; p = par[x]; }
     return x;
 }
-__device__ __noinline__ void sm_union(uint32_t *parent, uint32_t a, uint32_t b) {
+__device__ __noinline__ void sm_union(uint32_t *par, uint32_t a, uint32_t b) {
     for (;;) {
-        a = sm_find(parent, a);
-        b = sm_find(parent, b);
+        a = sm_find(par, a);
+        b = sm_find(par, b);
         if (a == b) return;
         if (a < b) { uint32_t t = a; a = b; b = t; }
-        uint32_t old = atomicMin(&parent[a], b);
+        uint32_t old = atomicMin(&par[a], b);
         if (old == a) return;
         a = old;
     }
 }
+// bits of columns x-1, x, x+1 of a bit row (bit 0 = x-1); x in [0, TW)
+__device__ __forceinline__ uint32_t get3(const uint32_t *row, int x) {
+    const int q = x + 31, j = q >> 5;
+    return __funnelshift_r(row[j], row[j + 1], q & 31) & 7u;
+}
 
-__global__ void __launch_bounds__(K4_NT) k4a_tile_label(const uint8_t *mask, int H, int W, int32_t *labels,
-                                                        uint32_t *rootbits, int aligned32) {
-    __shared__ uint32_t sm_mask[TH][TW / 4 + 1];
-    __shared__ uint32_t parent[TH * TW];
+struct K4Args {
+    const uint8_t *mask;
+    const float *sub;
+    int H, W, min_area, vec16, use_tma;
+    int32_t *labels;
+    uint32_t *edges;
+    Rec *rec;
+    uint32_t *reclist;
+    uint32_t *counters;
+};
+
+constexpr int SM_LAB = 0;
+constexpr int SM_LIST = SM_LAB + TPX * 4;
+constexpr int SM_BITS = SM_LIST + TPX * 2;
+constexpr int SM_STATD = SM_BITS + 1600;              // BROWS * BWORDS * 4 = 1584, padded
+constexpr int SM_PEAK = SM_STATD + 6 * NS * 8;
+constexpr int SM_BOX = SM_PEAK + NS * 8;
+constexpr int SM_MISC = SM_BOX + 4 * NS * 4;
+constexpr int K4_SMEM = SM_MISC + 32 * 4;
+
+__global__ void __launch_bounds__(K4_NT) k4a_tile_label(const __grid_constant__ CUtensorMap tmap_lab, K4Args a) {
+    extern __shared__ __align__(128) unsigned char sm[];
+    uint32_t *lab = reinterpret_cast<uint32_t *>(sm + SM_LAB);
+    uint16_t *list = reinterpret_cast<uint16_t *>(sm + SM_LIST);
+    uint32_t(*bits)[BWORDS] = reinterpret_cast<uint32_t(*)[BWORDS]>(sm + SM_BITS);
+    double(*s_d)[NS] = reinterpret_cast<double(*)[NS]>(sm + SM_STATD);
+    u64 *s_peak = reinterpret_cast<u64 *>(sm + SM_PEAK);
+    int(*s_box)[NS] = reinterpret_cast<int(*)[NS]>(sm + SM_BOX);
+    uint32_t *wsum = reinterpret_cast<uint32_t *>(sm + SM_MISC);   // [16] warp totals, [16] n_rec, [17] g_base
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int frame = blockIdx.z;
     const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;
+    const int H = a.H, W = a.W;
     const size_t fbase = (size_t)frame * H * W;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int rx0 = lane * 4;
-    const bool col_ok = (x0 + rx0) < W;
+    const size_t tile = ((size_t)frame * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
 
+    // ---- A: zero the label tile, mask bytes -> bit rows with halo ----------------------------------------
 #pragma unroll
-    for (int k = 0; k < TH / 8; ++k) {
-        int ry = warp + 8 * k;
-        uint32_t m = 0;
-        if (col_ok && (y0 + ry) < H) {
-            m = __ldcs(reinterpret_cast<const uint32_t *>(mask + fbase + (size_t)(y0 + ry) * W + x0 + rx0));
-            m = ((((m & 0x7F7F7F7Fu) + 0x7F7F7F7Fu) | m) & 0x80808080u) >> 7;   // bytes -> 0/1
+    for (int k = 0; k < TPX / 4 / K4_NT; ++k) reinterpret_cast<uint4 *>(lab)[k * K4_NT + tid] = make_uint4(0, 0, 0, 0);
+    if (tid == 0) wsum[16] = 0;
+    if (tid < BROWS * 4) {
+        const int hr = tid >> 2, w = tid & 3;
+        const int y = y0 - 1 + hr, x = x0 + 32 * w;
+        uint32_t word = 0;
+        if (y >= 0 && y < H && x < W) {
+            const uint8_t *src = a.mask + fbase + (size_t)y * W + x;
+            if (a.vec16) {
+                if (x + 16 <= W) {
+                    const uint4 v = __ldg(reinterpret_cast<const uint4 *>(src));
+                    word = bytes_to_nibble(v.x) | bytes_to_nibble(v.y) << 4 | bytes_to_nibble(v.z) << 8 | bytes_to_nibble(v.w) << 12;
+                }
+                if (x + 32 <= W) {
+                    const uint4 v = __ldg(reinterpret_cast<const uint4 *>(src + 16));
+                    word |= (bytes_to_nibble(v.x) | bytes_to_nibble(v.y) << 4 | bytes_to_nibble(v.z) << 8 | bytes_to_nibble(v.w) << 12) << 16;
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < 8; ++k)
+                    if (x + 4 * k < W) word |= bytes_to_nibble(__ldg(reinterpret_cast<const uint32_t *>(src + 4 * k))) << (4 * k);
+            }
         }
-        sm_mask[ry][lane] = m;
-#pragma unroll
-        for (int q = 0; q < 4; ++q) parent[ry * TW + rx0 + q] = ry * TW + rx0 + q;
+        bits[hr][1 + w] = word;
+    } else if (tid < BROWS * 4 + BROWS * 2) {
+        const int h = tid - BROWS * 4, hr = h >> 1, side = h & 1;
+        const int y = y0 - 1 + hr, x = side ? x0 + TW : x0 - 1;
+        uint32_t bit = 0;
+        if (y >= 0 && y < H && x >= 0 && x < W) bit = __ldg(a.mask + fbase + (size_t)y * W + x) ? 1u : 0u;
+        bits[hr][side ? 5 : 0] = side ? bit : bit << 31;
     }
     __syncthreads();
 
-    auto fg = [&](int ry, int rx) -> uint32_t {
-        if (ry < 0 || rx < 0 || rx >= TW) return 0u;
-        return (sm_mask[ry][rx >> 2] >> (8 * (rx & 3))) & 1u;
-    };
-    // not unrolled on purpose: the unrolled body (16 pixels x 4 inlined union loops) was 85 KB of SASS and
-    // the kernel was instruction-fetch bound (ncu: 65% stall_no_inst)
-#pragma unroll 1
-    for (int k = 0; k < TH / 8; ++k) {
-        int ry = warp + 8 * k;
-        uint32_t m = sm_mask[ry][lane];
-        if (!m) continue;
-#pragma unroll 1
-        for (int q = 0; q < 4; ++q) {
-            if (!((m >> (8 * q)) & 1u)) continue;
-            int rx = rx0 + q;
-            uint32_t p = ry * TW + rx;
-            uint32_t w = fg(ry, rx - 1), a = fg(ry - 1, rx - 1), b = fg(ry - 1, rx), c = fg(ry - 1, rx + 1);
-            if (w) sm_union(parent, p, p - 1);
-            if (b) { if (!w) sm_union(parent, p, p - TW); }
+    // border bit rows / columns for the seam merge
+    {
+        uint32_t *e = a.edges + tile * EDGE_WORDS;
+        if (tid < 4) e[tid] = bits[1][1 + tid];
+        else if (tid < 8) e[tid] = bits[TH][1 + tid - 4];
+        if (warp == 1 || warp == 2) {
+            const int row = tid - 32;
+            const uint32_t bl = __ballot_sync(0xffffffffu, bits[row + 1][1] & 1u);
+            const uint32_t br = __ballot_sync(0xffffffffu, bits[row + 1][4] >> 31);
+            if (lane == 0) { e[8 + warp - 1] = bl; e[10 + warp - 1] = br; }
+        }
+    }
+
+    // ---- B: compact list of foreground pixels (raster order); parent = start of the horizontal run ----------
+    uint32_t M = 0, prevbit = 0;
+    int row_w = 0, w_w = 0;
+    if (tid < TH * 4) {
+        row_w = tid >> 2; w_w = tid & 3;
+        M = bits[row_w + 1][1 + w_w];
+        prevbit = w_w ? bits[row_w + 1][w_w] >> 31 : 0u;
+    }
+    uint32_t incl = __popc(M);
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    if (lane == 31) wsum[warp] = incl;
+    __syncthreads();
+    uint32_t pos = incl - __popc(M);
+    int n = 0;
+#pragma unroll
+    for (int k = 0; k < K4_NT / 32; ++k) {
+        const uint32_t t = wsum[k];
+        if (k < warp) pos += t;
+        n += (int)t;
+    }
+    if (M) {
+        const uint32_t pbase = (uint32_t)(row_w * TW + w_w * 32);
+        uint32_t m = M, cur = 0;
+        while (m) {
+            const int i = __ffs(m) - 1;
+            m &= m - 1;
+            const uint32_t p = pbase + i;
+            const bool cont = i ? ((M >> (i - 1)) & 1u) : prevbit;
+            if (!cont) cur = p;
+            else if (i == 0) cur = p - 1;
+            lab[p] = cur;
+            list[pos++] = (uint16_t)p;
+        }
+    }
+    __syncthreads();
+
+    if (n > 0) {
+        // ---- C: vertical / diagonal links inside the tile (pruned: DESIGN.md section 6, K4) ------------------
+        for (int e = tid; e < n; e += K4_NT) {
+            const uint32_t p = list[e];
+            const int r = (int)(p >> 7), x = (int)(p & 127);
+            if (r == 0) continue;
+            const uint32_t u3 = get3(bits[r], x), m3 = get3(bits[r + 1], x);
+            // in-tile bits only (a halo pixel never prunes an in-tile link): the tile-local components are then
+            // exactly the components of the tile's own mask, so two tile-local roots never share a 2x2 block
+            const bool w = (m3 & 1u) && x > 0, na = u3 & 1u, nb = u3 & 2u, nc = u3 & 4u;
+            if (nb) { if (!w) sm_union(lab, p, p - TW); }
             else {
-                if (a && !w) sm_union(parent, p, p - TW - 1);
-                if (c) sm_union(parent, p, p - TW + 1);
+                if (na && !w && x > 0) sm_union(lab, p, p - TW - 1);
+                if (nc && x < TW - 1) sm_union(lab, p, p - TW + 1);
             }
+        }
+        __syncthreads();
+        // ---- D1: flatten ------------------------------------------------------------------------------------
+        for (int e = tid; e < n; e += K4_NT) {
+            const uint32_t p = list[e];
+            const uint32_t r = sm_find(lab, p);
+            if (r != p) lab[p] = r;
+        }
+        __syncthreads();
+        // ---- D2a: roots become counters ---------------------------------------------------------------------
+        for (int e = tid; e < n; e += K4_NT) {
+            const uint32_t p = list[e];
+            if (lab[p] == p) lab[p] = F_ROOT;
+        }
+        __syncthreads();
+        // ---- D2b: pixel counts (one atomic per run of equal roots in the list) and ring flags ----------------
+        for (int e0 = 0; e0 < n; e0 += K4_NT) {
+            const int e = e0 + tid;
+            const bool valid = e < n;
+            uint32_t p = 0, r = 0xFFFF0000u | lane;
+            bool ring = false;
+            if (valid) {
+                p = list[e];
+                const uint32_t own = lab[p];
+                r = (own & F_ROOT) ? p : own;
+                const int row = (int)(p >> 7), x = (int)(p & 127);
+                if (row == 0 || row == TH - 1 || x == 0 || x == TW - 1) {
+                    const uint32_t u3 = get3(bits[row], x), m3 = get3(bits[row + 1], x), d3 = get3(bits[row + 2], x);
+                    uint32_t out = 0;
+                    if (row == 0) out |= u3;
+                    if (row == TH - 1) out |= d3;
+                    if (x == 0) out |= (u3 | m3 | d3) & 1u;
+                    if (x == TW - 1) out |= (u3 | m3 | d3) & 4u;
+                    ring = out != 0;
+                }
+            }
+            const uint32_t prev = __shfl_up_sync(0xffffffffu, r, 1);
+            const bool head = lane == 0 || prev != r;
+            const uint32_t hm = __ballot_sync(0xffffffffu, head);
+            const uint32_t rest = lane == 31 ? 0u : hm & ~((2u << lane) - 1u);
+            const int tail = rest ? __ffs(rest) - 2 : 31;
+            if (valid && head) atomicAdd(&lab[r], (uint32_t)(tail - lane + 1));
+            if (ring) atomicOr(&lab[r], F_RING);
+        }
+        __syncthreads();
+        // ---- E: record slots for components that can matter ---------------------------------------------------
+        for (int e = tid; e < n; e += K4_NT) {
+            const uint32_t p = list[e];
+            const uint32_t own = lab[p];
+            if ((own & F_ROOT) && ((int)(own & CNT_MASK) >= a.min_area || (own & F_RING))) {
+                const uint32_t slot = atomicAdd(&wsum[16], 1u);
+                lab[p] = own | F_REC | (slot << SLOT_SHIFT);
+            }
+        }
+        __syncthreads();
+        const int nrec = (int)wsum[16];
+        if (nrec > 0 && tid == 0) wsum[17] = atomicAdd(a.counters + 0, (uint32_t)nrec);
+        // ---- F: partial sums of the recorded components, NS slots at a time ----------------------------------
+        for (int b0 = 0; b0 < nrec; b0 += NS) {
+            if (tid < NS) {
+#pragma unroll
+                for (int k = 0; k < 6; ++k) s_d[k][tid] = 0.0;
+                s_peak[tid] = 0ull;
+                s_box[0][tid] = 0x7FFFFFFF; s_box[1][tid] = -1; s_box[2][tid] = 0x7FFFFFFF; s_box[3][tid] = -1;
+            }
+            __syncthreads();
+            for (int e0 = 0; e0 < n; e0 += K4_NT) {
+                const int e = e0 + tid;
+                uint32_t key = 0xFFFF0000u | lane;
+                int s = 0, x = 0, row = 0;
+                double S0 = 0.0, S1 = 0.0, S2 = 0.0, dy = 0.0;
+                u64 pk = 0;
+                bool in = false;
+                if (e < n) {
+                    const uint32_t p = list[e];
+                    const uint32_t own = lab[p];
+                    const uint32_t r = (own & F_ROOT) ? p : own;
+                    const uint32_t rw = (own & F_ROOT) ? own : lab[r];
+                    s = (int)((rw >> SLOT_SHIFT) & 0x7FFu) - b0;
+                    in = (rw & F_REC) && s >= 0 && s < NS;
+                    if (in) {
+                        row = (int)(p >> 7); x = (int)(p & 127);
+                        key = ((uint32_t)(s + b0) << 6) | (uint32_t)row;
+                        const int gidx = (y0 + row) * W + x0 + x;
+                        const float I = __ldg(a.sub + fbase + (size_t)gidx);
+                        const double dx = (double)(x - (int)(r & 127));
+                        dy = (double)(row - (int)(r >> 7));
+                        S0 = (double)I; S1 = S0 * dx; S2 = S1 * dx;
+                        pk = ((u64)f32_to_key(I) << 32) | (u64)(0xFFFFFFFFu - (uint32_t)gidx);
+                    }
+                }
+                const uint32_t prev = __shfl_up_sync(0xffffffffu, key, 1);
+                const bool head = lane == 0 || prev != key;
+                const uint32_t hm = __ballot_sync(0xffffffffu, head);
+                if (hm == 0xffffffffu && !__any_sync(0xffffffffu, in)) continue;   // nothing recorded in this warp
+                const uint32_t rest = lane == 31 ? 0u : hm & ~((2u << lane) - 1u);
+                const int tail = rest ? __ffs(rest) - 2 : 31;
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const double o0 = __shfl_down_sync(0xffffffffu, S0, d), o1 = __shfl_down_sync(0xffffffffu, S1, d);
+                    const double o2 = __shfl_down_sync(0xffffffffu, S2, d);
+                    const u64 opk = __shfl_down_sync(0xffffffffu, pk, d);
+                    if (lane + d <= tail) { S0 += o0; S1 += o1; S2 += o2; pk = opk > pk ? opk : pk; }
+                }
+                const int xlast = __shfl_sync(0xffffffffu, x, tail);
+                if (in && head) {   // one flush per (component, row) run
+                    atomicAdd(&s_d[0][s], S0);
+                    atomicAdd(&s_d[1][s], S1);
+                    atomicAdd(&s_d[2][s], dy * S0);
+                    atomicAdd(&s_d[3][s], S2);
+                    atomicAdd(&s_d[4][s], dy * dy * S0);
+                    atomicAdd(&s_d[5][s], dy * S1);
+                    atomicMax(&s_peak[s], pk);
+                    atomicMin(&s_box[0][s], x0 + x); atomicMax(&s_box[1][s], x0 + xlast);
+                    atomicMin(&s_box[2][s], y0 + row); atomicMax(&s_box[3][s], y0 + row);
+                }
+            }
+            __syncthreads();
+            const uint32_t gbase = wsum[17];
+            for (int e = tid; e < n; e += K4_NT) {
+                const uint32_t p = list[e];
+                const uint32_t own = lab[p];
+                if (!(own & F_ROOT) || !(own & F_REC)) continue;
+                const int slot = (int)((own >> SLOT_SHIFT) & 0x7FFu), s = slot - b0;
+                if (s < 0 || s >= NS) continue;
+                const int gy = y0 + (int)(p >> 7), gx = x0 + (int)(p & 127);
+                const size_t blk = ((size_t)frame * ((H + 1) / 2) + (gy >> 1)) * (W / 2) + (gx >> 1);
+                Rec rr;
+                rr.f = s_d[0][s]; rr.sx = s_d[1][s]; rr.sy = s_d[2][s]; rr.sxx = s_d[3][s]; rr.syy = s_d[4][s]; rr.sxy = s_d[5][s];
+                rr.peak = s_peak[s];
+                rr.root = gy * W + gx; rr.frame = frame; rr.npix = (int)(own & CNT_MASK);
+                rr.xmin = s_box[0][s]; rr.xmax = s_box[1][s]; rr.ymin = s_box[2][s]; rr.ymax = s_box[3][s];
+                rr.pad[0] = rr.pad[1] = rr.pad[2] = 0;
+                uint4 *dst = reinterpret_cast<uint4 *>(a.rec + blk);
+                const uint4 *srcv = reinterpret_cast<const uint4 *>(&rr);
+#pragma unroll
+                for (int k = 0; k < 6; ++k) dst[k] = srcv[k];
+                a.reclist[gbase + slot] = (uint32_t)blk;
+            }
+            __syncthreads();
+        }
+        // ---- G: parents -> labels (1 + raster index of the tile-local root) ------------------------------------
+        for (int e = tid; e < n; e += K4_NT) {
+            const uint32_t p = list[e];
+            const uint32_t own = lab[p];
+            const uint32_t r = (own & F_ROOT) ? p : own;
+            lab[p] = (uint32_t)((y0 + (int)(r >> 7)) * W + x0 + (int)(r & 127) + 1);
         }
     }
-    __syncthreads();
 
-#pragma unroll 1
-    for (int k = 0; k < TH / 8; ++k) {
-        int ry = warp + 8 * k;
-        bool row_ok = col_ok && (y0 + ry) < H;
-        uint32_t m = sm_mask[ry][lane];
-        int out[4];
-        uint32_t nib = 0;
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            out[q] = 0;
-            if ((m >> (8 * q)) & 1u) {
-                uint32_t p = ry * TW + rx0 + q;
-                uint32_t r = sm_find(parent, p);
-                out[q] = (y0 + (int)(r / TW)) * W + x0 + (int)(r % TW) + 1;
-                if (r == p) nib |= 1u << q;
-            }
+    // ---- H: the label tile leaves shared memory ----------------------------------------------------------------
+    if (a.use_tma) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+        if (tid == 0) {
+            asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(&tmap_lab),
+                         "r"(x0), "r"(y0), "r"(frame), "r"(smem_u32(lab))
+                         : "memory");
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         }
-        size_t g = fbase + (size_t)(y0 + ry) * W + x0 + rx0;
-        if (row_ok) __stcg(reinterpret_cast<int4 *>(labels + g), make_int4(out[0], out[1], out[2], out[3]));
-        if (aligned32) {
-            uint32_t word = nib << (4 * (lane & 7));
-            word |= __shfl_xor_sync(0xffffffffu, word, 1);
-            word |= __shfl_xor_sync(0xffffffffu, word, 2);
-            word |= __shfl_xor_sync(0xffffffffu, word, 4);
-            if (row_ok && (lane & 7) == 0) rootbits[g >> 5] = word;
-        } else if (row_ok && nib) {
-            atomicOr(&rootbits[g >> 5], nib << (g & 31));
+    } else {
+        __syncthreads();
+        for (int i = tid; i < TPX / 4; i += K4_NT) {
+            const int r = i >> 5, c = (i & 31) * 4;
+            if (y0 + r < H && x0 + c < W)
+                __stcg(reinterpret_cast<uint4 *>(a.labels + fbase + (size_t)(y0 + r) * W + x0 + c), reinterpret_cast<const uint4 *>(lab)[i]);
         }
     }
 }
 
 // ------------------------------------------------------------------------------------------------ K4b
+// global union-find on the label array of one frame: L[a] = 1 + parent of a; a root has L[a] = a + 1
 __device__ __forceinline__ int g_find(const int32_t *L, int a) {
     for (;;) {
         int p = __ldcg(L + a) - 1;
@@ -188,317 +457,224 @@ __device__ __forceinline__ int g_find(const int32_t *L, int a) {
         a = p;
     }
 }
-__device__ __forceinline__ void g_union(int32_t *L, uint32_t *rootbits, size_t fbase, int a, int b) {
+__device__ __forceinline__ void g_union(int32_t *L, int a, int b) {
     for (;;) {
         a = g_find(L, a);
         b = g_find(L, b);
         if (a == b) return;
         if (a < b) { int t = a; a = b; b = t; }
         int old = atomicMin(L + a, b + 1);
-        if (old == a + 1) {   // a was a root and now hangs under b
-            size_t g = fbase + (size_t)a;
-            atomicAnd(&rootbits[g >> 5], ~(1u << (g & 31)));
-            return;
-        }
+        if (old == a + 1) return;   // a was a root and now hangs under b
         a = old - 1;
     }
 }
 
-// horizontal seams: row y = k*TH (k >= 1) against row y-1, all x
-__global__ void k4b_seam_h(const uint8_t *mask, int H, int W, int32_t *labels, uint32_t *rootbits) {
-    const int frame = blockIdx.z, seam = blockIdx.y + 1;
-    const int y = seam * TH;
-    const int x = blockIdx.x * blockDim.x + threadIdx.x;
-    if (y >= H || x >= W) return;
-    const size_t fbase = (size_t)frame * H * W;
-    const uint8_t *m = mask + fbase;
-    if (!m[(size_t)y * W + x]) return;
-    int32_t *L = labels + fbase;
-    const int p = y * W + x;
-    const uint8_t *up = m + (size_t)(y - 1) * W;
-    bool b = up[x], a = x > 0 && up[x - 1], c = x + 1 < W && up[x + 1];
-    if (b) g_union(L, rootbits, fbase, p, p - W);
-    else {
-        if (a) g_union(L, rootbits, fbase, p, p - W - 1);
-        if (c) g_union(L, rootbits, fbase, p, p - W + 1);
+// One thread per (tile, unit): units 0..3 = the four 32-pixel words of the tile's top row against the bottom
+// row of the tile above (links N, NW, NE of row-0 pixels); units 4, 5 = the two 32-row words of the tile's left
+// column against the right column of the tile to the left (link W of column-0 pixels, NW of column-0 pixels and
+// NE of the left tile's last column, rows >= 1 of the tile; row 0 belongs to units 0..3).  The conditions are
+// the same pruned rules K4a applies inside a tile, evaluated on the true neighbour bits.
+__global__ void __launch_bounds__(256) k4b_seams(const uint32_t *edges, int32_t *labels, int H, int W, int TX, int TY,
+                                                 size_t n_units) {
+    const size_t u = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= n_units) return;
+    const int unit = (int)(u % 6);
+    const size_t tile = u / 6;
+    const int tx = (int)(tile % TX), ty = (int)((tile / TX) % TY);
+    const size_t frame = tile / ((size_t)TX * TY);
+    int32_t *L = labels + frame * (size_t)H * W;
+    const uint32_t *E = edges + tile * EDGE_WORDS;
+    const int x0 = tx * TW, y0 = ty * TH;
+    if (unit < 4) {
+        if (ty == 0) return;
+        const int k = unit;
+        const uint32_t M = E[k];
+        if (!M) return;
+        const uint32_t *EU = E - (size_t)TX * EDGE_WORDS;   // tile above
+        const uint32_t Uc = EU[4 + k];
+        uint32_t lc, rc, ml;
+        if (k > 0) { lc = EU[4 + k - 1] >> 31; ml = E[k - 1] >> 31; }
+        else if (tx > 0) { lc = (EU - EDGE_WORDS)[4 + 3] >> 31; ml = (E - EDGE_WORDS)[3] >> 31; }
+        else { lc = 0; ml = 0; }
+        if (k < 3) rc = EU[4 + k + 1] & 1u;
+        else if (tx + 1 < TX) rc = (EU + EDGE_WORDS)[4] & 1u;
+        else rc = 0;
+        const uint32_t na = (Uc << 1) | lc, nb = Uc, nc = (Uc >> 1) | (rc << 31), wb = (M << 1) | ml;
+        uint32_t tN = M & ~wb & nb, tNW = M & ~wb & ~nb & na, tNE = M & ~nb & nc;
+        const int pbase = y0 * W + x0 + 32 * k;
+        while (tN) { const int i = __ffs(tN) - 1; tN &= tN - 1; g_union(L, pbase + i, pbase + i - W); }
+        while (tNW) { const int i = __ffs(tNW) - 1; tNW &= tNW - 1; g_union(L, pbase + i, pbase + i - W - 1); }
+        while (tNE) { const int i = __ffs(tNE) - 1; tNE &= tNE - 1; g_union(L, pbase + i, pbase + i - W + 1); }
+    } else {
+        if (tx == 0) return;
+        const int h = unit - 4;
+        const uint32_t *EA = E - EDGE_WORDS;   // tile to the left
+        const uint32_t R = E[8 + h], Lc = EA[10 + h];
+        if (!(R | Lc)) return;
+        const uint32_t cl = h ? EA[10] >> 31 : 0u, cr = h ? E[8] >> 31 : 0u;
+        const uint32_t Lup = (Lc << 1) | cl, Rup = (R << 1) | cr;
+        const uint32_t rows = h ? 0xFFFFFFFFu : 0xFFFFFFFEu;   // row 0 of the tile: units 0..3
+        uint32_t tW = R & Lc, tNW = R & ~Lc & ~Rup & Lup & rows, tNE = Lc & ~Lup & Rup & rows;
+        const int ybase = y0 + 32 * h;
+        while (tW) { const int i = __ffs(tW) - 1; tW &= tW - 1; const int p = (ybase + i) * W + x0; g_union(L, p, p - 1); }
+        while (tNW) { const int i = __ffs(tNW) - 1; tNW &= tNW - 1; const int p = (ybase + i) * W + x0; g_union(L, p, p - W - 1); }
+        while (tNE) { const int i = __ffs(tNE) - 1; tNE &= tNE - 1; const int q = (ybase + i) * W + x0 - 1; g_union(L, q, q - W + 1); }
     }
 }
 
-// vertical seams: columns x-1 | x with x = k*TW (k >= 1), all y; the 2x2 block (y-1..y) x (x-1..x)
-__global__ void k4b_seam_v(const uint8_t *mask, int H, int W, int32_t *labels, uint32_t *rootbits) {
-    const int frame = blockIdx.z, seam = blockIdx.y + 1;
-    const int x = seam * TW;
-    const int y = blockIdx.x * blockDim.x + threadIdx.x;
-    if (x >= W || y >= H) return;
-    const size_t fbase = (size_t)frame * H * W;
-    const uint8_t *m = mask + fbase;
-    int32_t *L = labels + fbase;
-    const bool m10 = m[(size_t)y * W + x - 1], m11 = m[(size_t)y * W + x];
-    if (!m10 && !m11) return;
-    const bool m00 = y > 0 && m[(size_t)(y - 1) * W + x - 1], m01 = y > 0 && m[(size_t)(y - 1) * W + x];
-    const int p = y * W + x;
-    if (m10 && m11) g_union(L, rootbits, fbase, p, p - 1);
-    if (m11 && m00 && !m01) g_union(L, rootbits, fbase, p, p - W - 1);
-    if (m10 && m01 && !m00) g_union(L, rootbits, fbase, p - 1, p - W);
+// ------------------------------------------------------------------------------------------------ K5
+__device__ __forceinline__ size_t blk2_of(int frame, int r, int H, int W) {
+    const int y = r / W, x = r - y * W;
+    return ((size_t)frame * ((H + 1) / 2) + (y >> 1)) * (W / 2) + (x >> 1);
 }
 
-// ------------------------------------------------------------------------------------------------ scans
-// MODE 0: popc(bits[i]), i < n (host n).  MODE 1: (area[i] >= min_area), i < *n_dev.
-struct ScanArgs {
-    const uint32_t *bits;
-    const int32_t *area;
-    const uint32_t *n_dev;
-    size_t n;
-    int min_area;
-    uint32_t *out;        // [n+1] exclusive prefix, out[n] = total
-    uint32_t *part;
-    uint32_t *total_out;
-};
-template <int MODE>
-__device__ __forceinline__ uint32_t scan_load(const ScanArgs &a, size_t i, size_t n) {
-    if (i >= n) return 0;
-    if (MODE == 0) return __popc(a.bits[i]);
-    return a.area[i] >= a.min_area ? 1u : 0u;
-}
-template <int MODE>
-__global__ void __launch_bounds__(SCAN_NT) scan_reduce(ScanArgs a) {
-    __shared__ uint32_t red[SCAN_NT / 32];
-    const size_t n = MODE == 0 ? a.n : (size_t)*a.n_dev;
-    const size_t b0 = (size_t)blockIdx.x * SCAN_ELEMS;
-    uint32_t s = 0;
-    if (b0 < n)
-        for (int k = 0; k < SCAN_PER; ++k) s += scan_load<MODE>(a, b0 + (size_t)k * SCAN_NT + threadIdx.x, n);
-    for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        uint32_t t = 0;
-        for (int w = 0; w < SCAN_NT / 32; ++w) t += red[w];
-        a.part[blockIdx.x] = t;
+// K5m: records whose tile-local root was linked under another root are added to the final root's record and
+// their pixels relabelled.  One thread looks at one record; the warp then serves its changed records together.
+__global__ void __launch_bounds__(256) k5m_merge_relabel(const uint32_t *reclist, const uint32_t *counters, Rec *rec,
+                                                         int32_t *labels, int H, int W) {
+    const uint32_t n = counters[0];
+    const int lane = threadIdx.x & 31;
+    const size_t HW = (size_t)H * W;
+    for (size_t base = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) & ~(size_t)31; base < n; base += (size_t)gridDim.x * blockDim.x) {
+        const size_t i = base + lane;
+        uint32_t blk = 0;
+        int r = 0, R = 0, frame = 0;
+        if (i < n) {
+            blk = reclist[i];
+            r = rec[blk].root; frame = rec[blk].frame;
+            R = g_find(labels + (size_t)frame * HW, r);
+        }
+        uint32_t todo = __ballot_sync(0xffffffffu, R != r);
+        while (todo) {
+            const int j = __ffs(todo) - 1;
+            todo &= todo - 1;
+            const uint32_t cb = __shfl_sync(0xffffffffu, blk, j);
+            const int cr = __shfl_sync(0xffffffffu, r, j), cR = __shfl_sync(0xffffffffu, R, j), cf = __shfl_sync(0xffffffffu, frame, j);
+            const Rec *c = rec + cb;
+            Rec *T = rec + blk2_of(cf, cR, H, W);
+            int32_t *L = labels + (size_t)cf * HW;
+            const int yc = cr / W, xc = cr - yc * W, yR = cR / W, xR = cR - yR * W;
+            const double ox = (double)(xc - xR), oy = (double)(yc - yR);
+            const double f = c->f, sx = c->sx, sy = c->sy;
+            switch (lane) {
+                case 0: atomicAdd(&T->f, f); break;
+                case 1: atomicAdd(&T->sx, sx + f * ox); break;
+                case 2: atomicAdd(&T->sy, sy + f * oy); break;
+                case 3: atomicAdd(&T->sxx, c->sxx + 2.0 * ox * sx + ox * ox * f); break;
+                case 4: atomicAdd(&T->syy, c->syy + 2.0 * oy * sy + oy * oy * f); break;
+                case 5: atomicAdd(&T->sxy, c->sxy + ox * sy + oy * sx + ox * oy * f); break;
+                case 6: atomicMax(&T->peak, c->peak); break;
+                case 7: atomicAdd(&T->npix, c->npix); break;
+                case 8: atomicMin(&T->xmin, c->xmin); break;
+                case 9: atomicMax(&T->xmax, c->xmax); break;
+                case 10: atomicMin(&T->ymin, c->ymin); break;
+                case 11: atomicMax(&T->ymax, c->ymax); break;
+                case 12: L[cr] = cR + 1; break;
+                default: break;
+            }
+            const int bx = c->xmin, by = c->ymin, bw = c->xmax - bx + 1, bh = c->ymax - by + 1;
+            const int old = cr + 1, neu = cR + 1;
+            for (int k = lane; k < bw * bh; k += 32) {
+                const int yy = by + k / bw, xx = bx + k - (k / bw) * bw;
+                int32_t *q = L + (size_t)yy * W + xx;
+                if (*q == old) *q = neu;
+            }
+        }
     }
 }
-__global__ void __launch_bounds__(1024) scan_top(uint32_t *part, size_t nblk, uint32_t *total_out) {
+
+constexpr int RB_SHIFT = 12;   // ranking blocks of 4096 pixels (128 bitmap words)
+
+// K5k: final roots with npix >= min_area -> bit in the per-pixel bitmap, count in the 4096-pixel block
+__global__ void __launch_bounds__(256) k5k_mark_kept(const uint32_t *reclist, const uint32_t *counters, const Rec *rec,
+                                                     const int32_t *labels, int H, int W, int min_area, uint32_t *keptbits,
+                                                     uint32_t *blkcnt) {
+    const uint32_t n = counters[0];
+    const size_t HW = (size_t)H * W;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const Rec *c = rec + reclist[i];
+        const int r = c->root, frame = c->frame;
+        if (c->npix < min_area) continue;
+        const size_t g = (size_t)frame * HW + r;
+        if (__ldcg(labels + g) != r + 1) continue;
+        atomicOr(&keptbits[g >> 5], 1u << (g & 31));
+        atomicAdd(&blkcnt[g >> RB_SHIFT], 1u);
+    }
+}
+
+// K5s: exclusive scan of the block counts (one CTA; thread t owns a contiguous chunk), total -> *total_out
+__global__ void __launch_bounds__(1024) k5s_scan_blocks(const uint32_t *cnt, size_t n, uint32_t *prefix, uint32_t *total_out) {
     __shared__ uint32_t red[32];
-    __shared__ uint32_t carry_s;
-    if (threadIdx.x == 0) carry_s = 0;
-    __syncthreads();
-    for (size_t base = 0; base < nblk; base += 1024) {
-        size_t i = base + threadIdx.x;
-        uint32_t v = i < nblk ? part[i] : 0, incl = v;
-        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-        for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
-        if (lane == 31) red[warp] = incl;
-        __syncthreads();
-        uint32_t wbase = 0;
-        for (int w = 0; w < warp; ++w) wbase += red[w];
-        uint32_t carry = carry_s;
-        if (i < nblk) part[i] = carry + wbase + incl - v;
-        __syncthreads();
-        if (threadIdx.x == 1023) carry_s = carry + wbase + incl;
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) *total_out = carry_s;
-}
-template <int MODE>
-__global__ void __launch_bounds__(SCAN_NT) scan_apply(ScanArgs a) {
-    __shared__ uint32_t red[SCAN_NT / 32];
-    const size_t n = MODE == 0 ? a.n : (size_t)*a.n_dev;
-    const size_t b0 = (size_t)blockIdx.x * SCAN_ELEMS;
-    if (b0 > n) return;
-    // thread t owns SCAN_PER consecutive elements
-    const size_t t0 = b0 + (size_t)threadIdx.x * SCAN_PER;
-    uint32_t v[SCAN_PER], local = 0;
-#pragma unroll
-    for (int k = 0; k < SCAN_PER; ++k) { v[k] = scan_load<MODE>(a, t0 + k, n); local += v[k]; }
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const size_t per = (n + 1023) / 1024, i0 = (size_t)tid * per, i1 = i0 + per < n ? i0 + per : n;
+    uint32_t local = 0;
+    for (size_t i = i0; i < i1; ++i) local += cnt[i];
     uint32_t incl = local;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
     for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
     if (lane == 31) red[warp] = incl;
     __syncthreads();
-    uint32_t run = a.part[blockIdx.x] + incl - local;
-    for (int w = 0; w < warp; ++w) run += red[w];
-#pragma unroll
-    for (int k = 0; k < SCAN_PER; ++k) {
-        if (t0 + k <= n) a.out[t0 + k] = run;   // also writes out[n] = total
-        run += v[k];
+    uint32_t run = incl - local, tot = 0;
+    for (int w = 0; w < 32; ++w) { if (w < warp) run += red[w]; tot += red[w]; }
+    for (size_t i = i0; i < i1; ++i) { const uint32_t c = cnt[i]; prefix[i] = run; run += c; }
+    if (tid == 0) { prefix[n] = tot; *total_out = tot; }
+}
+
+// number of kept roots with global pixel index < g
+__device__ __forceinline__ uint32_t kept_rank(const uint32_t *keptbits, const uint32_t *blkprefix, size_t g) {
+    const size_t w0 = (g >> RB_SHIFT) << (RB_SHIFT - 5), w1 = g >> 5;
+    uint32_t rank = blkprefix[g >> RB_SHIFT];
+    for (size_t w = w0; w < w1; ++w) rank += __popc(__ldg(keptbits + w));
+    return rank + __popc(__ldg(keptbits + w1) & ((1u << (g & 31)) - 1u));
+}
+
+// K5f: catalogue records in ascending (frame, label) order; per-frame counts
+__global__ void __launch_bounds__(256) k5f_finalize(const uint32_t *reclist, const uint32_t *counters, const Rec *rec,
+                                                    const int32_t *labels, int B, int H, int W, int min_area,
+                                                    const uint32_t *keptbits, const uint32_t *blkprefix, bd_source *cat,
+                                                    int64_t cap, int64_t *n_sources) {
+    const uint32_t n = counters[0];
+    const size_t HW = (size_t)H * W;
+    const size_t t0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t0 < (size_t)B)
+        n_sources[t0] = (int64_t)kept_rank(keptbits, blkprefix, (t0 + 1) * HW) - (int64_t)kept_rank(keptbits, blkprefix, t0 * HW);
+    if (!cat || cap <= 0) return;
+    for (size_t i = t0; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const Rec *c = rec + reclist[i];
+        const int r = c->root, frame = c->frame;
+        if (c->npix < min_area) continue;
+        const size_t g = (size_t)frame * HW + r;
+        if (__ldcg(labels + g) != r + 1) continue;
+        const uint32_t rank = kept_rank(keptbits, blkprefix, g);
+        if ((int64_t)rank >= cap) continue;
+        const Rec a = *c;
+        const int yr = r / W, xr = r - yr * W;
+        bd_source s;
+        s.frame = frame;
+        s.label = r + 1;
+        s.npix = a.npix;
+        s.xmin = a.xmin; s.xmax = a.xmax; s.ymin = a.ymin; s.ymax = a.ymax;
+        const uint32_t pidx = 0xFFFFFFFFu - (uint32_t)(a.peak & 0xFFFFFFFFull);
+        s.ypeak = (int)(pidx / (uint32_t)W);
+        s.xpeak = (int)(pidx - (uint32_t)s.ypeak * (uint32_t)W);
+        s.peak = key_to_f32((uint32_t)(a.peak >> 32));
+        s.flux = a.f;
+        const double mx = a.sx / a.f, my = a.sy / a.f;
+        s.x = (double)xr + mx;
+        s.y = (double)yr + my;
+        s.x2 = a.sxx / a.f - mx * mx;
+        s.y2 = a.syy / a.f - my * my;
+        s.xy = a.sxy / a.f - mx * my;
+        cat[rank] = s;
     }
-}
-
-// ------------------------------------------------------------------------------------------------ K4c / K5
-__device__ __forceinline__ uint32_t root_rank(const uint32_t *rootbits, const uint32_t *rootprefix, size_t g) {
-    return __ldg(rootprefix + (g >> 5)) + __popc(__ldg(rootbits + (g >> 5)) & ((1u << (g & 31)) - 1u));
-}
-
-__global__ void k_zero_area(int32_t *area, const uint32_t *n_roots) {
-    size_t n = *n_roots;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) area[i] = 0;
-}
-
-// flatten to roots + area count; one thread per 4 pixels
-__global__ void __launch_bounds__(256) k4c_flatten_count(int32_t *labels, int H, int W, size_t n4_per_frame,
-                                                         const uint32_t *rootbits, const uint32_t *rootprefix,
-                                                         int32_t *area) {
-    const int frame = blockIdx.y;
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n4_per_frame) return;
-    const size_t fbase = (size_t)frame * H * W;
-    int32_t *L = labels + fbase;
-    int4 v = __ldcg(reinterpret_cast<const int4 *>(L) + i);
-    if (!(v.x | v.y | v.z | v.w)) return;
-    int l[4] = {v.x, v.y, v.z, v.w};
-    bool changed = false;
-    int prev_root = -1;
-    uint32_t prev_id = 0;
-    int run = 0;
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        if (!l[q]) continue;
-        int r = g_find(L, l[q] - 1);
-        if (r + 1 != l[q]) { l[q] = r + 1; changed = true; }
-        if (r == prev_root) { ++run; continue; }
-        if (run) atomicAdd(&area[prev_id], run);
-        prev_root = r;
-        prev_id = root_rank(rootbits, rootprefix, fbase + (size_t)r);
-        run = 1;
-    }
-    if (run) atomicAdd(&area[prev_id], run);
-    if (changed) __stcg(reinterpret_cast<int4 *>(L) + i, make_int4(l[0], l[1], l[2], l[3]));
-}
-
-__global__ void k_init_acc(Acc *acc, const uint32_t *n_kept, int64_t cap) {
-    size_t n = *n_kept;
-    if ((int64_t)n > cap) n = (size_t)cap;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        Acc a;
-        a.f = a.sx = a.sy = a.sxx = a.syy = a.sxy = 0.0;
-        a.peak = 0; a.root = 0;
-        a.xmin = 0x7FFFFFFF; a.ymin = 0x7FFFFFFF; a.xmax = -1; a.ymax = -1;
-        acc[i] = a;
-    }
-}
-
-__global__ void k_frame_counts(const uint32_t *rootbits, const uint32_t *rootprefix, const uint32_t *keptprefix,
-                               int B, size_t HW, int64_t *n_sources) {
-    int f = blockIdx.x * blockDim.x + threadIdx.x;
-    if (f >= B) return;
-    uint32_t r0 = root_rank(rootbits, rootprefix, (size_t)f * HW), r1 = root_rank(rootbits, rootprefix, (size_t)(f + 1) * HW);
-    n_sources[f] = (int64_t)(keptprefix[r1] - keptprefix[r0]);
-}
-
-struct Part {   // a thread's running partial for one slot
-    double f, sx, sy, sxx, syy, sxy;
-    u64 peak;
-    int xmin, xmax, ymin, ymax;
-};
-__device__ __forceinline__ void flush_part(Acc *acc, uint32_t slot, const Part &p) {
-    Acc *a = acc + slot;
-    atomicAdd(&a->f, p.f);
-    atomicAdd(&a->sx, p.sx);
-    atomicAdd(&a->sy, p.sy);
-    atomicAdd(&a->sxx, p.sxx);
-    atomicAdd(&a->syy, p.syy);
-    atomicAdd(&a->sxy, p.sxy);
-    atomicMax(&a->peak, p.peak);
-    atomicMin(&a->xmin, p.xmin);
-    atomicMax(&a->xmax, p.xmax);
-    atomicMin(&a->ymin, p.ymin);
-    atomicMax(&a->ymax, p.ymax);
-}
-
-__global__ void __launch_bounds__(256) k5b_accumulate(const int32_t *labels, const float *sub, int H, int W,
-                                                      size_t n4_per_frame, const uint32_t *rootbits,
-                                                      const uint32_t *rootprefix, const int32_t *area,
-                                                      const uint32_t *keptprefix, int min_area, Acc *acc, int64_t cap) {
-    const int frame = blockIdx.y;
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n4_per_frame) return;
-    const size_t fbase = (size_t)frame * H * W;
-    int4 v = __ldcs(reinterpret_cast<const int4 *>(labels + fbase) + i);
-    if (!(v.x | v.y | v.z | v.w)) return;
-    const int l[4] = {v.x, v.y, v.z, v.w};
-    const float4 sv = __ldcs(reinterpret_cast<const float4 *>(sub + fbase) + i);
-    const float I4[4] = {sv.x, sv.y, sv.z, sv.w};
-    const int p0 = (int)(i * 4);
-    const int y = p0 / W, x0 = p0 - y * W;
-
-    int prev_root = -1;
-    bool have = false;
-    uint32_t slot = 0;
-    int xr = 0, yr = 0;
-    Part part;
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        if (!l[q]) continue;
-        const int r = l[q] - 1;
-        if (r != prev_root) {
-            if (have) flush_part(acc, slot, part);
-            prev_root = r;
-            have = false;
-            uint32_t id = root_rank(rootbits, rootprefix, fbase + (size_t)r);
-            if (__ldg(area + id) >= min_area) {
-                slot = __ldg(keptprefix + id);
-                if ((int64_t)slot < cap) {
-                    have = true;
-                    yr = r / W; xr = r - yr * W;
-                    part.f = part.sx = part.sy = part.sxx = part.syy = part.sxy = 0.0;
-                    part.peak = 0;
-                    part.xmin = 0x7FFFFFFF; part.ymin = 0x7FFFFFFF; part.xmax = -1; part.ymax = -1;
-                }
-            }
-        }
-        if (!have) continue;
-        const int x = x0 + q;
-        if (p0 + q == r) acc[slot].root = (u64)(fbase + (size_t)r);
-        const double I = (double)I4[q], dx = (double)(x - xr), dy = (double)(y - yr);
-        part.f += I;
-        part.sx = fma(I, dx, part.sx);
-        part.sy = fma(I, dy, part.sy);
-        part.sxx = fma(I * dx, dx, part.sxx);
-        part.syy = fma(I * dy, dy, part.syy);
-        part.sxy = fma(I * dx, dy, part.sxy);
-        u64 pk = ((u64)f32_to_key(I4[q]) << 32) | (u64)(0xFFFFFFFFu - (uint32_t)(p0 + q));
-        part.peak = pk > part.peak ? pk : part.peak;
-        part.xmin = min(part.xmin, x); part.xmax = max(part.xmax, x);
-        part.ymin = min(part.ymin, y); part.ymax = max(part.ymax, y);
-    }
-    if (have) flush_part(acc, slot, part);
-}
-
-__global__ void k5c_finalize(const Acc *acc, const uint32_t *n_kept, int64_t cap, const int32_t *area,
-                             const uint32_t *rootbits, const uint32_t *rootprefix, size_t HW, int W, bd_source *cat) {
-    size_t n = *n_kept;
-    if ((int64_t)n > cap) n = (size_t)cap;
-    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    Acc a = acc[i];
-    bd_source s;
-    const size_t g = (size_t)a.root;
-    const int frame = (int)(g / HW);
-    const int r = (int)(g - (size_t)frame * HW);
-    const int yr = r / W, xr = r - yr * W;
-    s.frame = frame;
-    s.label = r + 1;
-    s.npix = area[root_rank(rootbits, rootprefix, g)];
-    s.xmin = a.xmin; s.xmax = a.xmax; s.ymin = a.ymin; s.ymax = a.ymax;
-    const uint32_t pidx = 0xFFFFFFFFu - (uint32_t)(a.peak & 0xFFFFFFFFull);
-    s.ypeak = (int)(pidx / (uint32_t)W);
-    s.xpeak = (int)(pidx - (uint32_t)s.ypeak * (uint32_t)W);
-    s.peak = key_to_f32((uint32_t)(a.peak >> 32));
-    s.flux = a.f;
-    const double mx = a.sx / a.f, my = a.sy / a.f;
-    s.x = (double)xr + mx;
-    s.y = (double)yr + my;
-    s.x2 = a.sxx / a.f - mx * mx;
-    s.y2 = a.syy / a.f - my * my;
-    s.xy = a.sxy / a.f - mx * my;
-    cat[i] = s;
 }
 
 }  // namespace
 
 size_t k45_workspace_bytes(int B, int H, int W, int64_t cat_capacity) {
+    (void)cat_capacity;   // the record table is sized by the frame, not by the catalogue
     Ws w;
-    return carve(w, nullptr, B, H, W, cat_capacity) + 256;
+    return carve(w, nullptr, B, H, W) + 256;
 }
 
 int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_t *d_mask, int B, int H, int W,
@@ -506,11 +682,10 @@ int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_
                int64_t *d_n_sources, void *d_ws, size_t ws_bytes, cudaStream_t st) {
     Ws w;
     char *base = (char *)bd_align_up((size_t)d_ws, 256);
-    size_t need = carve(w, base, B, H, W, cat_capacity);
+    size_t need = carve(w, base, B, H, W);
     if ((size_t)(base - (char *)d_ws) + need > ws_bytes)
         return bd_set_error(ctx, BD_EWORKSPACE, "detect workspace: need %zu bytes, got %zu", need + 256, ws_bytes);
-    const size_t HW = (size_t)H * W, P = w.P;
-    const size_t n4f = HW / 4;
+    const size_t P = w.P;
 
     const uint8_t *mask = d_mask;
     if (!mask) {
@@ -518,54 +693,40 @@ int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_
         k_make_mask<<<(unsigned)((n4 + 255) / 256), 256, 0, st>>>(d_sub, d_rms, n4, detect_k, w.maskbuf);
         mask = w.maskbuf;
     }
-    const int aligned32 = (W % 32 == 0 && HW % 32 == 0) ? 1 : 0;
-    if (aligned32) BD_CUDA_CHECK(ctx, cudaMemsetAsync(w.rootbits + w.NW, 0, sizeof(uint32_t), st));
-    else BD_CUDA_CHECK(ctx, cudaMemsetAsync(w.rootbits, 0, (w.NW + 1) * sizeof(uint32_t), st));
+    BD_CUDA_CHECK(ctx, cudaMemsetAsync(w.counters, 0, 64 * sizeof(uint32_t), st));
+    BD_CUDA_CHECK(ctx, cudaMemsetAsync(w.keptbits, 0, w.zero_bytes, st));
 
-    dim3 tg((W + TW - 1) / TW, (H + TH - 1) / TH, B);
-    k4a_tile_label<<<tg, K4_NT, 0, st>>>(mask, H, W, d_labels, w.rootbits, aligned32);
-    if (tg.y > 1) {
-        dim3 g((W + 255) / 256, tg.y - 1, B);
-        k4b_seam_h<<<g, 256, 0, st>>>(mask, H, W, d_labels, w.rootbits);
+    const int TX = (W + TW - 1) / TW, TY = (H + TH - 1) / TH;
+    K4Args a;
+    a.mask = mask; a.sub = d_sub; a.H = H; a.W = W; a.min_area = min_area;
+    a.vec16 = (W % 16 == 0 && ((uintptr_t)mask & 15) == 0) ? 1 : 0;
+    a.labels = d_labels; a.edges = w.edges; a.rec = w.rec; a.reclist = w.reclist; a.counters = w.counters;
+    a.use_tma = (W >= TW && H >= TH && ctx->encode_tiled) ? 1 : 0;
+    CUtensorMap tmap;
+    memset(&tmap, 0, sizeof(tmap));
+    if (a.use_tma) {
+        cuuint64_t dims[3] = {(cuuint64_t)W, (cuuint64_t)H, (cuuint64_t)B};
+        cuuint64_t strides[2] = {(cuuint64_t)W * sizeof(int32_t), (cuuint64_t)W * H * sizeof(int32_t)};
+        cuuint32_t box[3] = {TW, TH, 1};
+        cuuint32_t estr[3] = {1, 1, 1};
+        CUresult r = ctx->encode_tiled(&tmap, CU_TENSOR_MAP_DATA_TYPE_INT32, 3, (void *)d_labels, dims, strides, box, estr,
+                                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                       CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return bd_set_error(ctx, BD_ECUDA, "cuTensorMapEncodeTiled(labels) failed (%d)", (int)r);
     }
-    if (tg.x > 1) {
-        dim3 g((H + 127) / 128, tg.x - 1, B);
-        k4b_seam_v<<<g, 128, 0, st>>>(mask, H, W, d_labels, w.rootbits);
+    BD_CUDA_CHECK(ctx, cudaFuncSetAttribute(k4a_tile_label, cudaFuncAttributeMaxDynamicSharedMemorySize, K4_SMEM));
+    k4a_tile_label<<<dim3(TX, TY, B), K4_NT, K4_SMEM, st>>>(tmap, a);
+    if (TX > 1 || TY > 1) {
+        const size_t n_units = w.ntiles * 6;
+        k4b_seams<<<(unsigned)((n_units + 255) / 256), 256, 0, st>>>(w.edges, d_labels, H, W, TX, TY, n_units);
     }
-    // rank of every root in raster order
-    {
-        ScanArgs a = {};
-        a.bits = w.rootbits; a.n = w.NW + 1; a.out = w.rootprefix; a.part = w.scanpart; a.total_out = w.counters + 0;
-        size_t nblk = (a.n + SCAN_ELEMS) / SCAN_ELEMS;
-        scan_reduce<0><<<(unsigned)nblk, SCAN_NT, 0, st>>>(a);
-        scan_top<<<1, 1024, 0, st>>>(w.scanpart, nblk, a.total_out);
-        scan_apply<0><<<(unsigned)nblk, SCAN_NT, 0, st>>>(a);
-    }
-    k_zero_area<<<ctx->num_sms * 8, 256, 0, st>>>(w.area, w.counters + 0);
-    {
-        dim3 g((unsigned)((n4f + 255) / 256), B);
-        k4c_flatten_count<<<g, 256, 0, st>>>(d_labels, H, W, n4f, w.rootbits, w.rootprefix, w.area);
-    }
-    // catalogue slot of every kept root
-    {
-        ScanArgs a = {};
-        a.area = w.area; a.n_dev = w.counters + 0; a.min_area = min_area; a.out = w.keptprefix; a.part = w.scanpart;
-        a.total_out = w.counters + 1;
-        size_t nblk = (w.maxroots + SCAN_ELEMS) / SCAN_ELEMS;
-        scan_reduce<1><<<(unsigned)nblk, SCAN_NT, 0, st>>>(a);
-        scan_top<<<1, 1024, 0, st>>>(w.scanpart, nblk, a.total_out);
-        scan_apply<1><<<(unsigned)nblk, SCAN_NT, 0, st>>>(a);
-    }
-    k_frame_counts<<<(B + 127) / 128, 128, 0, st>>>(w.rootbits, w.rootprefix, w.keptprefix, B, HW, d_n_sources);
-    if (cat_capacity > 0 && d_cat) {
-        k_init_acc<<<ctx->num_sms * 4, 256, 0, st>>>(w.acc, w.counters + 1, cat_capacity);
-        dim3 g((unsigned)((n4f + 255) / 256), B);
-        k5b_accumulate<<<g, 256, 0, st>>>(d_labels, d_sub, H, W, n4f, w.rootbits, w.rootprefix, w.area, w.keptprefix,
-                                           min_area, w.acc, cat_capacity);
-        size_t maxrec = (size_t)(cat_capacity < (int64_t)w.maxroots ? cat_capacity : (int64_t)w.maxroots);
-        k5c_finalize<<<(unsigned)((maxrec + 255) / 256), 256, 0, st>>>(w.acc, w.counters + 1, cat_capacity, w.area,
-                                                                       w.rootbits, w.rootprefix, HW, W, d_cat);
-    }
+    const int nb = ctx->num_sms * 8;
+    k5m_merge_relabel<<<nb, 256, 0, st>>>(w.reclist, w.counters, w.rec, d_labels, H, W);
+    k5k_mark_kept<<<nb, 256, 0, st>>>(w.reclist, w.counters, w.rec, d_labels, H, W, min_area, w.keptbits, w.blkcnt);
+    k5s_scan_blocks<<<1, 1024, 0, st>>>(w.blkcnt, w.NB, w.blkprefix, w.counters + 1);
+    const int nbf = nb * 256 >= B ? nb : (B + 255) / 256;
+    k5f_finalize<<<nbf, 256, 0, st>>>(w.reclist, w.counters, w.rec, d_labels, B, H, W, min_area, w.keptbits, w.blkprefix,
+                                      d_cat, cat_capacity, d_n_sources);
     BD_CUDA_CHECK(ctx, cudaGetLastError());
     return BD_OK;
 }
