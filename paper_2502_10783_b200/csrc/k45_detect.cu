@@ -32,18 +32,20 @@ namespace {
 
 typedef unsigned long long u64;
 
-constexpr int TW = 128, TH = 64, K4_NT = 512;
+constexpr int TW = 128, TH = 64, K4_NT = 256;   // one thread per 32-pixel bit word of the tile
 constexpr int TPX = TW * TH;             // 8192 pixels per tile
 constexpr int BROWS = TH + 2;            // bit rows incl. halo rows y0-1 and y0+TH
 constexpr int BWORDS = 6;                // [0] bit 31 = column x0-1, [1..4] the tile, [5] bit 0 = column x0+TW
-constexpr int NS = 64;                   // shared-memory stat slots per batch
 constexpr int EDGE_WORDS = 12;           // per tile: top[4], bottom[4], left[2], right[2]
 
-constexpr uint32_t F_ROOT = 0x80000000u; // root word: F_ROOT | F_REC | F_RING | slot << 14 | count
-constexpr uint32_t F_REC = 0x40000000u;
-constexpr uint32_t F_RING = 0x20000000u;
+// lab[] word of a foreground pixel p (local index, 13 bits):
+//   non-root: index of its parent / (after the flatten) of its root;
+//   root:     p | count << 13 (14 bits) | F_RING, and once the record slot is known p | slot << 13 | F_REC | F_RING
+constexpr uint32_t IDX_MASK = 0x1FFFu;
+constexpr int CNT_SHIFT = 13;
 constexpr uint32_t CNT_MASK = 0x3FFFu;   // count <= 8192
-constexpr int SLOT_SHIFT = 14;           // slot < 2048 (at most one root per 2x2 block)
+constexpr uint32_t F_REC = 0x80000000u;
+constexpr uint32_t F_RING = 0x40000000u;
 
 struct Rec {   // 96 bytes; sums are about the record's own root pixel
     double f, sx, sy, sxx, syy, sxy;
@@ -84,9 +86,9 @@ size_t carve(Ws &w, void *base, int B, int H, int W) {
     w.edges = (uint32_t *)take(w.ntiles * EDGE_WORDS * sizeof(uint32_t));
     w.reclist = (uint32_t *)take(w.nblk2 * sizeof(uint32_t));
     w.keptbits = (uint32_t *)take(w.NWk * sizeof(uint32_t));
-    w.blkcnt = (uint32_t *)take((w.NB + 1) * sizeof(uint32_t));
+    w.blkcnt = (uint32_t *)take((w.NB + 8) * sizeof(uint32_t));
     w.zero_bytes = (size_t)((char *)w.blkcnt - (char *)w.keptbits) + (w.NB + 1) * sizeof(uint32_t);
-    w.blkprefix = (uint32_t *)take((w.NB + 2) * sizeof(uint32_t));
+    w.blkprefix = (uint32_t *)take((w.NB + 8) * sizeof(uint32_t));
     w.rec = (Rec *)take(w.nblk2 * sizeof(Rec));
     w.total = off;
     return off;
@@ -114,22 +116,11 @@ __device__ __forceinline__ uint32_t bytes_to_nibble(uint32_t v) {
 }
 
 // ------------------------------------------------------------------------------------------------ K4a
-// shared-memory union-find on lab[]: a root points to itself, union by minimum index
+// shared-memory union-find on lab[]: a root's low 13 bits point to itself, union by minimum index
 __device__ __forceinline__ uint32_t sm_find(volatile uint32_t *par, uint32_t x) {
-    uint32_t p = par[x];
-    while (p != x) { x = p; p = par[x]; }
+    uint32_t p = par[x] & IDX_MASK;
+    while (p != x) { x = p; p = par[x] & IDX_MASK; }
     return x;
-}
-__device__ __noinline__ void sm_union(uint32_t *par, uint32_t a, uint32_t b) {
-    for (;;) {
-        a = sm_find(par, a);
-        b = sm_find(par, b);
-        if (a == b) return;
-        if (a < b) { uint32_t t = a; a = b; b = t; }
-        uint32_t old = atomicMin(&par[a], b);
-        if (old == a) return;
-        a = old;
-    }
 }
 // bits of columns x-1, x, x+1 of a bit row (bit 0 = x-1); x in [0, TW)
 __device__ __forceinline__ uint32_t get3(const uint32_t *row, int x) {
@@ -151,21 +142,38 @@ struct K4Args {
 constexpr int SM_LAB = 0;
 constexpr int SM_LIST = SM_LAB + TPX * 4;
 constexpr int SM_BITS = SM_LIST + TPX * 2;
-constexpr int SM_STATD = SM_BITS + 1600;              // BROWS * BWORDS * 4 = 1584, padded
-constexpr int SM_PEAK = SM_STATD + 6 * NS * 8;
-constexpr int SM_BOX = SM_PEAK + NS * 8;
-constexpr int SM_MISC = SM_BOX + 4 * NS * 4;
-constexpr int K4_SMEM = SM_MISC + 32 * 4;
+constexpr int SM_MISC = SM_BITS + 1600;               // BROWS * BWORDS * 4 = 1584, padded
+constexpr int K4_SMEM = SM_MISC + 16 * 4;
 
-__global__ void __launch_bounds__(K4_NT) k4a_tile_label(const __grid_constant__ CUtensorMap tmap_lab, K4Args a) {
+// one 32-pixel word of a mask row -> 32 bits (0 outside the frame)
+__device__ __forceinline__ uint32_t load_mask_word(const K4Args &a, size_t fbase, int y, int x) {
+    uint32_t word = 0;
+    if (y >= 0 && y < a.H && x < a.W) {
+        const uint8_t *src = a.mask + fbase + (size_t)y * a.W + x;
+        if (a.vec16) {
+            if (x + 16 <= a.W) {
+                const uint4 v = __ldg(reinterpret_cast<const uint4 *>(src));
+                word = bytes_to_nibble(v.x) | bytes_to_nibble(v.y) << 4 | bytes_to_nibble(v.z) << 8 | bytes_to_nibble(v.w) << 12;
+            }
+            if (x + 32 <= a.W) {
+                const uint4 v = __ldg(reinterpret_cast<const uint4 *>(src + 16));
+                word |= (bytes_to_nibble(v.x) | bytes_to_nibble(v.y) << 4 | bytes_to_nibble(v.z) << 8 | bytes_to_nibble(v.w) << 12) << 16;
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+                if (x + 4 * k < a.W) word |= bytes_to_nibble(__ldg(reinterpret_cast<const uint32_t *>(src + 4 * k))) << (4 * k);
+        }
+    }
+    return word;
+}
+
+__global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant__ CUtensorMap tmap_lab, K4Args a) {
     extern __shared__ __align__(128) unsigned char sm[];
     uint32_t *lab = reinterpret_cast<uint32_t *>(sm + SM_LAB);
     uint16_t *list = reinterpret_cast<uint16_t *>(sm + SM_LIST);
     uint32_t(*bits)[BWORDS] = reinterpret_cast<uint32_t(*)[BWORDS]>(sm + SM_BITS);
-    double(*s_d)[NS] = reinterpret_cast<double(*)[NS]>(sm + SM_STATD);
-    u64 *s_peak = reinterpret_cast<u64 *>(sm + SM_PEAK);
-    int(*s_box)[NS] = reinterpret_cast<int(*)[NS]>(sm + SM_BOX);
-    uint32_t *wsum = reinterpret_cast<uint32_t *>(sm + SM_MISC);   // [16] warp totals, [16] n_rec, [17] g_base
+    uint32_t *wsum = reinterpret_cast<uint32_t *>(sm + SM_MISC);   // [0..7] warp totals, [8] n_rec, [9] g_base
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int frame = blockIdx.z;
@@ -173,40 +181,33 @@ __global__ void __launch_bounds__(K4_NT) k4a_tile_label(const __grid_constant__ 
     const int H = a.H, W = a.W;
     const size_t fbase = (size_t)frame * H * W;
     const size_t tile = ((size_t)frame * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+    const int row_w = tid >> 2, w_w = tid & 3;   // this thread's bit word of the tile
 
-    // ---- A: zero the label tile, mask bytes -> bit rows with halo ----------------------------------------
+    // ---- A: zero the label tile, mask bytes -> bit rows with a 1-pixel halo -------------------------------
 #pragma unroll
     for (int k = 0; k < TPX / 4 / K4_NT; ++k) reinterpret_cast<uint4 *>(lab)[k * K4_NT + tid] = make_uint4(0, 0, 0, 0);
-    if (tid == 0) wsum[16] = 0;
-    if (tid < BROWS * 4) {
-        const int hr = tid >> 2, w = tid & 3;
-        const int y = y0 - 1 + hr, x = x0 + 32 * w;
-        uint32_t word = 0;
-        if (y >= 0 && y < H && x < W) {
-            const uint8_t *src = a.mask + fbase + (size_t)y * W + x;
-            if (a.vec16) {
-                if (x + 16 <= W) {
-                    const uint4 v = __ldg(reinterpret_cast<const uint4 *>(src));
-                    word = bytes_to_nibble(v.x) | bytes_to_nibble(v.y) << 4 | bytes_to_nibble(v.z) << 8 | bytes_to_nibble(v.w) << 12;
-                }
-                if (x + 32 <= W) {
-                    const uint4 v = __ldg(reinterpret_cast<const uint4 *>(src + 16));
-                    word |= (bytes_to_nibble(v.x) | bytes_to_nibble(v.y) << 4 | bytes_to_nibble(v.z) << 8 | bytes_to_nibble(v.w) << 12) << 16;
-                }
-            } else {
-#pragma unroll
-                for (int k = 0; k < 8; ++k)
-                    if (x + 4 * k < W) word |= bytes_to_nibble(__ldg(reinterpret_cast<const uint32_t *>(src + 4 * k))) << (4 * k);
-            }
-        }
-        bits[hr][1 + w] = word;
-    } else if (tid < BROWS * 4 + BROWS * 2) {
-        const int h = tid - BROWS * 4, hr = h >> 1, side = h & 1;
+    if (tid == 0) wsum[8] = 0;
+    const uint32_t M = load_mask_word(a, fbase, y0 + row_w, x0 + 32 * w_w);
+    bits[row_w + 1][1 + w_w] = M;
+    if (tid < 8) {   // halo rows y0-1 and y0+TH
+        const int hr = tid < 4 ? 0 : BROWS - 1;
+        bits[hr][1 + (tid & 3)] = load_mask_word(a, fbase, y0 - 1 + hr, x0 + 32 * (tid & 3));
+    } else if (tid < 8 + BROWS * 2) {   // halo columns x0-1 and x0+TW
+        const int h = tid - 8, hr = h >> 1, side = h & 1;
         const int y = y0 - 1 + hr, x = side ? x0 + TW : x0 - 1;
         uint32_t bit = 0;
         if (y >= 0 && y < H && x >= 0 && x < W) bit = __ldg(a.mask + fbase + (size_t)y * W + x) ? 1u : 0u;
         bits[hr][side ? 5 : 0] = side ? bit : bit << 31;
     }
+
+    // ---- B: compact list of the foreground pixels (raster order); parent = start of the horizontal run ------
+    uint32_t incl = __popc(M);
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    if (lane == 31) wsum[warp] = incl;
     __syncthreads();
 
     // border bit rows / columns for the seam merge
@@ -221,23 +222,6 @@ __global__ void __launch_bounds__(K4_NT) k4a_tile_label(const __grid_constant__ 
             if (lane == 0) { e[8 + warp - 1] = bl; e[10 + warp - 1] = br; }
         }
     }
-
-    // ---- B: compact list of foreground pixels (raster order); parent = start of the horizontal run ----------
-    uint32_t M = 0, prevbit = 0;
-    int row_w = 0, w_w = 0;
-    if (tid < TH * 4) {
-        row_w = tid >> 2; w_w = tid & 3;
-        M = bits[row_w + 1][1 + w_w];
-        prevbit = w_w ? bits[row_w + 1][w_w] >> 31 : 0u;
-    }
-    uint32_t incl = __popc(M);
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += t;
-    }
-    if (lane == 31) wsum[warp] = incl;
-    __syncthreads();
     uint32_t pos = incl - __popc(M);
     int n = 0;
 #pragma unroll
@@ -247,6 +231,7 @@ __global__ void __launch_bounds__(K4_NT) k4a_tile_label(const __grid_constant__ 
         n += (int)t;
     }
     if (M) {
+        const uint32_t prevbit = w_w ? bits[row_w + 1][w_w] >> 31 : 0u;   // left neighbour word of the same tile row
         const uint32_t pbase = (uint32_t)(row_w * TW + w_w * 32);
         uint32_t m = M, cur = 0;
         while (m) {
@@ -263,45 +248,49 @@ __global__ void __launch_bounds__(K4_NT) k4a_tile_label(const __grid_constant__ 
     __syncthreads();
 
     if (n > 0) {
-        // ---- C: vertical / diagonal links inside the tile (pruned: DESIGN.md section 6, K4) ------------------
+        // ---- C: vertical / diagonal links inside the tile.  Rules (w, a, b, c = W, NW, N, NE neighbours):
+        //      b && !w -> N;  !b && a && !w -> NW;  !b && c -> NE.  In-tile bits only (a halo pixel never prunes an
+        //      in-tile link): the tile-local components are then exactly the components of the tile's own mask, so
+        //      two tile-local roots never share a 2x2 block.
+        constexpr uint32_t NONE = 0xFFFFFFFFu;
         for (int e = tid; e < n; e += K4_NT) {
             const uint32_t p = list[e];
             const int r = (int)(p >> 7), x = (int)(p & 127);
             if (r == 0) continue;
             const uint32_t u3 = get3(bits[r], x), m3 = get3(bits[r + 1], x);
-            // in-tile bits only (a halo pixel never prunes an in-tile link): the tile-local components are then
-            // exactly the components of the tile's own mask, so two tile-local roots never share a 2x2 block
             const bool w = (m3 & 1u) && x > 0, na = u3 & 1u, nb = u3 & 2u, nc = u3 & 4u;
-            if (nb) { if (!w) sm_union(lab, p, p - TW); }
+            uint32_t t0 = NONE, t1 = NONE;
+            if (nb) { if (!w) t0 = p - TW; }
             else {
-                if (na && !w && x > 0) sm_union(lab, p, p - TW - 1);
-                if (nc && x < TW - 1) sm_union(lab, p, p - TW + 1);
+                if (na && !w && x > 0) t0 = p - TW - 1;
+                if (nc && x < TW - 1) t1 = p - TW + 1;
+            }
+#pragma unroll 1
+            for (int k = 0; k < 2; ++k) {
+                uint32_t ub = k ? t1 : t0;
+                if (ub == NONE) continue;
+                uint32_t ua = p;
+                for (;;) {
+                    ua = sm_find(lab, ua);
+                    ub = sm_find(lab, ub);
+                    if (ua == ub) break;
+                    if (ua < ub) { const uint32_t t = ua; ua = ub; ub = t; }
+                    const uint32_t old = atomicMin(&lab[ua], ub);
+                    if (old == ua) break;
+                    ua = old;
+                }
             }
         }
         __syncthreads();
-        // ---- D1: flatten ------------------------------------------------------------------------------------
-        for (int e = tid; e < n; e += K4_NT) {
-            const uint32_t p = list[e];
-            const uint32_t r = sm_find(lab, p);
-            if (r != p) lab[p] = r;
-        }
-        __syncthreads();
-        // ---- D2a: roots become counters ---------------------------------------------------------------------
-        for (int e = tid; e < n; e += K4_NT) {
-            const uint32_t p = list[e];
-            if (lab[p] == p) lab[p] = F_ROOT;
-        }
-        __syncthreads();
-        // ---- D2b: pixel counts (one atomic per run of equal roots in the list) and ring flags ----------------
+        // ---- D: flatten; pixel counts (one atomic per run of equal roots in the list); ring flags -------------
         for (int e0 = 0; e0 < n; e0 += K4_NT) {
             const int e = e0 + tid;
-            const bool valid = e < n;
-            uint32_t p = 0, r = 0xFFFF0000u | lane;
+            uint32_t r = 0xFFFF0000u | lane;
             bool ring = false;
-            if (valid) {
-                p = list[e];
-                const uint32_t own = lab[p];
-                r = (own & F_ROOT) ? p : own;
+            if (e < n) {
+                const uint32_t p = list[e];
+                r = sm_find(lab, p);
+                if (r != p) lab[p] = r;
                 const int row = (int)(p >> 7), x = (int)(p & 127);
                 if (row == 0 || row == TH - 1 || x == 0 || x == TW - 1) {
                     const uint32_t u3 = get3(bits[row], x), m3 = get3(bits[row + 1], x), d3 = get3(bits[row + 2], x);
@@ -318,112 +307,101 @@ __global__ void __launch_bounds__(K4_NT) k4a_tile_label(const __grid_constant__ 
             const uint32_t hm = __ballot_sync(0xffffffffu, head);
             const uint32_t rest = lane == 31 ? 0u : hm & ~((2u << lane) - 1u);
             const int tail = rest ? __ffs(rest) - 2 : 31;
-            if (valid && head) atomicAdd(&lab[r], (uint32_t)(tail - lane + 1));
+            if (e < n && head) atomicAdd(&lab[r], (uint32_t)(tail - lane + 1) << CNT_SHIFT);
             if (ring) atomicOr(&lab[r], F_RING);
         }
         __syncthreads();
-        // ---- E: record slots for components that can matter ---------------------------------------------------
+        // ---- E: components that can matter get a (zeroed) record in the direct-mapped table -------------------
         for (int e = tid; e < n; e += K4_NT) {
             const uint32_t p = list[e];
-            const uint32_t own = lab[p];
-            if ((own & F_ROOT) && ((int)(own & CNT_MASK) >= a.min_area || (own & F_RING))) {
-                const uint32_t slot = atomicAdd(&wsum[16], 1u);
-                lab[p] = own | F_REC | (slot << SLOT_SHIFT);
+            const uint32_t wd = lab[p];
+            if ((wd & IDX_MASK) != p) continue;
+            const int cnt = (int)((wd >> CNT_SHIFT) & CNT_MASK);
+            if (cnt >= a.min_area || (wd & F_RING)) {
+                const uint32_t slot = atomicAdd(&wsum[8], 1u);
+                lab[p] = p | (slot << CNT_SHIFT) | F_REC | (wd & F_RING);
+                const int gy = y0 + (int)(p >> 7), gx = x0 + (int)(p & 127);
+                const size_t blk = ((size_t)frame * ((H + 1) / 2) + (gy >> 1)) * (W / 2) + (gx >> 1);
+                uint4 *dst = reinterpret_cast<uint4 *>(a.rec + blk);
+                dst[0] = make_uint4(0, 0, 0, 0); dst[1] = make_uint4(0, 0, 0, 0); dst[2] = make_uint4(0, 0, 0, 0);
+                dst[3] = make_uint4(0, 0, (uint32_t)(gy * W + gx), (uint32_t)frame);           // peak, root, frame
+                dst[4] = make_uint4((uint32_t)cnt, 0x7FFFFFFFu, 0xFFFFFFFFu, 0x7FFFFFFFu);     // npix, xmin, xmax, ymin
+                dst[5] = make_uint4(0xFFFFFFFFu, 0, 0, 0);                                     // ymax, pad
             }
         }
         __syncthreads();
-        const int nrec = (int)wsum[16];
-        if (nrec > 0 && tid == 0) wsum[17] = atomicAdd(a.counters + 0, (uint32_t)nrec);
-        // ---- F: partial sums of the recorded components, NS slots at a time ----------------------------------
-        for (int b0 = 0; b0 < nrec; b0 += NS) {
-            if (tid < NS) {
-#pragma unroll
-                for (int k = 0; k < 6; ++k) s_d[k][tid] = 0.0;
-                s_peak[tid] = 0ull;
-                s_box[0][tid] = 0x7FFFFFFF; s_box[1][tid] = -1; s_box[2][tid] = 0x7FFFFFFF; s_box[3][tid] = -1;
-            }
-            __syncthreads();
+        const int nrec = (int)wsum[8];
+        if (nrec > 0) {
+            if (tid == 0) wsum[9] = atomicAdd(a.counters + 0, (uint32_t)nrec);
+            // ---- F: partial sums of the recorded components.  One segment = the consecutive list entries of one
+            //      (component, row); segmented shuffle reduction, then the head lane adds the run to the record.
             for (int e0 = 0; e0 < n; e0 += K4_NT) {
                 const int e = e0 + tid;
-                uint32_t key = 0xFFFF0000u | lane;
-                int s = 0, x = 0, row = 0;
-                double S0 = 0.0, S1 = 0.0, S2 = 0.0, dy = 0.0;
+                uint32_t key = 0xFFFF0000u | lane, r = 0;
+                int x = 0, row = 0;
+                double S0 = 0.0, S1 = 0.0, S2 = 0.0;
                 u64 pk = 0;
                 bool in = false;
                 if (e < n) {
                     const uint32_t p = list[e];
                     const uint32_t own = lab[p];
-                    const uint32_t r = (own & F_ROOT) ? p : own;
-                    const uint32_t rw = (own & F_ROOT) ? own : lab[r];
-                    s = (int)((rw >> SLOT_SHIFT) & 0x7FFu) - b0;
-                    in = (rw & F_REC) && s >= 0 && s < NS;
+                    const bool isroot = (own & IDX_MASK) == p;
+                    r = isroot ? p : own;
+                    const uint32_t rw = isroot ? own : lab[r];
+                    in = rw & F_REC;
                     if (in) {
                         row = (int)(p >> 7); x = (int)(p & 127);
-                        key = ((uint32_t)(s + b0) << 6) | (uint32_t)row;
+                        key = (r << 6) | (uint32_t)row;
                         const int gidx = (y0 + row) * W + x0 + x;
                         const float I = __ldg(a.sub + fbase + (size_t)gidx);
                         const double dx = (double)(x - (int)(r & 127));
-                        dy = (double)(row - (int)(r >> 7));
                         S0 = (double)I; S1 = S0 * dx; S2 = S1 * dx;
                         pk = ((u64)f32_to_key(I) << 32) | (u64)(0xFFFFFFFFu - (uint32_t)gidx);
                     }
                 }
+                if (!__any_sync(0xffffffffu, in)) continue;
                 const uint32_t prev = __shfl_up_sync(0xffffffffu, key, 1);
                 const bool head = lane == 0 || prev != key;
                 const uint32_t hm = __ballot_sync(0xffffffffu, head);
-                if (hm == 0xffffffffu && !__any_sync(0xffffffffu, in)) continue;   // nothing recorded in this warp
                 const uint32_t rest = lane == 31 ? 0u : hm & ~((2u << lane) - 1u);
                 const int tail = rest ? __ffs(rest) - 2 : 31;
-#pragma unroll
-                for (int d = 1; d < 32; d <<= 1) {
+                const int maxlen = __reduce_max_sync(0xffffffffu, in ? tail - lane : 0);
+                for (int d = 1; d <= maxlen; d <<= 1) {
                     const double o0 = __shfl_down_sync(0xffffffffu, S0, d), o1 = __shfl_down_sync(0xffffffffu, S1, d);
                     const double o2 = __shfl_down_sync(0xffffffffu, S2, d);
                     const u64 opk = __shfl_down_sync(0xffffffffu, pk, d);
                     if (lane + d <= tail) { S0 += o0; S1 += o1; S2 += o2; pk = opk > pk ? opk : pk; }
                 }
                 const int xlast = __shfl_sync(0xffffffffu, x, tail);
-                if (in && head) {   // one flush per (component, row) run
-                    atomicAdd(&s_d[0][s], S0);
-                    atomicAdd(&s_d[1][s], S1);
-                    atomicAdd(&s_d[2][s], dy * S0);
-                    atomicAdd(&s_d[3][s], S2);
-                    atomicAdd(&s_d[4][s], dy * dy * S0);
-                    atomicAdd(&s_d[5][s], dy * S1);
-                    atomicMax(&s_peak[s], pk);
-                    atomicMin(&s_box[0][s], x0 + x); atomicMax(&s_box[1][s], x0 + xlast);
-                    atomicMin(&s_box[2][s], y0 + row); atomicMax(&s_box[3][s], y0 + row);
+                if (in && head) {
+                    const int ry = (int)(r >> 7), gy = y0 + ry, gx = x0 + (int)(r & 127);
+                    Rec *T = a.rec + (((size_t)frame * ((H + 1) / 2) + (gy >> 1)) * (W / 2) + (gx >> 1));
+                    const double dy = (double)(row - ry);
+                    atomicAdd(&T->f, S0);
+                    atomicAdd(&T->sx, S1);
+                    atomicAdd(&T->sy, dy * S0);
+                    atomicAdd(&T->sxx, S2);
+                    atomicAdd(&T->syy, dy * dy * S0);
+                    atomicAdd(&T->sxy, dy * S1);
+                    atomicMax(&T->peak, pk);
+                    atomicMin(&T->xmin, x0 + x); atomicMax(&T->xmax, x0 + xlast);
+                    atomicMin(&T->ymin, y0 + row); atomicMax(&T->ymax, y0 + row);
                 }
             }
-            __syncthreads();
-            const uint32_t gbase = wsum[17];
-            for (int e = tid; e < n; e += K4_NT) {
-                const uint32_t p = list[e];
-                const uint32_t own = lab[p];
-                if (!(own & F_ROOT) || !(own & F_REC)) continue;
-                const int slot = (int)((own >> SLOT_SHIFT) & 0x7FFu), s = slot - b0;
-                if (s < 0 || s >= NS) continue;
-                const int gy = y0 + (int)(p >> 7), gx = x0 + (int)(p & 127);
-                const size_t blk = ((size_t)frame * ((H + 1) / 2) + (gy >> 1)) * (W / 2) + (gx >> 1);
-                Rec rr;
-                rr.f = s_d[0][s]; rr.sx = s_d[1][s]; rr.sy = s_d[2][s]; rr.sxx = s_d[3][s]; rr.syy = s_d[4][s]; rr.sxy = s_d[5][s];
-                rr.peak = s_peak[s];
-                rr.root = gy * W + gx; rr.frame = frame; rr.npix = (int)(own & CNT_MASK);
-                rr.xmin = s_box[0][s]; rr.xmax = s_box[1][s]; rr.ymin = s_box[2][s]; rr.ymax = s_box[3][s];
-                rr.pad[0] = rr.pad[1] = rr.pad[2] = 0;
-                uint4 *dst = reinterpret_cast<uint4 *>(a.rec + blk);
-                const uint4 *srcv = reinterpret_cast<const uint4 *>(&rr);
-#pragma unroll
-                for (int k = 0; k < 6; ++k) dst[k] = srcv[k];
-                a.reclist[gbase + slot] = (uint32_t)blk;
-            }
-            __syncthreads();
         }
-        // ---- G: parents -> labels (1 + raster index of the tile-local root) ------------------------------------
+        __syncthreads();
+        // ---- G: parents -> labels (1 + raster index of the tile-local root); record list -----------------------
+        const uint32_t gbase = wsum[9];
         for (int e = tid; e < n; e += K4_NT) {
             const uint32_t p = list[e];
             const uint32_t own = lab[p];
-            const uint32_t r = (own & F_ROOT) ? p : own;
-            lab[p] = (uint32_t)((y0 + (int)(r >> 7)) * W + x0 + (int)(r & 127) + 1);
+            const bool isroot = (own & IDX_MASK) == p;
+            const uint32_t r = isroot ? p : own;
+            const int gy = y0 + (int)(r >> 7), gx = x0 + (int)(r & 127);
+            lab[p] = (uint32_t)(gy * W + gx + 1);
+            if (isroot && (own & F_REC))
+                a.reclist[gbase + ((own >> CNT_SHIFT) & 0x7FFu)] =
+                    (uint32_t)(((size_t)frame * ((H + 1) / 2) + (gy >> 1)) * (W / 2) + (gx >> 1));
         }
     }
 
@@ -469,14 +447,16 @@ __device__ __forceinline__ void g_union(int32_t *L, int a, int b) {
     }
 }
 
-// One thread per (tile, unit): units 0..3 = the four 32-pixel words of the tile's top row against the bottom
+// One WARP per (tile, unit): units 0..3 = the four 32-pixel words of the tile's top row against the bottom
 // row of the tile above (links N, NW, NE of row-0 pixels); units 4, 5 = the two 32-row words of the tile's left
 // column against the right column of the tile to the left (link W of column-0 pixels, NW of column-0 pixels and
 // NE of the left tile's last column, rows >= 1 of the tile; row 0 belongs to units 0..3).  The conditions are
-// the same pruned rules K4a applies inside a tile, evaluated on the true neighbour bits.
+// the pruned rules of K4a evaluated on the true neighbour bits; every lane computes the three task words, lane l
+// executes the l-th set bit of each (the unions are chains of dependent L2 accesses: one per lane, in parallel).
 __global__ void __launch_bounds__(256) k4b_seams(const uint32_t *edges, int32_t *labels, int H, int W, int TX, int TY,
                                                  size_t n_units) {
-    const size_t u = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t u = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
     if (u >= n_units) return;
     const int unit = (int)(u % 6);
     const size_t tile = u / 6;
@@ -500,11 +480,12 @@ __global__ void __launch_bounds__(256) k4b_seams(const uint32_t *edges, int32_t 
         else if (tx + 1 < TX) rc = (EU + EDGE_WORDS)[4] & 1u;
         else rc = 0;
         const uint32_t na = (Uc << 1) | lc, nb = Uc, nc = (Uc >> 1) | (rc << 31), wb = (M << 1) | ml;
-        uint32_t tN = M & ~wb & nb, tNW = M & ~wb & ~nb & na, tNE = M & ~nb & nc;
+        const uint32_t tN = M & ~wb & nb, tNW = M & ~wb & ~nb & na, tNE = M & ~nb & nc;
         const int pbase = y0 * W + x0 + 32 * k;
-        while (tN) { const int i = __ffs(tN) - 1; tN &= tN - 1; g_union(L, pbase + i, pbase + i - W); }
-        while (tNW) { const int i = __ffs(tNW) - 1; tNW &= tNW - 1; g_union(L, pbase + i, pbase + i - W - 1); }
-        while (tNE) { const int i = __ffs(tNE) - 1; tNE &= tNE - 1; g_union(L, pbase + i, pbase + i - W + 1); }
+        uint32_t i;
+        if ((i = __fns(tN, 0, lane + 1)) != 0xFFFFFFFFu) g_union(L, pbase + (int)i, pbase + (int)i - W);
+        if ((i = __fns(tNW, 0, lane + 1)) != 0xFFFFFFFFu) g_union(L, pbase + (int)i, pbase + (int)i - W - 1);
+        if ((i = __fns(tNE, 0, lane + 1)) != 0xFFFFFFFFu) g_union(L, pbase + (int)i, pbase + (int)i - W + 1);
     } else {
         if (tx == 0) return;
         const int h = unit - 4;
@@ -514,11 +495,12 @@ __global__ void __launch_bounds__(256) k4b_seams(const uint32_t *edges, int32_t 
         const uint32_t cl = h ? EA[10] >> 31 : 0u, cr = h ? E[8] >> 31 : 0u;
         const uint32_t Lup = (Lc << 1) | cl, Rup = (R << 1) | cr;
         const uint32_t rows = h ? 0xFFFFFFFFu : 0xFFFFFFFEu;   // row 0 of the tile: units 0..3
-        uint32_t tW = R & Lc, tNW = R & ~Lc & ~Rup & Lup & rows, tNE = Lc & ~Lup & Rup & rows;
+        const uint32_t tW = R & Lc, tNW = R & ~Lc & ~Rup & Lup & rows, tNE = Lc & ~Lup & Rup & rows;
         const int ybase = y0 + 32 * h;
-        while (tW) { const int i = __ffs(tW) - 1; tW &= tW - 1; const int p = (ybase + i) * W + x0; g_union(L, p, p - 1); }
-        while (tNW) { const int i = __ffs(tNW) - 1; tNW &= tNW - 1; const int p = (ybase + i) * W + x0; g_union(L, p, p - W - 1); }
-        while (tNE) { const int i = __ffs(tNE) - 1; tNE &= tNE - 1; const int q = (ybase + i) * W + x0 - 1; g_union(L, q, q - W + 1); }
+        uint32_t i;
+        if ((i = __fns(tW, 0, lane + 1)) != 0xFFFFFFFFu) { const int p = (ybase + (int)i) * W + x0; g_union(L, p, p - 1); }
+        if ((i = __fns(tNW, 0, lane + 1)) != 0xFFFFFFFFu) { const int p = (ybase + (int)i) * W + x0; g_union(L, p, p - W - 1); }
+        if ((i = __fns(tNE, 0, lane + 1)) != 0xFFFFFFFFu) { const int q = (ybase + (int)i) * W + x0 - 1; g_union(L, q, q - W + 1); }
     }
 }
 
@@ -602,13 +584,31 @@ __global__ void __launch_bounds__(256) k5k_mark_kept(const uint32_t *reclist, co
     }
 }
 
-// K5s: exclusive scan of the block counts (one CTA; thread t owns a contiguous chunk), total -> *total_out
+// K5s: exclusive scan of the block counts (one CTA; thread t owns a contiguous chunk, held in registers when
+// the chunk is <= 32 counts), total -> *total_out.  cnt[] is readable up to the next multiple of 4 past n.
 __global__ void __launch_bounds__(1024) k5s_scan_blocks(const uint32_t *cnt, size_t n, uint32_t *prefix, uint32_t *total_out) {
     __shared__ uint32_t red[32];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const size_t per = (n + 1023) / 1024, i0 = (size_t)tid * per, i1 = i0 + per < n ? i0 + per : n;
+    const size_t per = (((n + 1023) / 1024) + 3) & ~(size_t)3, i0 = (size_t)tid * per, i1 = i0 + per < n ? i0 + per : n;
+    const bool in_regs = per <= 32;
+    uint4 v[8];
     uint32_t local = 0;
-    for (size_t i = i0; i < i1; ++i) local += cnt[i];
+    if (in_regs) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            v[k] = make_uint4(0, 0, 0, 0);
+            const size_t i = i0 + 4 * k;
+            if (4 * k < (int)per && i < n) {
+                v[k] = *reinterpret_cast<const uint4 *>(cnt + i);
+                if (i + 1 >= n) v[k].y = 0;
+                if (i + 2 >= n) v[k].z = 0;
+                if (i + 3 >= n) v[k].w = 0;
+            }
+            local += v[k].x + v[k].y + v[k].z + v[k].w;
+        }
+    } else {
+        for (size_t i = i0; i < i1; ++i) local += cnt[i];
+    }
     uint32_t incl = local;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
@@ -616,16 +616,43 @@ __global__ void __launch_bounds__(1024) k5s_scan_blocks(const uint32_t *cnt, siz
     __syncthreads();
     uint32_t run = incl - local, tot = 0;
     for (int w = 0; w < 32; ++w) { if (w < warp) run += red[w]; tot += red[w]; }
-    for (size_t i = i0; i < i1; ++i) { const uint32_t c = cnt[i]; prefix[i] = run; run += c; }
+    if (in_regs) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const size_t i = i0 + 4 * k;
+            if (4 * k < (int)per && i < n) {
+                uint4 o;
+                o.x = run; run += v[k].x; o.y = run; run += v[k].y; o.z = run; run += v[k].z; o.w = run; run += v[k].w;
+                *reinterpret_cast<uint4 *>(prefix + i) = o;   // prefix[] has room up to the next multiple of 4 past n + 1
+            }
+        }
+    } else {
+        for (size_t i = i0; i < i1; ++i) { const uint32_t c = cnt[i]; prefix[i] = run; run += c; }
+    }
+    __syncthreads();
     if (tid == 0) { prefix[n] = tot; *total_out = tot; }
 }
 
-// number of kept roots with global pixel index < g
+// number of kept roots with global pixel index < g: block prefix + popcount of the block's bitmap words below g
+// (<= 128 words, read as predicated 128-bit loads that are all in flight together)
 __device__ __forceinline__ uint32_t kept_rank(const uint32_t *keptbits, const uint32_t *blkprefix, size_t g) {
-    const size_t w0 = (g >> RB_SHIFT) << (RB_SHIFT - 5), w1 = g >> 5;
-    uint32_t rank = blkprefix[g >> RB_SHIFT];
-    for (size_t w = w0; w < w1; ++w) rank += __popc(__ldg(keptbits + w));
-    return rank + __popc(__ldg(keptbits + w1) & ((1u << (g & 31)) - 1u));
+    const size_t w0 = (g >> RB_SHIFT) << (RB_SHIFT - 5);
+    const int nw = (int)((g >> 5) - w0);                    // full words below g's word
+    const uint32_t pm = (1u << (g & 31)) - 1u;              // partial mask of g's word
+    const uint4 *kb = reinterpret_cast<const uint4 *>(keptbits + w0);
+    uint32_t rank = __ldg(blkprefix + (g >> RB_SHIFT));
+#pragma unroll
+    for (int k = 0; k < 32; ++k) {
+        if (4 * k <= nw) {
+            const uint4 v = __ldg(kb + k);
+            const int b = 4 * k;
+            rank += __popc(v.x & (b < nw ? 0xFFFFFFFFu : pm));
+            rank += __popc(v.y & (b + 1 < nw ? 0xFFFFFFFFu : (b + 1 == nw ? pm : 0u)));
+            rank += __popc(v.z & (b + 2 < nw ? 0xFFFFFFFFu : (b + 2 == nw ? pm : 0u)));
+            rank += __popc(v.w & (b + 3 < nw ? 0xFFFFFFFFu : (b + 3 == nw ? pm : 0u)));
+        }
+    }
+    return rank;
 }
 
 // K5f: catalogue records in ascending (frame, label) order; per-frame counts
@@ -718,9 +745,9 @@ int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_
     k4a_tile_label<<<dim3(TX, TY, B), K4_NT, K4_SMEM, st>>>(tmap, a);
     if (TX > 1 || TY > 1) {
         const size_t n_units = w.ntiles * 6;
-        k4b_seams<<<(unsigned)((n_units + 255) / 256), 256, 0, st>>>(w.edges, d_labels, H, W, TX, TY, n_units);
+        k4b_seams<<<(unsigned)((n_units + 7) / 8), 256, 0, st>>>(w.edges, d_labels, H, W, TX, TY, n_units);
     }
-    const int nb = ctx->num_sms * 8;
+    const int nb = ctx->num_sms * 32;
     k5m_merge_relabel<<<nb, 256, 0, st>>>(w.reclist, w.counters, w.rec, d_labels, H, W);
     k5k_mark_kept<<<nb, 256, 0, st>>>(w.reclist, w.counters, w.rec, d_labels, H, W, min_area, w.keptbits, w.blkcnt);
     k5s_scan_blocks<<<1, 1024, 0, st>>>(w.blkcnt, w.NB, w.blkprefix, w.counters + 1);
