@@ -54,7 +54,8 @@ struct Rec {   // 96 bytes; sums are about the record's own root pixel
     int32_t frame;
     int32_t npix;
     int32_t xmin, xmax, ymin, ymax;
-    int32_t pad[3];
+    int32_t merged;    // set by K5m: this record was added to another root's record
+    int32_t pad[2];
 };
 static_assert(sizeof(Rec) == 96, "Rec must be 96 bytes");
 
@@ -62,11 +63,11 @@ struct Ws {
     uint32_t *counters;     // [0] n_rec, [1] n_kept
     uint8_t *maskbuf;       // [P] (only used when the caller gave no mask)
     uint32_t *edges;        // [ntiles * EDGE_WORDS]
-    uint32_t *reclist;      // [nblk2] 2x2-block ids of the records written by K4a
+    uint32_t *recidx;       // [nblk2] direct-mapped by the 2x2 block of a root: index of its record
     uint32_t *keptbits;     // [NWk] one bit per pixel  |
     uint32_t *blkcnt;       // [NB + 1] per 4096 px     |  zeroed together every call
     uint32_t *blkprefix;    // [NB + 2]
-    Rec *rec;               // [nblk2] direct-mapped by 2x2 block
+    Rec *rec;               // [nblk2] records, compact: 0 .. n_rec-1 (capacity = one per 2x2 block, the worst case)
     size_t P, nblk2, NWk, NB, ntiles;
     size_t zero_bytes;      // bytes from keptbits to the end of blkcnt
     size_t total;
@@ -84,7 +85,7 @@ size_t carve(Ws &w, void *base, int B, int H, int W) {
     w.counters = (uint32_t *)take(64 * sizeof(uint32_t));
     w.maskbuf = (uint8_t *)take(P);
     w.edges = (uint32_t *)take(w.ntiles * EDGE_WORDS * sizeof(uint32_t));
-    w.reclist = (uint32_t *)take(w.nblk2 * sizeof(uint32_t));
+    w.recidx = (uint32_t *)take(w.nblk2 * sizeof(uint32_t));
     w.keptbits = (uint32_t *)take(w.NWk * sizeof(uint32_t));
     w.blkcnt = (uint32_t *)take((w.NB + 8) * sizeof(uint32_t));
     w.zero_bytes = (size_t)((char *)w.blkcnt - (char *)w.keptbits) + (w.NB + 1) * sizeof(uint32_t);
@@ -135,8 +136,9 @@ struct K4Args {
     int32_t *labels;
     uint32_t *edges;
     Rec *rec;
-    uint32_t *reclist;
+    uint32_t *recidx;
     uint32_t *counters;
+    int skip_isolated;   // min_area > 1: pixels without any foreground neighbour never enter the list
 };
 
 constexpr int SM_LAB = 0;
@@ -200,8 +202,29 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
         bits[hr][side ? 5 : 0] = side ? bit : bit << 31;
     }
 
-    // ---- B: compact list of the foreground pixels (raster order); parent = start of the horizontal run ------
-    uint32_t incl = __popc(M);
+    __syncthreads();
+
+    // ---- B: compact list of the foreground pixels that have a foreground neighbour (raster order); parent =
+    //      start of the horizontal run.  A pixel whose 3x3 neighbourhood (halo included) is empty is a complete
+    //      component of one pixel: it gets its label here and, when min_area > 1, takes no further part.
+    uint32_t Mc = M;
+    if (a.skip_isolated && M) {
+        const uint32_t *ru = bits[row_w], *rm = bits[row_w + 1], *rd = bits[row_w + 2];
+        const int j = 1 + w_w;
+        const uint32_t U = ru[j], D = rd[j];
+        const uint32_t nb = U | (U << 1) | (ru[j - 1] >> 31) | (U >> 1) | (ru[j + 1] << 31) |
+                            D | (D << 1) | (rd[j - 1] >> 31) | (D >> 1) | (rd[j + 1] << 31) |
+                            (M << 1) | (rm[j - 1] >> 31) | (M >> 1) | (rm[j + 1] << 31);
+        Mc = M & nb;
+        uint32_t iso = M & ~nb;
+        const int gbase_px = (y0 + row_w) * W + x0 + w_w * 32 + 1;
+        while (iso) {
+            const int i = __ffs(iso) - 1;
+            iso &= iso - 1;
+            lab[row_w * TW + w_w * 32 + i] = (uint32_t)(gbase_px + i);
+        }
+    }
+    uint32_t incl = __popc(Mc);
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
         const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
@@ -222,7 +245,7 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
             if (lane == 0) { e[8 + warp - 1] = bl; e[10 + warp - 1] = br; }
         }
     }
-    uint32_t pos = incl - __popc(M);
+    uint32_t pos = incl - __popc(Mc);
     int n = 0;
 #pragma unroll
     for (int k = 0; k < K4_NT / 32; ++k) {
@@ -230,10 +253,10 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
         if (k < warp) pos += t;
         n += (int)t;
     }
-    if (M) {
+    if (Mc) {
         const uint32_t prevbit = w_w ? bits[row_w + 1][w_w] >> 31 : 0u;   // left neighbour word of the same tile row
         const uint32_t pbase = (uint32_t)(row_w * TW + w_w * 32);
-        uint32_t m = M, cur = 0;
+        uint32_t m = Mc, cur = 0;
         while (m) {
             const int i = __ffs(m) - 1;
             m &= m - 1;
@@ -311,7 +334,7 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
             if (ring) atomicOr(&lab[r], F_RING);
         }
         __syncthreads();
-        // ---- E: components that can matter get a (zeroed) record in the direct-mapped table -------------------
+        // ---- E: components that can matter get a record slot; the tile reserves a contiguous range of records -
         for (int e = tid; e < n; e += K4_NT) {
             const uint32_t p = list[e];
             const uint32_t wd = lab[p];
@@ -320,24 +343,33 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
             if (cnt >= a.min_area || (wd & F_RING)) {
                 const uint32_t slot = atomicAdd(&wsum[8], 1u);
                 lab[p] = p | (slot << CNT_SHIFT) | F_REC | (wd & F_RING);
-                const int gy = y0 + (int)(p >> 7), gx = x0 + (int)(p & 127);
-                const size_t blk = ((size_t)frame * ((H + 1) / 2) + (gy >> 1)) * (W / 2) + (gx >> 1);
-                uint4 *dst = reinterpret_cast<uint4 *>(a.rec + blk);
-                dst[0] = make_uint4(0, 0, 0, 0); dst[1] = make_uint4(0, 0, 0, 0); dst[2] = make_uint4(0, 0, 0, 0);
-                dst[3] = make_uint4(0, 0, (uint32_t)(gy * W + gx), (uint32_t)frame);           // peak, root, frame
-                dst[4] = make_uint4((uint32_t)cnt, 0x7FFFFFFFu, 0xFFFFFFFFu, 0x7FFFFFFFu);     // npix, xmin, xmax, ymin
-                dst[5] = make_uint4(0xFFFFFFFFu, 0, 0, 0);                                     // ymax, pad
             }
         }
         __syncthreads();
         const int nrec = (int)wsum[8];
         if (nrec > 0) {
             if (tid == 0) wsum[9] = atomicAdd(a.counters + 0, (uint32_t)nrec);
+            __syncthreads();
+            const uint32_t gbase = wsum[9];
+            for (int e = tid; e < n; e += K4_NT) {   // zeroed records + the root -> record index
+                const uint32_t p = list[e];
+                const uint32_t wd = lab[p];
+                if ((wd & IDX_MASK) != p || !(wd & F_REC)) continue;
+                const uint32_t slot = (wd >> CNT_SHIFT) & 0x7FFu;
+                const int gy = y0 + (int)(p >> 7), gx = x0 + (int)(p & 127);
+                a.recidx[((size_t)frame * ((H + 1) / 2) + (gy >> 1)) * (W / 2) + (gx >> 1)] = gbase + slot;
+                uint4 *dst = reinterpret_cast<uint4 *>(a.rec + gbase + slot);
+                dst[0] = make_uint4(0, 0, 0, 0); dst[1] = make_uint4(0, 0, 0, 0); dst[2] = make_uint4(0, 0, 0, 0);
+                dst[3] = make_uint4(0, 0, (uint32_t)(gy * W + gx), (uint32_t)frame);                            // peak, root, frame
+                dst[4] = make_uint4(0, 0x7FFFFFFFu, 0xFFFFFFFFu, 0x7FFFFFFFu);    // npix (summed in F), xmin, xmax, ymin
+                dst[5] = make_uint4(0xFFFFFFFFu, 0, 0, 0);                                                      // ymax, merged
+            }
+            __syncthreads();
             // ---- F: partial sums of the recorded components.  One segment = the consecutive list entries of one
             //      (component, row); segmented shuffle reduction, then the head lane adds the run to the record.
             for (int e0 = 0; e0 < n; e0 += K4_NT) {
                 const int e = e0 + tid;
-                uint32_t key = 0xFFFF0000u | lane, r = 0;
+                uint32_t key = 0xFFFF0000u | lane, r = 0, rslot = 0;
                 int x = 0, row = 0;
                 double S0 = 0.0, S1 = 0.0, S2 = 0.0;
                 u64 pk = 0;
@@ -349,6 +381,7 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
                     r = isroot ? p : own;
                     const uint32_t rw = isroot ? own : lab[r];
                     in = rw & F_REC;
+                    rslot = (rw >> CNT_SHIFT) & 0x7FFu;
                     if (in) {
                         row = (int)(p >> 7); x = (int)(p & 127);
                         key = (r << 6) | (uint32_t)row;
@@ -374,8 +407,8 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
                 }
                 const int xlast = __shfl_sync(0xffffffffu, x, tail);
                 if (in && head) {
-                    const int ry = (int)(r >> 7), gy = y0 + ry, gx = x0 + (int)(r & 127);
-                    Rec *T = a.rec + (((size_t)frame * ((H + 1) / 2) + (gy >> 1)) * (W / 2) + (gx >> 1));
+                    const int ry = (int)(r >> 7);
+                    Rec *T = a.rec + gbase + rslot;
                     const double dy = (double)(row - ry);
                     atomicAdd(&T->f, S0);
                     atomicAdd(&T->sx, S1);
@@ -384,24 +417,19 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
                     atomicAdd(&T->syy, dy * dy * S0);
                     atomicAdd(&T->sxy, dy * S1);
                     atomicMax(&T->peak, pk);
+                    atomicAdd(&T->npix, tail - lane + 1);
                     atomicMin(&T->xmin, x0 + x); atomicMax(&T->xmax, x0 + xlast);
                     atomicMin(&T->ymin, y0 + row); atomicMax(&T->ymax, y0 + row);
                 }
             }
         }
         __syncthreads();
-        // ---- G: parents -> labels (1 + raster index of the tile-local root); record list -----------------------
-        const uint32_t gbase = wsum[9];
+        // ---- G: parents -> labels (1 + raster index of the tile-local root) ------------------------------------
         for (int e = tid; e < n; e += K4_NT) {
             const uint32_t p = list[e];
             const uint32_t own = lab[p];
-            const bool isroot = (own & IDX_MASK) == p;
-            const uint32_t r = isroot ? p : own;
-            const int gy = y0 + (int)(r >> 7), gx = x0 + (int)(r & 127);
-            lab[p] = (uint32_t)(gy * W + gx + 1);
-            if (isroot && (own & F_REC))
-                a.reclist[gbase + ((own >> CNT_SHIFT) & 0x7FFu)] =
-                    (uint32_t)(((size_t)frame * ((H + 1) / 2) + (gy >> 1)) * (W / 2) + (gx >> 1));
+            const uint32_t r = (own & IDX_MASK) == p ? p : own;
+            lab[p] = (uint32_t)((y0 + (int)(r >> 7)) * W + x0 + (int)(r & 127) + 1);
         }
     }
 
@@ -452,7 +480,7 @@ __device__ __forceinline__ void g_union(int32_t *L, int a, int b) {
 // column against the right column of the tile to the left (link W of column-0 pixels, NW of column-0 pixels and
 // NE of the left tile's last column, rows >= 1 of the tile; row 0 belongs to units 0..3).  The conditions are
 // the pruned rules of K4a evaluated on the true neighbour bits; every lane computes the three task words, lane l
-// executes the l-th set bit of each (the unions are chains of dependent L2 accesses: one per lane, in parallel).
+// executes bit l of each (the unions are chains of dependent L2 accesses: one per lane, in parallel).
 __global__ void __launch_bounds__(256) k4b_seams(const uint32_t *edges, int32_t *labels, int H, int W, int TX, int TY,
                                                  size_t n_units) {
     const size_t u = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -482,10 +510,10 @@ __global__ void __launch_bounds__(256) k4b_seams(const uint32_t *edges, int32_t 
         const uint32_t na = (Uc << 1) | lc, nb = Uc, nc = (Uc >> 1) | (rc << 31), wb = (M << 1) | ml;
         const uint32_t tN = M & ~wb & nb, tNW = M & ~wb & ~nb & na, tNE = M & ~nb & nc;
         const int pbase = y0 * W + x0 + 32 * k;
-        uint32_t i;
-        if ((i = __fns(tN, 0, lane + 1)) != 0xFFFFFFFFu) g_union(L, pbase + (int)i, pbase + (int)i - W);
-        if ((i = __fns(tNW, 0, lane + 1)) != 0xFFFFFFFFu) g_union(L, pbase + (int)i, pbase + (int)i - W - 1);
-        if ((i = __fns(tNE, 0, lane + 1)) != 0xFFFFFFFFu) g_union(L, pbase + (int)i, pbase + (int)i - W + 1);
+        const int p = pbase + lane;   // lane l owns bit l
+        if ((tN >> lane) & 1u) g_union(L, p, p - W);
+        if ((tNW >> lane) & 1u) g_union(L, p, p - W - 1);
+        if ((tNE >> lane) & 1u) g_union(L, p, p - W + 1);
     } else {
         if (tx == 0) return;
         const int h = unit - 4;
@@ -497,10 +525,10 @@ __global__ void __launch_bounds__(256) k4b_seams(const uint32_t *edges, int32_t 
         const uint32_t rows = h ? 0xFFFFFFFFu : 0xFFFFFFFEu;   // row 0 of the tile: units 0..3
         const uint32_t tW = R & Lc, tNW = R & ~Lc & ~Rup & Lup & rows, tNE = Lc & ~Lup & Rup & rows;
         const int ybase = y0 + 32 * h;
-        uint32_t i;
-        if ((i = __fns(tW, 0, lane + 1)) != 0xFFFFFFFFu) { const int p = (ybase + (int)i) * W + x0; g_union(L, p, p - 1); }
-        if ((i = __fns(tNW, 0, lane + 1)) != 0xFFFFFFFFu) { const int p = (ybase + (int)i) * W + x0; g_union(L, p, p - W - 1); }
-        if ((i = __fns(tNE, 0, lane + 1)) != 0xFFFFFFFFu) { const int q = (ybase + (int)i) * W + x0 - 1; g_union(L, q, q - W + 1); }
+        const int p = (ybase + lane) * W + x0;   // lane l owns row l of the word
+        if ((tW >> lane) & 1u) g_union(L, p, p - 1);
+        if ((tNW >> lane) & 1u) g_union(L, p, p - W - 1);
+        if ((tNE >> lane) & 1u) g_union(L, p - 1, p - 1 - W + 1);
     }
 }
 
@@ -511,54 +539,69 @@ __device__ __forceinline__ size_t blk2_of(int frame, int r, int H, int W) {
 }
 
 // K5m: records whose tile-local root was linked under another root are added to the final root's record and
-// their pixels relabelled.  One thread looks at one record; the warp then serves its changed records together.
-__global__ void __launch_bounds__(256) k5m_merge_relabel(const uint32_t *reclist, const uint32_t *counters, Rec *rec,
+// their pixels relabelled.  One thread per record (records are contiguous: coalesced reads).  A changed record
+// with a small bounding box is served by its own thread; larger boxes are served by the whole warp.
+constexpr int K5M_SOLO_AREA = 48;
+
+__device__ __forceinline__ void k5m_merge_into(const Rec *c, Rec *T, int cr, int cR, int W) {
+    const int yc = cr / W, xc = cr - yc * W, yR = cR / W, xR = cR - yR * W;
+    const double ox = (double)(xc - xR), oy = (double)(yc - yR);
+    const double f = c->f, sx = c->sx, sy = c->sy;
+    atomicAdd(&T->f, f);
+    atomicAdd(&T->sx, sx + f * ox);
+    atomicAdd(&T->sy, sy + f * oy);
+    atomicAdd(&T->sxx, c->sxx + 2.0 * ox * sx + ox * ox * f);
+    atomicAdd(&T->syy, c->syy + 2.0 * oy * sy + oy * oy * f);
+    atomicAdd(&T->sxy, c->sxy + ox * sy + oy * sx + ox * oy * f);
+    atomicMax(&T->peak, c->peak);
+    atomicAdd(&T->npix, c->npix);
+    atomicMin(&T->xmin, c->xmin); atomicMax(&T->xmax, c->xmax);
+    atomicMin(&T->ymin, c->ymin); atomicMax(&T->ymax, c->ymax);
+}
+
+__global__ void __launch_bounds__(256) k5m_merge_relabel(const uint32_t *counters, Rec *rec, const uint32_t *recidx,
                                                          int32_t *labels, int H, int W) {
     const uint32_t n = counters[0];
     const int lane = threadIdx.x & 31;
     const size_t HW = (size_t)H * W;
     for (size_t base = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) & ~(size_t)31; base < n; base += (size_t)gridDim.x * blockDim.x) {
         const size_t i = base + lane;
-        uint32_t blk = 0;
-        int r = 0, R = 0, frame = 0;
+        int r = 0, R = 0, frame = 0, bx = 0, by = 0, bw = 0, bh = 0;
         if (i < n) {
-            blk = reclist[i];
-            r = rec[blk].root; frame = rec[blk].frame;
+            const int4 v = *reinterpret_cast<const int4 *>(&rec[i].peak);       // peak (2 words), root, frame
+            const int4 bb = *reinterpret_cast<const int4 *>(&rec[i].npix);      // npix, xmin, xmax, ymin
+            r = v.z; frame = v.w;
+            bx = bb.y; bw = bb.z - bb.y + 1; by = bb.w; bh = rec[i].ymax - bb.w + 1;
             R = g_find(labels + (size_t)frame * HW, r);
         }
-        uint32_t todo = __ballot_sync(0xffffffffu, R != r);
-        while (todo) {
+        const bool changed = R != r;
+        const bool solo = changed && bw * bh <= K5M_SOLO_AREA;
+        if (changed) {
+            int32_t *L = labels + (size_t)frame * HW;
+            rec[i].merged = 1;
+            k5m_merge_into(rec + i, rec + recidx[blk2_of(frame, R, H, W)], r, R, W);
+            L[r] = R + 1;
+            if (solo) {
+                const int old = r + 1, neu = R + 1;
+                for (int yy = 0; yy < bh; ++yy) {
+                    int32_t *q = L + (size_t)(by + yy) * W + bx;
+                    for (int xx = 0; xx < bw; ++xx)
+                        if (q[xx] == old) q[xx] = neu;
+                }
+            }
+        }
+        uint32_t todo = __ballot_sync(0xffffffffu, changed && !solo);
+        while (todo) {   // large boxes: the warp relabels them together
             const int j = __ffs(todo) - 1;
             todo &= todo - 1;
-            const uint32_t cb = __shfl_sync(0xffffffffu, blk, j);
             const int cr = __shfl_sync(0xffffffffu, r, j), cR = __shfl_sync(0xffffffffu, R, j), cf = __shfl_sync(0xffffffffu, frame, j);
-            const Rec *c = rec + cb;
-            Rec *T = rec + blk2_of(cf, cR, H, W);
+            const int cbx = __shfl_sync(0xffffffffu, bx, j), cby = __shfl_sync(0xffffffffu, by, j);
+            const int cbw = __shfl_sync(0xffffffffu, bw, j), cbh = __shfl_sync(0xffffffffu, bh, j);
             int32_t *L = labels + (size_t)cf * HW;
-            const int yc = cr / W, xc = cr - yc * W, yR = cR / W, xR = cR - yR * W;
-            const double ox = (double)(xc - xR), oy = (double)(yc - yR);
-            const double f = c->f, sx = c->sx, sy = c->sy;
-            switch (lane) {
-                case 0: atomicAdd(&T->f, f); break;
-                case 1: atomicAdd(&T->sx, sx + f * ox); break;
-                case 2: atomicAdd(&T->sy, sy + f * oy); break;
-                case 3: atomicAdd(&T->sxx, c->sxx + 2.0 * ox * sx + ox * ox * f); break;
-                case 4: atomicAdd(&T->syy, c->syy + 2.0 * oy * sy + oy * oy * f); break;
-                case 5: atomicAdd(&T->sxy, c->sxy + ox * sy + oy * sx + ox * oy * f); break;
-                case 6: atomicMax(&T->peak, c->peak); break;
-                case 7: atomicAdd(&T->npix, c->npix); break;
-                case 8: atomicMin(&T->xmin, c->xmin); break;
-                case 9: atomicMax(&T->xmax, c->xmax); break;
-                case 10: atomicMin(&T->ymin, c->ymin); break;
-                case 11: atomicMax(&T->ymax, c->ymax); break;
-                case 12: L[cr] = cR + 1; break;
-                default: break;
-            }
-            const int bx = c->xmin, by = c->ymin, bw = c->xmax - bx + 1, bh = c->ymax - by + 1;
             const int old = cr + 1, neu = cR + 1;
-            for (int k = lane; k < bw * bh; k += 32) {
-                const int yy = by + k / bw, xx = bx + k - (k / bw) * bw;
-                int32_t *q = L + (size_t)yy * W + xx;
+            for (int k = lane; k < cbw * cbh; k += 32) {
+                const int yy = k / cbw, xx = k - yy * cbw;
+                int32_t *q = L + (size_t)(cby + yy) * W + cbx + xx;
                 if (*q == old) *q = neu;
             }
         }
@@ -568,17 +611,14 @@ __global__ void __launch_bounds__(256) k5m_merge_relabel(const uint32_t *reclist
 constexpr int RB_SHIFT = 12;   // ranking blocks of 4096 pixels (128 bitmap words)
 
 // K5k: final roots with npix >= min_area -> bit in the per-pixel bitmap, count in the 4096-pixel block
-__global__ void __launch_bounds__(256) k5k_mark_kept(const uint32_t *reclist, const uint32_t *counters, const Rec *rec,
-                                                     const int32_t *labels, int H, int W, int min_area, uint32_t *keptbits,
-                                                     uint32_t *blkcnt) {
+__global__ void __launch_bounds__(256) k5k_mark_kept(const uint32_t *counters, const Rec *rec, int H, int W, int min_area,
+                                                     uint32_t *keptbits, uint32_t *blkcnt) {
     const uint32_t n = counters[0];
     const size_t HW = (size_t)H * W;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        const Rec *c = rec + reclist[i];
-        const int r = c->root, frame = c->frame;
-        if (c->npix < min_area) continue;
-        const size_t g = (size_t)frame * HW + r;
-        if (__ldcg(labels + g) != r + 1) continue;
+        const Rec *c = rec + i;
+        if (c->merged || c->npix < min_area) continue;
+        const size_t g = (size_t)c->frame * HW + c->root;
         atomicOr(&keptbits[g >> 5], 1u << (g & 31));
         atomicAdd(&blkcnt[g >> RB_SHIFT], 1u);
     }
@@ -656,10 +696,9 @@ __device__ __forceinline__ uint32_t kept_rank(const uint32_t *keptbits, const ui
 }
 
 // K5f: catalogue records in ascending (frame, label) order; per-frame counts
-__global__ void __launch_bounds__(256) k5f_finalize(const uint32_t *reclist, const uint32_t *counters, const Rec *rec,
-                                                    const int32_t *labels, int B, int H, int W, int min_area,
-                                                    const uint32_t *keptbits, const uint32_t *blkprefix, bd_source *cat,
-                                                    int64_t cap, int64_t *n_sources) {
+__global__ void __launch_bounds__(256) k5f_finalize(const uint32_t *counters, const Rec *rec, int B, int H, int W,
+                                                    int min_area, const uint32_t *keptbits, const uint32_t *blkprefix,
+                                                    bd_source *cat, int64_t cap, int64_t *n_sources) {
     const uint32_t n = counters[0];
     const size_t HW = (size_t)H * W;
     const size_t t0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -667,14 +706,12 @@ __global__ void __launch_bounds__(256) k5f_finalize(const uint32_t *reclist, con
         n_sources[t0] = (int64_t)kept_rank(keptbits, blkprefix, (t0 + 1) * HW) - (int64_t)kept_rank(keptbits, blkprefix, t0 * HW);
     if (!cat || cap <= 0) return;
     for (size_t i = t0; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        const Rec *c = rec + reclist[i];
-        const int r = c->root, frame = c->frame;
-        if (c->npix < min_area) continue;
-        const size_t g = (size_t)frame * HW + r;
-        if (__ldcg(labels + g) != r + 1) continue;
-        const uint32_t rank = kept_rank(keptbits, blkprefix, g);
-        if ((int64_t)rank >= cap) continue;
+        const Rec *c = rec + i;
+        if (c->merged || c->npix < min_area) continue;
         const Rec a = *c;
+        const int r = a.root, frame = a.frame;
+        const uint32_t rank = kept_rank(keptbits, blkprefix, (size_t)frame * HW + r);
+        if ((int64_t)rank >= cap) continue;
         const int yr = r / W, xr = r - yr * W;
         bd_source s;
         s.frame = frame;
@@ -727,7 +764,8 @@ int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_
     K4Args a;
     a.mask = mask; a.sub = d_sub; a.H = H; a.W = W; a.min_area = min_area;
     a.vec16 = (W % 16 == 0 && ((uintptr_t)mask & 15) == 0) ? 1 : 0;
-    a.labels = d_labels; a.edges = w.edges; a.rec = w.rec; a.reclist = w.reclist; a.counters = w.counters;
+    a.labels = d_labels; a.edges = w.edges; a.rec = w.rec; a.recidx = w.recidx; a.counters = w.counters;
+    a.skip_isolated = min_area > 1 ? 1 : 0;
     a.use_tma = (W >= TW && H >= TH && ctx->encode_tiled) ? 1 : 0;
     CUtensorMap tmap;
     memset(&tmap, 0, sizeof(tmap));
@@ -748,11 +786,11 @@ int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_
         k4b_seams<<<(unsigned)((n_units + 7) / 8), 256, 0, st>>>(w.edges, d_labels, H, W, TX, TY, n_units);
     }
     const int nb = ctx->num_sms * 32;
-    k5m_merge_relabel<<<nb, 256, 0, st>>>(w.reclist, w.counters, w.rec, d_labels, H, W);
-    k5k_mark_kept<<<nb, 256, 0, st>>>(w.reclist, w.counters, w.rec, d_labels, H, W, min_area, w.keptbits, w.blkcnt);
+    k5m_merge_relabel<<<nb, 256, 0, st>>>(w.counters, w.rec, w.recidx, d_labels, H, W);
+    k5k_mark_kept<<<nb, 256, 0, st>>>(w.counters, w.rec, H, W, min_area, w.keptbits, w.blkcnt);
     k5s_scan_blocks<<<1, 1024, 0, st>>>(w.blkcnt, w.NB, w.blkprefix, w.counters + 1);
     const int nbf = nb * 256 >= B ? nb : (B + 255) / 256;
-    k5f_finalize<<<nbf, 256, 0, st>>>(w.reclist, w.counters, w.rec, d_labels, B, H, W, min_area, w.keptbits, w.blkprefix,
+    k5f_finalize<<<nbf, 256, 0, st>>>(w.counters, w.rec, B, H, W, min_area, w.keptbits, w.blkprefix,
                                       d_cat, cat_capacity, d_n_sources);
     BD_CUDA_CHECK(ctx, cudaGetLastError());
     return BD_OK;
