@@ -46,6 +46,8 @@ struct K1Plan {
     size_t smem_bytes;  // dynamic shared memory per CTA
     int use_tma;
     int tailcap;        // capacity of the tail-pixel list (team total)
+    int stream;         // 1: no slab, one CTA per mesh sweeps global memory (meshes larger than one CTA's slab)
+    size_t slab_bytes;  // shared memory in front of the fixed part: the slab, or room for the sort arrays
 };
 int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan);
 int k1_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg_params *p, double *d_bkg_raw,

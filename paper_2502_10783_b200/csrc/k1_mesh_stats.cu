@@ -29,6 +29,7 @@
 // the key range of [mean - sd, mean + sd] (the median lies within one standard deviation of the mean).
 // It reads the slab from shared memory when C = 1 and the mesh from global memory (L2) otherwise.
 #include <cooperative_groups.h>
+#include <stdlib.h>
 
 #include "common.cuh"
 
@@ -51,6 +52,8 @@ struct K1Args {
     const float *img;
     int B, H, W, mh, mw, ny, nx;
     int slab_rows, use_tma, tailcap, allow_fast;
+    int stream;          // no slab: the sweeps read the mesh from global memory (second sweep: L2)
+    int slab_bytes;      // shared memory reserved in front of Smem (the slab, or room for the sort arrays)
     double k_c;
     int iters, skew_guard;
     double median_factor, mean_factor;
@@ -492,10 +495,10 @@ __device__ __noinline__ void k1_slow_path(const MeshSrc &src, Smem &s, uint8_t *
 
 // ---- the kernel ------------------------------------------------------------------------------------------
 template <int C>
-__global__ void k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a) {
+__global__ void __launch_bounds__(1024) k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float *slab = reinterpret_cast<float *>(smem_raw);   // [slab_rows * mw], 128-B aligned for TMA
-    const size_t slab_bytes = ((size_t)a.slab_rows * a.mw * sizeof(float) + 127) & ~(size_t)127;
+    const size_t slab_bytes = (size_t)a.slab_bytes;
     Smem &s = *reinterpret_cast<Smem *>(smem_raw + slab_bytes);
     unsigned char *area = smem_raw + slab_bytes + ((sizeof(Smem) + 127) & ~(size_t)127);
     uint8_t *hist8 = area;                                  // [K1_NBIN][nt] byte counters
@@ -516,7 +519,8 @@ __global__ void k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a
     const int tid = threadIdx.x, nt = blockDim.x;
 
     // ---- stage the slab ---------------------------------------------------------------------------------
-    const bool tma = a.use_tma && vw == a.mw;
+    const bool stream = C == 1 && a.stream;
+    const bool tma = a.use_tma && vw == a.mw && !stream;
     if (tma && tid == 0) {
         uint32_t bar = smem_u32(&s.mbar);
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
@@ -596,7 +600,7 @@ __global__ void k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a
                 : "r"(bar)
                 : "memory");
         }
-    } else if (C == 1 || fast) {   // plain loader: valid pixels packed row-major
+    } else if (!stream && (C == 1 || fast)) {   // plain loader: valid pixels packed row-major
         for (int i = tid; i < n_c; i += nt) {
             int r = i / vw, c = i - r * vw;
             slab[i] = mesh_ptr[(size_t)(row0 + r) * a.W + c];
@@ -618,6 +622,37 @@ __global__ void k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a
         if (tid < n_tail4) { const float e = slab[(n4 << 2) + tid]; BODY }\
     }
 
+    // The same sweep over global memory (stream mode): thread t owns the 128-bit words t, t + nt, ... of the mesh,
+    // 8 loads in flight.  The assignment of pixels to threads is the same on every sweep.
+    const int f4_row = vw >> 2, n_f4 = vh * f4_row;
+#define K1_SWEEP_G(BODY)                                                                          \
+    {                                                                                             \
+        const int dr_ = nt / f4_row, dc_ = nt - dr_ * f4_row;                                     \
+        for (int i0_ = tid; i0_ < n_f4; i0_ += nt * 8) {                                          \
+            float4 v_[8];                                                                         \
+            int r_ = i0_ / f4_row, c_ = i0_ - r_ * f4_row;                                        \
+            _Pragma("unroll") for (int k_ = 0; k_ < 8; ++k_) {                                    \
+                if (i0_ + k_ * nt < n_f4)                                                         \
+                    v_[k_] = __ldg(reinterpret_cast<const float4 *>(mesh_ptr + (size_t)r_ * a.W) + c_); \
+                r_ += dr_; c_ += dc_;                                                             \
+                if (c_ >= f4_row) { c_ -= f4_row; ++r_; }                                         \
+            }                                                                                     \
+            _Pragma("unroll") for (int k_ = 0; k_ < 8; ++k_) {                                    \
+                if (i0_ + k_ * nt < n_f4) {                                                       \
+                    { const float e = v_[k_].x; BODY }                                            \
+                    { const float e = v_[k_].y; BODY }                                            \
+                    { const float e = v_[k_].z; BODY }                                            \
+                    { const float e = v_[k_].w; BODY }                                            \
+                }                                                                                 \
+            }                                                                                     \
+        }                                                                                         \
+    }
+#define K1_SWEEP_ANY(BODY)                      \
+    {                                           \
+        if (stream) K1_SWEEP_G(BODY)            \
+        else K1_SWEEP(BODY)                     \
+    }
+
     double med = 0, mu = 0, sd = 0;
     int n_final = n_tot;
     bool done_fast = false;
@@ -626,15 +661,14 @@ __global__ void k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a
     if (fast) {
         // ---- sweep 1: core sums, tail count, bracket histogram ---------------------------------------------
         const uint32_t span = kb - ka;
-        int shift = 0;
-        while ((span >> shift) >= (uint32_t)K1_NBIN) ++shift;
+        const int shift = max(0, 26 - __clz(span));   // smallest shift with (span >> shift) < K1_NBIN = 64
         for (int i = tid; i < (K1_NBIN * nt) / 16; i += nt) reinterpret_cast<uint4 *>(hist8)[i] = make_uint4(0, 0, 0, 0);
         __syncthreads();
         double t1 = 0, t2 = 0;
         int c_core = 0, c_tail = 0;
         uint32_t below = 0;
         uint8_t *col = hist8 + tid;
-        K1_SWEEP({
+        K1_SWEEP_ANY({
             const uint32_t k = f32_to_key(e);
             const uint32_t t = k - ka;
             if (t <= span) col[(t >> shift) * nt] += 1;
@@ -701,7 +735,7 @@ __global__ void k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a
             uint32_t packed_tot;
             const uint32_t packed = block_scan_excl(s, mycnt | ((uint32_t)c_tail << 16), packed_tot);
             uint32_t pos_c = packed & 0xFFFFu, pos_t = packed >> 16;   // (the scan's barriers: histogram is dead)
-            K1_SWEEP({
+            K1_SWEEP_ANY({
                 const uint32_t k = f32_to_key(e);
                 if (k - kga <= gspan) s.list[pos_c++] = k;
                 if (!(e >= A_f && e <= B_f)) tail[pos_t++] = e;
@@ -787,6 +821,8 @@ __global__ void k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a
             }
         }
     }
+#undef K1_SWEEP_ANY
+#undef K1_SWEEP_G
 #undef K1_SWEEP
     if constexpr (C > 1) {
         if (!fast) {   // nothing was exchanged yet (or everybody passed #2): the peers have no further part
@@ -797,7 +833,7 @@ __global__ void k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a
     if (!done_fast) {
         if (tid == 0) atomicAdd(&g_k1_slow_meshes, 1ull);
         MeshSrc src;
-        src.slab = (C == 1 && !slab_dirty) ? slab : nullptr;
+        src.slab = (C == 1 && !slab_dirty && !stream) ? slab : nullptr;
         src.n_slab = n_c;
         src.g = mesh_ptr; src.W = a.W; src.vh = vh; src.vw = vw;
         src.vec4 = (vw % 4 == 0) && (a.mw % 4 == 0) && (a.W % 4 == 0);
@@ -827,10 +863,45 @@ static size_t k1_smem_bytes(int slab_rows, int mw, int threads) {
     return bd_align_up((size_t)slab_rows * mw * sizeof(float), 128) + bd_align_up(sizeof(Smem), 128) + area + 128;
 }
 
+// what one thread of a lone CTA sees of the whole mesh when it walks it row by row in global memory (slow path)
+static size_t k1_rowwalk_per_thread(int mesh_h, int mesh_w, int threads) {
+    const int nw = threads / 32;
+    const size_t rows_w = (size_t)(mesh_h + nw - 1) / nw;
+    const size_t per_row = mesh_w % 4 == 0 ? (size_t)((mesh_w + 127) / 128) * 4 : (size_t)(mesh_w + 31) / 32;
+    return rows_w * per_row;
+}
+
 int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan) {
-    // Smallest team whose slab stays <= 64 KiB (several CTAs per SM overlap one team's load with another's
-    // sweeps); if even 8 CTAs cannot do that, allow slabs up to the opt-in shared-memory limit.
     const size_t soft = 64 * 1024;
+    plan->stream = 0;
+    // (1) The mesh fits one CTA's slab (<= 64 KiB): slab mode, one TMA load, every sweep in shared memory.
+    // (2) Larger meshes with mesh_w % 4 == 0: stream mode -- one CTA per mesh, no slab; the two sweeps of the fast
+    //     path read global memory (the second one from L2) with 8 x 128-bit loads in flight per thread.  (The first
+    //     version gave such a mesh to a cluster of 4 CTAs with DSMEM exchanges: 570 us on config 3, two thirds of
+    //     the instructions being per-mesh overhead replicated in every CTA, and rank 0 finishing alone.)
+    // (3) Otherwise: a cluster of 2..8 CTAs, each with a slab of rows (plain loader), slabs up to the opt-in limit.
+    const size_t mesh_bytes = (size_t)mesh_h * mesh_w * sizeof(float);
+    if (mesh_bytes > soft && mesh_w % 4 == 0 && !getenv("BKGDET_K1_NOSTREAM")) {
+        for (int threads = 512; threads <= 1024; threads *= 2) {
+            const size_t n_f4 = (size_t)mesh_h * (mesh_w / 4);
+            size_t per_thread = (n_f4 + threads - 1) / threads * 4;
+            const size_t walk = k1_rowwalk_per_thread(mesh_h, mesh_w, threads);
+            if (walk > per_thread) per_thread = walk;
+            const size_t slab_bytes = bd_align_up(12 * 1024, 128);   // SortArea
+            const size_t smem = slab_bytes + bd_align_up(sizeof(Smem), 128) + (size_t)K1_NBIN * threads + 128;
+            if (per_thread <= 255 && smem <= ctx->smem_optin) {
+                plan->cluster = 1;
+                plan->slab_rows = mesh_h;
+                plan->smem_bytes = smem;
+                plan->slab_bytes = slab_bytes;
+                plan->threads = threads;
+                plan->tailcap = K1_NBIN * threads / 4;
+                plan->use_tma = 0;
+                plan->stream = 1;
+                return BD_OK;
+            }
+        }
+    }
     for (int pass = 0; pass < 2; ++pass) {
         for (int c = 1; c <= K1_MAXC; c *= 2) {
             int rows = (mesh_h + c - 1) / c;
@@ -842,16 +913,13 @@ int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan) {
             // byte counters: what one thread can see of (a) its slab, (b) the whole mesh read from global
             // memory by a lone CTA (slow path of a team), must stay <= 255 per bin
             size_t per_thread = px / threads + 5;
-            {
-                int nw = threads / 32;
-                size_t rows_w = (size_t)(mesh_h + nw - 1) / nw;
-                size_t per_row = mesh_w % 4 == 0 ? (size_t)((mesh_w + 127) / 128) * 4 : (size_t)(mesh_w + 31) / 32;
-                if (rows_w * per_row > per_thread) per_thread = rows_w * per_row;
-            }
+            const size_t walk = k1_rowwalk_per_thread(mesh_h, mesh_w, threads);
+            if (walk > per_thread) per_thread = walk;
             if (ok && smem <= ctx->smem_optin && per_thread <= 255) {
                 plan->cluster = c;
                 plan->slab_rows = rows;
                 plan->smem_bytes = smem;
+                plan->slab_bytes = bd_align_up((size_t)rows * mesh_w * sizeof(float), 128);
                 plan->threads = threads;
                 plan->tailcap = K1_NBIN * threads / 4;
                 plan->use_tma = (mesh_w % 4 == 0 && mesh_w <= 256 && rows <= 256) ? 1 : 0;
@@ -890,6 +958,7 @@ int k1_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg
     a.img = d_img; a.B = B; a.H = H; a.W = W; a.mh = p->mesh_h; a.mw = p->mesh_w;
     a.ny = (H + a.mh - 1) / a.mh; a.nx = (W + a.mw - 1) / a.mw;
     a.slab_rows = plan.slab_rows; a.use_tma = plan.use_tma; a.tailcap = plan.tailcap;
+    a.stream = plan.stream; a.slab_bytes = (int)plan.slab_bytes;
     a.allow_fast = ctx->k1_force_slow ? 0 : 1;
     a.k_c = p->clip_sigma; a.iters = p->clip_iters; a.skew_guard = p->skew_guard;
     a.median_factor = p->median_factor; a.mean_factor = p->mean_factor;
