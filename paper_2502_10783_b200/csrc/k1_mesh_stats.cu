@@ -39,7 +39,7 @@ namespace {
 
 constexpr int K1_NBIN = 64;        // histogram bins per level
 constexpr int K1_T1 = 512;         // slow path: stop refining when the target bin holds <= this many pixels
-constexpr int K1_LISTCAP = 2048;   // candidate window capacity (team total)
+constexpr int K1_LISTCAP = 4096;   // candidate window capacity (team total) with >= 512 threads; 2048 with 256
 constexpr int K1_MAXWARPS = 16;
 constexpr int K1_MAXC = 8;
 constexpr int K1_FAST_MIN_PX = 8192;   // below this the fixed costs of the fast path exceed the sweeps it saves
@@ -228,7 +228,7 @@ __device__ __forceinline__ uint32_t bin_prefix(const BinHit &h, uint32_t b) {
 }
 
 // thread 0: grow a window of bins around b while it holds <= K1_LISTCAP pixels
-__device__ void grow_window(Smem &s, const uint32_t *cnt, int nb, uint32_t b, uint32_t cntb) {
+__device__ void grow_window(Smem &s, const uint32_t *cnt, int nb, uint32_t b, uint32_t cntb, uint32_t cap) {
     int b0 = (int)b, b1 = (int)b;
     uint32_t tot = cntb;
     // later rounds clip mostly positive outliers (sources, hot pixels), which moves the median rank DOWN:
@@ -236,8 +236,8 @@ __device__ void grow_window(Smem &s, const uint32_t *cnt, int nb, uint32_t b, ui
     for (int g = 0; g < K1_NBIN; ++g) {
         bool grew = false;
         for (int rep = 0; rep < 2; ++rep)
-            if (b0 - 1 >= 0 && tot + cnt[b0 - 1] <= (uint32_t)K1_LISTCAP) { --b0; tot += cnt[b0]; grew = true; }
-        if (b1 + 1 < nb && tot + cnt[b1 + 1] <= (uint32_t)K1_LISTCAP) { ++b1; tot += cnt[b1]; grew = true; }
+            if (b0 - 1 >= 0 && tot + cnt[b0 - 1] <= cap) { --b0; tot += cnt[b0]; grew = true; }
+        if (b1 + 1 < nb && tot + cnt[b1 + 1] <= cap) { ++b1; tot += cnt[b1]; grew = true; }
         if (!grew) break;
     }
     s.win_b0 = b0; s.win_b1 = b1;
@@ -247,11 +247,18 @@ __device__ void grow_window(Smem &s, const uint32_t *cnt, int nb, uint32_t b, ui
 // by key, shared-memory atomics on m <= 2048 elements only, then an insertion sort inside the (tiny) bins that
 // hold more than one key.  fcur is scratch [K1_FB].
 constexpr int K1_FB = 1024;
-struct SortArea {
-    uint32_t sorted[K1_LISTCAP];
-    uint32_t fcur[K1_FB];
+struct SortArea {   // carved from a dead region of shared memory: (listcap + K1_FB) words
+    uint32_t *sorted;   // [listcap]
+    uint32_t *fcur;     // [K1_FB]
 };
-__device__ void sort_candidates(Smem &s, const uint32_t *list, uint32_t m, uint32_t kga, uint32_t gspan, SortArea &srt) {
+__device__ __forceinline__ uint32_t k1_listcap() { return blockDim.x >= 512 ? (uint32_t)K1_LISTCAP : 2048u; }
+__device__ __forceinline__ SortArea make_sort_area(void *base) {
+    SortArea a;
+    a.sorted = reinterpret_cast<uint32_t *>(base);
+    a.fcur = a.sorted + k1_listcap();
+    return a;
+}
+__device__ void sort_candidates(Smem &s, const uint32_t *list, uint32_t m, uint32_t kga, uint32_t gspan, const SortArea &srt) {
     const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31;
     int fshift = 0;
     while ((gspan >> fshift) >= (uint32_t)K1_FB) ++fshift;
@@ -324,15 +331,26 @@ __device__ __forceinline__ void for_each_px(const MeshSrc &m, F f) {
         }
         if (tid < n_tail) f(m.slab[(n4 << 2) + tid]);
     } else {
-        const int lane = tid & 31, warp = tid >> 5, nw = nt >> 5;
-        for (int r = warp; r < m.vh; r += nw) {
-            const float *row = m.g + (size_t)r * m.W;
-            if (m.vec4) {
-                for (int c = lane * 4; c < m.vw; c += 128) {
-                    const float4 v = __ldg(reinterpret_cast<const float4 *>(row + c));
-                    f(v.x); f(v.y); f(v.z); f(v.w);
+        if (m.vec4) {   // thread t owns the 128-bit words t, t + nt, ... of the mesh; 4 loads in flight
+            const int f4_row = m.vw >> 2, n_f4 = m.vh * f4_row;
+            const int dr = nt / f4_row, dc = nt - dr * f4_row;
+            for (int i0 = tid; i0 < n_f4; i0 += nt * 4) {
+                float4 v[4];
+                int r = i0 / f4_row, c = i0 - r * f4_row;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    if (i0 + k * nt < n_f4) v[k] = __ldg(reinterpret_cast<const float4 *>(m.g + (size_t)r * m.W) + c);
+                    r += dr; c += dc;
+                    if (c >= f4_row) { c -= f4_row; ++r; }
                 }
-            } else {
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (i0 + k * nt < n_f4) { f(v[k].x); f(v[k].y); f(v[k].z); f(v[k].w); }
+            }
+        } else {
+            const int lane = tid & 31, warp = tid >> 5, nw = nt >> 5;
+            for (int r = warp; r < m.vh; r += nw) {
+                const float *row = m.g + (size_t)r * m.W;
                 for (int c = lane; c < m.vw; c += 32) f(__ldg(row + c));
             }
         }
@@ -344,7 +362,8 @@ __device__ __forceinline__ void for_each_px(const MeshSrc &m, F f) {
 __device__ __noinline__ void k1_slow_path(const MeshSrc &src, Smem &s, uint8_t *hist8, int n_tot, double k_c, int iters,
                                           double &med, double &mu, double &sd, int &n_out) {
     const int tid = threadIdx.x, nt = blockDim.x;
-    SortArea &srt = *reinterpret_cast<SortArea *>(hist8);
+    const SortArea srt = make_sort_area(hist8);
+    const uint32_t listcap = k1_listcap();
     // pivot of the round-0 sums: any pixel of the mesh would do for correctness; take the mean of a few
     double pivot;
     {
@@ -409,7 +428,7 @@ __device__ __noinline__ void k1_slow_path(const MeshSrc &src, Smem &s, uint8_t *
                 __syncthreads();
                 continue;
             }
-            if (tid == 0) grow_window(s, s.tot.cnt, (int)(span >> shift) + 1, h.b, h.cnt);
+            if (tid == 0) grow_window(s, s.tot.cnt, (int)(span >> shift) + 1, h.b, h.cnt, listcap);
             __syncthreads();
             const uint32_t b0 = s.win_b0, b1 = s.win_b1;
             const uint32_t pre0 = bin_prefix(h, b0);
@@ -495,7 +514,13 @@ __device__ __noinline__ void k1_slow_path(const MeshSrc &src, Smem &s, uint8_t *
 
 // ---- the kernel ------------------------------------------------------------------------------------------
 template <int C>
-__global__ void __launch_bounds__(1024) k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a) {
+#ifndef K1_MINB
+#define K1_MINB 2
+#endif
+#ifndef K1_U
+#define K1_U 8
+#endif
+__global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float *slab = reinterpret_cast<float *>(smem_raw);   // [slab_rows * mw], 128-B aligned for TMA
     const size_t slab_bytes = (size_t)a.slab_bytes;
@@ -628,16 +653,16 @@ __global__ void __launch_bounds__(1024) k1_mesh_stats(const __grid_constant__ CU
 #define K1_SWEEP_G(BODY)                                                                          \
     {                                                                                             \
         const int dr_ = nt / f4_row, dc_ = nt - dr_ * f4_row;                                     \
-        for (int i0_ = tid; i0_ < n_f4; i0_ += nt * 8) {                                          \
-            float4 v_[8];                                                                         \
+        for (int i0_ = tid; i0_ < n_f4; i0_ += nt * K1_U) {                                          \
+            float4 v_[K1_U];                                                                         \
             int r_ = i0_ / f4_row, c_ = i0_ - r_ * f4_row;                                        \
-            _Pragma("unroll") for (int k_ = 0; k_ < 8; ++k_) {                                    \
+            _Pragma("unroll") for (int k_ = 0; k_ < K1_U; ++k_) {                                    \
                 if (i0_ + k_ * nt < n_f4)                                                         \
                     v_[k_] = __ldg(reinterpret_cast<const float4 *>(mesh_ptr + (size_t)r_ * a.W) + c_); \
                 r_ += dr_; c_ += dc_;                                                             \
                 if (c_ >= f4_row) { c_ -= f4_row; ++r_; }                                         \
             }                                                                                     \
-            _Pragma("unroll") for (int k_ = 0; k_ < 8; ++k_) {                                    \
+            _Pragma("unroll") for (int k_ = 0; k_ < K1_U; ++k_) {                                    \
                 if (i0_ + k_ * nt < n_f4) {                                                       \
                     { const float e = v_[k_].x; BODY }                                            \
                     { const float e = v_[k_].y; BODY }                                            \
@@ -717,12 +742,12 @@ __global__ void __launch_bounds__(1024) k1_mesh_stats(const __grid_constant__ CU
         if (tid == 0 && rank == 0) {
             if (!(n_tail_tot <= a.tailcap)) atomicAdd(&g_k1_reason[2], 1ull);
             else if (!ok) atomicAdd(&g_k1_reason[3], 1ull);
-            else if (h.cnt > (uint32_t)K1_LISTCAP) atomicAdd(&g_k1_reason[4], 1ull);
+            else if (h.cnt > k1_listcap()) atomicAdd(&g_k1_reason[4], 1ull);
         }
-        ok = ok && h.cnt <= (uint32_t)K1_LISTCAP;
+        ok = ok && h.cnt <= k1_listcap();
         uint32_t m_tot = 0, list_off = 0, kga = 0, gspan = 0;
         if (ok) {
-            if (tid == 0) grow_window(s, s.tot.cnt, (int)(span >> shift) + 1, h.b, h.cnt);
+            if (tid == 0) grow_window(s, s.tot.cnt, (int)(span >> shift) + 1, h.b, h.cnt, k1_listcap());
             __syncthreads();
             const uint32_t b0 = s.win_b0, b1 = s.win_b1;
             list_off = off + bin_prefix(h, b0);
@@ -764,7 +789,7 @@ __global__ void __launch_bounds__(1024) k1_mesh_stats(const __grid_constant__ CU
                 if (rank != 0) return;
             }
             __syncthreads();
-            SortArea &srt = *reinterpret_cast<SortArea *>(slab);   // the slab is dead from here on
+            const SortArea srt = make_sort_area(slab);   // the slab is dead from here on
             slab_dirty = true;
             sort_candidates(s, s.list, m_tot, kga, gspan, srt);
             // ---- clipping rounds on the tail list --------------------------------------------------------
@@ -867,8 +892,8 @@ static size_t k1_smem_bytes(int slab_rows, int mw, int threads) {
 static size_t k1_rowwalk_per_thread(int mesh_h, int mesh_w, int threads) {
     const int nw = threads / 32;
     const size_t rows_w = (size_t)(mesh_h + nw - 1) / nw;
-    const size_t per_row = mesh_w % 4 == 0 ? (size_t)((mesh_w + 127) / 128) * 4 : (size_t)(mesh_w + 31) / 32;
-    return rows_w * per_row;
+    if (mesh_w % 4 == 0) return ((size_t)mesh_h * (mesh_w / 4) + threads - 1) / threads * 4;   // flattened 128-bit words
+    return rows_w * (size_t)((mesh_w + 31) / 32);
 }
 
 int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan) {
@@ -882,20 +907,21 @@ int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan) {
     // (3) Otherwise: a cluster of 2..8 CTAs, each with a slab of rows (plain loader), slabs up to the opt-in limit.
     const size_t mesh_bytes = (size_t)mesh_h * mesh_w * sizeof(float);
     if (mesh_bytes > soft && mesh_w % 4 == 0 && !getenv("BKGDET_K1_NOSTREAM")) {
-        for (int threads = 512; threads <= 1024; threads *= 2) {
+        for (int threads = 512; threads <= 512; threads *= 2) {
             const size_t n_f4 = (size_t)mesh_h * (mesh_w / 4);
             size_t per_thread = (n_f4 + threads - 1) / threads * 4;
             const size_t walk = k1_rowwalk_per_thread(mesh_h, mesh_w, threads);
             if (walk > per_thread) per_thread = walk;
-            const size_t slab_bytes = bd_align_up(12 * 1024, 128);   // SortArea
-            const size_t smem = slab_bytes + bd_align_up(sizeof(Smem), 128) + (size_t)K1_NBIN * threads + 128;
+            const size_t slab_bytes = bd_align_up((K1_LISTCAP + K1_FB) * sizeof(uint32_t), 128);   // sort arrays
+            const size_t area = 64 * 1024;   // byte histograms (32 KiB), then up to 16384 tail pixels
+            const size_t smem = slab_bytes + bd_align_up(sizeof(Smem), 128) + area + 128;
             if (per_thread <= 255 && smem <= ctx->smem_optin) {
                 plan->cluster = 1;
                 plan->slab_rows = mesh_h;
                 plan->smem_bytes = smem;
                 plan->slab_bytes = slab_bytes;
                 plan->threads = threads;
-                plan->tailcap = K1_NBIN * threads / 4;
+                plan->tailcap = (int)(area / sizeof(float));
                 plan->use_tma = 0;
                 plan->stream = 1;
                 return BD_OK;
@@ -933,6 +959,8 @@ int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan) {
 template <int C>
 static cudaError_t k1_launch_c(const CUtensorMap &tmap, const K1Args &a, const K1Plan &plan, int n_mesh, cudaStream_t st) {
     cudaError_t e = cudaFuncSetAttribute(k1_mesh_stats<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)plan.smem_bytes);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k1_mesh_stats<C>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)n_mesh * C);
