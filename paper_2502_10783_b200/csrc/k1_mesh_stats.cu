@@ -107,6 +107,46 @@ struct Team {
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
+// Sweep primitives on precomputed shared-memory addresses, predicated instead of branched (the compiler's version
+// of `if (t <= span) col[(t >> shift) * nt] += 1` re-derived tid, the shared base and blockDim for every pixel and
+// wrapped it in BSSY/BSYNC: ~75 instructions per pixel over the two sweeps).
+// byte counter of bin (t >> shift), column `col_s` (= this thread's), row pitch nt:  if (t <= span) ++counter
+__device__ __forceinline__ void k1_hist_inc(uint32_t col_s, uint32_t t, uint32_t span, int shift, int nt) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .u32 a, v;\n\t"
+        "setp.le.u32 p, %1, %2;\n\t"
+        "shr.u32 a, %1, %3;\n\t"
+        "mad.lo.u32 a, a, %4, %0;\n\t"
+        "@p ld.shared.u8 v, [a];\n\t"
+        "@p add.u32 v, v, 1;\n\t"
+        "@p st.shared.u8 [a], v;\n\t}"
+        ::"r"(col_s), "r"(t), "r"(span), "r"(shift), "r"(nt)
+        : "memory");
+}
+// if (t <= span) { *addr = k; addr += 4; }
+__device__ __forceinline__ void k1_push_u32_if_le(uint32_t &addr, uint32_t t, uint32_t span, uint32_t k) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.le.u32 p, %1, %2;\n\t"
+        "@p st.shared.u32 [%0], %3;\n\t"
+        "@p add.u32 %0, %0, 4;\n\t}"
+        : "+r"(addr)
+        : "r"(t), "r"(span), "r"(k)
+        : "memory");
+}
+// if (!(lo <= e && e <= hi)) { *addr = e; addr += 4; }
+__device__ __forceinline__ void k1_push_f32_if_outside(uint32_t &addr, float e, float lo, float hi) {
+    asm volatile(
+        "{\n\t.reg .pred p, q;\n\t"
+        "setp.ge.f32 p, %1, %2;\n\t"
+        "setp.le.and.f32 q, %1, %3, p;\n\t"
+        "@!q st.shared.f32 [%0], %1;\n\t"
+        "@!q add.u32 %0, %0, 4;\n\t}"
+        : "+r"(addr)
+        : "f"(e), "f"(lo), "f"(hi)
+        : "memory");
+}
+
 // ---- block-wide reductions (result valid in every thread) -------------------------------------------------
 __device__ void block_reduce_stats(Smem &s, double &s1, double &s2, int &n_in, int &n_below) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
@@ -246,22 +286,26 @@ __device__ void grow_window(Smem &s, const uint32_t *cnt, int nb, uint32_t b, ui
 // Counting sort of the candidate keys list[0..m) (all in [kga, kga + gspan]) into sorted[0..m): K1_FB fine bins
 // by key, shared-memory atomics on m <= 2048 elements only, then an insertion sort inside the (tiny) bins that
 // hold more than one key.  fcur is scratch [K1_FB].
-constexpr int K1_FB = 1024;
-struct SortArea {   // carved from a dead region of shared memory: (listcap + K1_FB) words
+#ifndef K1_FB_DIV
+#define K1_FB_DIV 4
+#endif
+// fine bins of the counting sort: listcap / K1_FB_DIV are used (more bins made tie-heavy integer frames 1.8x
+// slower and changed nothing on continuous data: measured on configs 2 and 3)
+struct SortArea {   // carved from a dead region of shared memory: 2 * listcap words
     uint32_t *sorted;   // [listcap]
-    uint32_t *fcur;     // [K1_FB]
+    uint32_t *fcur;     // [listcap]
 };
 __device__ __forceinline__ uint32_t k1_listcap() { return blockDim.x >= 512 ? (uint32_t)K1_LISTCAP : 2048u; }
 __device__ __forceinline__ SortArea make_sort_area(void *base) {
     SortArea a;
     a.sorted = reinterpret_cast<uint32_t *>(base);
-    a.fcur = a.sorted + k1_listcap();
+    a.fcur = a.sorted + k1_listcap();   // [listcap] fine-bin cursors
     return a;
 }
 __device__ void sort_candidates(Smem &s, const uint32_t *list, uint32_t m, uint32_t kga, uint32_t gspan, const SortArea &srt) {
     const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31;
     int fshift = 0;
-    while ((gspan >> fshift) >= (uint32_t)K1_FB) ++fshift;
+    while ((gspan >> fshift) >= k1_listcap() / K1_FB_DIV) ++fshift;
     const int nfb = (int)(gspan >> fshift) + 1;
     for (int i = tid; i < nfb; i += nt) srt.fcur[i] = 0;
     __syncthreads();
@@ -518,7 +562,7 @@ template <int C>
 #define K1_MINB 2
 #endif
 #ifndef K1_U
-#define K1_U 8
+#define K1_U 4
 #endif
 __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_mesh_stats(const __grid_constant__ CUtensorMap tmap, K1Args a) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -693,13 +737,13 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
         int c_core = 0, c_tail = 0;
         uint32_t below = 0;
         uint8_t *col = hist8 + tid;
+        const uint32_t col_s = smem_u32(col);
         K1_SWEEP_ANY({
             const uint32_t k = f32_to_key(e);
-            const uint32_t t = k - ka;
-            if (t <= span) col[(t >> shift) * nt] += 1;
-            else if (k < ka) ++below;
+            k1_hist_inc(col_s, k - ka, span, shift, nt);
+            below += k < ka ? 1u : 0u;
+            const double d = (double)e - pivot;
             if (e >= A_f && e <= B_f) {
-                const double d = (double)e - pivot;
                 t1 += d;
                 t2 = fma(d, d, t2);
                 ++c_core;
@@ -760,10 +804,10 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
             uint32_t packed_tot;
             const uint32_t packed = block_scan_excl(s, mycnt | ((uint32_t)c_tail << 16), packed_tot);
             uint32_t pos_c = packed & 0xFFFFu, pos_t = packed >> 16;   // (the scan's barriers: histogram is dead)
+            uint32_t addr_c = smem_u32(&s.list[pos_c]), addr_t = smem_u32(&tail[pos_t]);
             K1_SWEEP_ANY({
-                const uint32_t k = f32_to_key(e);
-                if (k - kga <= gspan) s.list[pos_c++] = k;
-                if (!(e >= A_f && e <= B_f)) tail[pos_t++] = e;
+                k1_push_u32_if_le(addr_c, f32_to_key(e) - kga, gspan, f32_to_key(e));
+                k1_push_f32_if_outside(addr_t, e, A_f, B_f);
             })
             if (tid == 0) { s.xch.m_cand = packed_tot & 0xFFFFu; s.xch.m_tail = packed_tot >> 16; }
         }
@@ -912,8 +956,8 @@ int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan) {
             size_t per_thread = (n_f4 + threads - 1) / threads * 4;
             const size_t walk = k1_rowwalk_per_thread(mesh_h, mesh_w, threads);
             if (walk > per_thread) per_thread = walk;
-            const size_t slab_bytes = bd_align_up((K1_LISTCAP + K1_FB) * sizeof(uint32_t), 128);   // sort arrays
-            const size_t area = 64 * 1024;   // byte histograms (32 KiB), then up to 16384 tail pixels
+            const size_t slab_bytes = bd_align_up(2 * K1_LISTCAP * sizeof(uint32_t), 128);   // sort arrays
+            const size_t area = 56 * 1024;   // byte histograms (32 KiB), then up to 14336 tail pixels
             const size_t smem = slab_bytes + bd_align_up(sizeof(Smem), 128) + area + 128;
             if (per_thread <= 255 && smem <= ctx->smem_optin) {
                 plan->cluster = 1;
