@@ -129,6 +129,13 @@ __device__ __forceinline__ uint32_t get3(const uint32_t *row, int x) {
     return __funnelshift_r(row[j], row[j + 1], q & 31) & 7u;
 }
 
+#ifdef K4_TIMING
+__device__ unsigned long long g_k4_t[16];
+#define K4_T(i) do { if (tid == 0) { const long long t_ = clock64(); atomicAdd(&g_k4_t[i], (unsigned long long)(t_ - t_prev)); t_prev = t_; } } while (0)
+#else
+#define K4_T(i) do { } while (0)
+#endif
+
 struct K4Args {
     const uint8_t *mask;
     const float *sub;
@@ -144,29 +151,40 @@ struct K4Args {
 constexpr int SM_LAB = 0;
 constexpr int SM_LIST = SM_LAB + TPX * 4;
 constexpr int SM_BITS = SM_LIST + TPX * 2;
-constexpr int SM_MISC = SM_BITS + 1600;               // BROWS * BWORDS * 4 = 1584, padded
+constexpr int SM_ROOTS = SM_BITS + 1600;              // BROWS * BWORDS * 4 = 1584, padded
+constexpr int SM_MISC = SM_ROOTS + (TPX / 4) * 2;     // at most one root per 2x2 block
 constexpr int K4_SMEM = SM_MISC + 16 * 4;
 
-// one 32-pixel word of a mask row -> 32 bits (0 outside the frame)
-__device__ __forceinline__ uint32_t load_mask_word(const K4Args &a, size_t fbase, int y, int x) {
-    uint32_t word = 0;
+// one 32-pixel word of a mask row: the 32 raw bytes (0 outside the frame), loaded first and converted later so
+// that a thread's main and halo loads are in flight together
+struct Raw8 { uint32_t v[8]; };
+__device__ __forceinline__ Raw8 load_mask_raw(const K4Args &a, size_t fbase, int y, int x) {
+    Raw8 r;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) r.v[k] = 0;
     if (y >= 0 && y < a.H && x < a.W) {
         const uint8_t *src = a.mask + fbase + (size_t)y * a.W + x;
         if (a.vec16) {
             if (x + 16 <= a.W) {
                 const uint4 v = __ldg(reinterpret_cast<const uint4 *>(src));
-                word = bytes_to_nibble(v.x) | bytes_to_nibble(v.y) << 4 | bytes_to_nibble(v.z) << 8 | bytes_to_nibble(v.w) << 12;
+                r.v[0] = v.x; r.v[1] = v.y; r.v[2] = v.z; r.v[3] = v.w;
             }
             if (x + 32 <= a.W) {
                 const uint4 v = __ldg(reinterpret_cast<const uint4 *>(src + 16));
-                word |= (bytes_to_nibble(v.x) | bytes_to_nibble(v.y) << 4 | bytes_to_nibble(v.z) << 8 | bytes_to_nibble(v.w) << 12) << 16;
+                r.v[4] = v.x; r.v[5] = v.y; r.v[6] = v.z; r.v[7] = v.w;
             }
         } else {
 #pragma unroll
             for (int k = 0; k < 8; ++k)
-                if (x + 4 * k < a.W) word |= bytes_to_nibble(__ldg(reinterpret_cast<const uint32_t *>(src + 4 * k))) << (4 * k);
+                if (x + 4 * k < a.W) r.v[k] = __ldg(reinterpret_cast<const uint32_t *>(src + 4 * k));
         }
     }
+    return r;
+}
+__device__ __forceinline__ uint32_t raw_to_word(const Raw8 &r) {
+    uint32_t word = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) word |= bytes_to_nibble(r.v[k]) << (4 * k);
     return word;
 }
 
@@ -175,7 +193,8 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
     uint32_t *lab = reinterpret_cast<uint32_t *>(sm + SM_LAB);
     uint16_t *list = reinterpret_cast<uint16_t *>(sm + SM_LIST);
     uint32_t(*bits)[BWORDS] = reinterpret_cast<uint32_t(*)[BWORDS]>(sm + SM_BITS);
-    uint32_t *wsum = reinterpret_cast<uint32_t *>(sm + SM_MISC);   // [0..7] warp totals, [8] n_rec, [9] g_base
+    uint16_t *roots = reinterpret_cast<uint16_t *>(sm + SM_ROOTS);   // the tile-local roots (filled in D)
+    uint32_t *wsum = reinterpret_cast<uint32_t *>(sm + SM_MISC);   // [0..7] warp totals, [8] n_rec, [9] g_base, [10] n_roots
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int frame = blockIdx.z;
@@ -184,25 +203,31 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
     const size_t fbase = (size_t)frame * H * W;
     const size_t tile = ((size_t)frame * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
     const int row_w = tid >> 2, w_w = tid & 3;   // this thread's bit word of the tile
+#ifdef K4_TIMING
+    long long t_prev = clock64();
+#endif
 
     // ---- A: zero the label tile, mask bytes -> bit rows with a 1-pixel halo -------------------------------
 #pragma unroll
     for (int k = 0; k < TPX / 4 / K4_NT; ++k) reinterpret_cast<uint4 *>(lab)[k * K4_NT + tid] = make_uint4(0, 0, 0, 0);
-    if (tid == 0) wsum[8] = 0;
-    const uint32_t M = load_mask_word(a, fbase, y0 + row_w, x0 + 32 * w_w);
-    bits[row_w + 1][1 + w_w] = M;
-    if (tid < 8) {   // halo rows y0-1 and y0+TH
-        const int hr = tid < 4 ? 0 : BROWS - 1;
-        bits[hr][1 + (tid & 3)] = load_mask_word(a, fbase, y0 - 1 + hr, x0 + 32 * (tid & 3));
-    } else if (tid < 8 + BROWS * 2) {   // halo columns x0-1 and x0+TW
-        const int h = tid - 8, hr = h >> 1, side = h & 1;
-        const int y = y0 - 1 + hr, x = side ? x0 + TW : x0 - 1;
-        uint32_t bit = 0;
-        if (y >= 0 && y < H && x >= 0 && x < W) bit = __ldg(a.mask + fbase + (size_t)y * W + x) ? 1u : 0u;
-        bits[hr][side ? 5 : 0] = side ? bit : bit << 31;
+    if (tid == 0) { wsum[8] = 0; wsum[10] = 0; }
+    const Raw8 raw_m = load_mask_raw(a, fbase, y0 + row_w, x0 + 32 * w_w);
+    Raw8 raw_h;
+    uint32_t hbit = 0;
+    const int hcol = tid - 8;   // halo column element (if 0 <= hcol < 2 * BROWS)
+    if (tid < 8) {              // halo rows y0-1 and y0+TH
+        raw_h = load_mask_raw(a, fbase, y0 - 1 + (tid < 4 ? 0 : BROWS - 1), x0 + 32 * (tid & 3));
+    } else if (hcol < BROWS * 2) {   // halo columns x0-1 and x0+TW
+        const int y = y0 - 1 + (hcol >> 1), x = (hcol & 1) ? x0 + TW : x0 - 1;
+        if (y >= 0 && y < H && x >= 0 && x < W) hbit = __ldg(a.mask + fbase + (size_t)y * W + x) ? 1u : 0u;
     }
+    const uint32_t M = raw_to_word(raw_m);
+    bits[row_w + 1][1 + w_w] = M;
+    if (tid < 8) bits[tid < 4 ? 0 : BROWS - 1][1 + (tid & 3)] = raw_to_word(raw_h);
+    else if (hcol < BROWS * 2) bits[hcol >> 1][(hcol & 1) ? 5 : 0] = (hcol & 1) ? hbit : hbit << 31;
 
     __syncthreads();
+    K4_T(0);
 
     // ---- B: compact list of the foreground pixels that have a foreground neighbour (raster order); parent =
     //      start of the horizontal run.  A pixel whose 3x3 neighbourhood (halo included) is empty is a complete
@@ -232,6 +257,7 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
     }
     if (lane == 31) wsum[warp] = incl;
     __syncthreads();
+    K4_T(1);
 
     // border bit rows / columns for the seam merge
     {
@@ -269,8 +295,15 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
         }
     }
     __syncthreads();
+    K4_T(2);
 
     if (n > 0) {
+        // sub of this thread's first list entry: requested now, used in F (hides the DRAM latency behind C..E)
+        float I_pre = 0.f;
+        if (tid < n) {
+            const uint32_t p = list[tid];
+            I_pre = __ldg(a.sub + fbase + (size_t)(y0 + (int)(p >> 7)) * W + x0 + (int)(p & 127));
+        }
         // ---- C: vertical / diagonal links inside the tile.  Rules (w, a, b, c = W, NW, N, NE neighbours):
         //      b && !w -> N;  !b && a && !w -> NW;  !b && c -> NE.  In-tile bits only (a halo pixel never prunes an
         //      in-tile link): the tile-local components are then exactly the components of the tile's own mask, so
@@ -305,15 +338,18 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
             }
         }
         __syncthreads();
+        K4_T(3);
         // ---- D: flatten; pixel counts (one atomic per run of equal roots in the list); ring flags -------------
         for (int e0 = 0; e0 < n; e0 += K4_NT) {
             const int e = e0 + tid;
             uint32_t r = 0xFFFF0000u | lane;
-            bool ring = false;
+            bool ring = false, isroot = false;
+            uint32_t p = 0;
             if (e < n) {
-                const uint32_t p = list[e];
+                p = list[e];
                 r = sm_find(lab, p);
                 if (r != p) lab[p] = r;
+                isroot = r == p;
                 const int row = (int)(p >> 7), x = (int)(p & 127);
                 if (row == 0 || row == TH - 1 || x == 0 || x == TW - 1) {
                     const uint32_t u3 = get3(bits[row], x), m3 = get3(bits[row + 1], x), d3 = get3(bits[row + 2], x);
@@ -332,13 +368,21 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
             const int tail = rest ? __ffs(rest) - 2 : 31;
             if (e < n && head) atomicAdd(&lab[r], (uint32_t)(tail - lane + 1) << CNT_SHIFT);
             if (ring) atomicOr(&lab[r], F_RING);
+            const uint32_t rb = __ballot_sync(0xffffffffu, isroot);
+            if (rb) {   // the warp's roots go to the root list with one shared atomic
+                uint32_t base = 0;
+                if (lane == __ffs(rb) - 1) base = atomicAdd(&wsum[10], (uint32_t)__popc(rb));
+                base = __shfl_sync(0xffffffffu, base, __ffs(rb) - 1);
+                if (isroot) roots[base + __popc(rb & ((1u << lane) - 1u))] = (uint16_t)p;
+            }
         }
         __syncthreads();
+        K4_T(4);
+        const int nroots = (int)wsum[10];
         // ---- E: components that can matter get a record slot; the tile reserves a contiguous range of records -
-        for (int e = tid; e < n; e += K4_NT) {
-            const uint32_t p = list[e];
+        for (int e = tid; e < nroots; e += K4_NT) {
+            const uint32_t p = roots[e];
             const uint32_t wd = lab[p];
-            if ((wd & IDX_MASK) != p) continue;
             const int cnt = (int)((wd >> CNT_SHIFT) & CNT_MASK);
             if (cnt >= a.min_area || (wd & F_RING)) {
                 const uint32_t slot = atomicAdd(&wsum[8], 1u);
@@ -346,15 +390,17 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
             }
         }
         __syncthreads();
+        K4_T(5);
         const int nrec = (int)wsum[8];
         if (nrec > 0) {
             if (tid == 0) wsum[9] = atomicAdd(a.counters + 0, (uint32_t)nrec);
             __syncthreads();
+            K4_T(6);
             const uint32_t gbase = wsum[9];
-            for (int e = tid; e < n; e += K4_NT) {   // zeroed records + the root -> record index
-                const uint32_t p = list[e];
+            for (int e = tid; e < nroots; e += K4_NT) {   // zeroed records + the root -> record index
+                const uint32_t p = roots[e];
                 const uint32_t wd = lab[p];
-                if ((wd & IDX_MASK) != p || !(wd & F_REC)) continue;
+                if (!(wd & F_REC)) continue;
                 const uint32_t slot = (wd >> CNT_SHIFT) & 0x7FFu;
                 const int gy = y0 + (int)(p >> 7), gx = x0 + (int)(p & 127);
                 a.recidx[((size_t)frame * ((H + 1) / 2) + (gy >> 1)) * (W / 2) + (gx >> 1)] = gbase + slot;
@@ -365,6 +411,7 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
                 dst[5] = make_uint4(0xFFFFFFFFu, 0, 0, 0);                                                      // ymax, merged
             }
             __syncthreads();
+            K4_T(7);
             // ---- F: partial sums of the recorded components.  One segment = the consecutive list entries of one
             //      (component, row); segmented shuffle reduction, then the head lane adds the run to the record.
             for (int e0 = 0; e0 < n; e0 += K4_NT) {
@@ -386,7 +433,7 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
                         row = (int)(p >> 7); x = (int)(p & 127);
                         key = (r << 6) | (uint32_t)row;
                         const int gidx = (y0 + row) * W + x0 + x;
-                        const float I = __ldg(a.sub + fbase + (size_t)gidx);
+                        const float I = e0 == 0 ? I_pre : __ldg(a.sub + fbase + (size_t)gidx);
                         const double dx = (double)(x - (int)(r & 127));
                         S0 = (double)I; S1 = S0 * dx; S2 = S1 * dx;
                         pk = ((u64)f32_to_key(I) << 32) | (u64)(0xFFFFFFFFu - (uint32_t)gidx);
@@ -424,6 +471,7 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
             }
         }
         __syncthreads();
+        K4_T(8);
         // ---- G: parents -> labels (1 + raster index of the tile-local root) ------------------------------------
         for (int e = tid; e < n; e += K4_NT) {
             const uint32_t p = list[e];
@@ -437,12 +485,14 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
     if (a.use_tma) {
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();
+        K4_T(9);
         if (tid == 0) {
             asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(&tmap_lab),
                          "r"(x0), "r"(y0), "r"(frame), "r"(smem_u32(lab))
                          : "memory");
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
             asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+            K4_T(10);
         }
     } else {
         __syncthreads();
@@ -464,6 +514,10 @@ __device__ __forceinline__ int g_find(const int32_t *L, int a) {
     }
 }
 __device__ __forceinline__ void g_union(int32_t *L, int a, int b) {
+    {   // first hop of both walks together (two independent misses instead of two in a row)
+        const int pa = __ldcg(L + a) - 1, pb = __ldcg(L + b) - 1;
+        a = pa; b = pb;
+    }
     for (;;) {
         a = g_find(L, a);
         b = g_find(L, b);
@@ -581,12 +635,20 @@ __global__ void __launch_bounds__(256) k5m_merge_relabel(const uint32_t *counter
             rec[i].merged = 1;
             k5m_merge_into(rec + i, rec + recidx[blk2_of(frame, R, H, W)], r, R, W);
             L[r] = R + 1;
-            if (solo) {
-                const int old = r + 1, neu = R + 1;
-                for (int yy = 0; yy < bh; ++yy) {
-                    int32_t *q = L + (size_t)(by + yy) * W + bx;
-                    for (int xx = 0; xx < bw; ++xx)
-                        if (q[xx] == old) q[xx] = neu;
+            if (solo) {   // 8 loads in flight, then the stores (a load-compare-store loop waits for every load)
+                const int old = r + 1, neu = R + 1, area = bw * bh;
+                for (int k0 = 0; k0 < area; k0 += 8) {
+                    int32_t *q[8];
+                    int v[8];
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) {
+                        const int kk = min(k0 + k, area - 1), yy = kk / bw;
+                        q[k] = L + (size_t)(by + yy) * W + bx + (kk - yy * bw);
+                        v[k] = __ldcg(q[k]);
+                    }
+#pragma unroll
+                    for (int k = 0; k < 8; ++k)
+                        if (v[k] == old) *q[k] = neu;
                 }
             }
         }
@@ -795,3 +857,12 @@ int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_
     BD_CUDA_CHECK(ctx, cudaGetLastError());
     return BD_OK;
 }
+
+#ifdef K4_TIMING
+extern "C" int bd_debug_k4_timing(unsigned long long *out16, int reset) {
+    unsigned long long z[16] = {0};
+    if (cudaMemcpyFromSymbol(out16, g_k4_t, sizeof(z)) != cudaSuccess) return BD_ECUDA;
+    if (reset && cudaMemcpyToSymbol(g_k4_t, z, sizeof(z)) != cudaSuccess) return BD_ECUDA;
+    return BD_OK;
+}
+#endif
