@@ -32,8 +32,12 @@ from synth import CONFIGS, make_frames  # noqa: E402
 
 METRIC = "Mpix/s background+detection per frame"
 K3_BYTES_PER_PX = 17.0          # img 4 read; sub 4 + bkg 4 + rms 4 + mask 1 written
+TILE_BYTES_PER_PX = 22.0        # fused tile kernel = pass a3 (17) + pass a4 (mask 1 read, labels 4 written)
 CHAIN_BYTES_PER_PX = 30.0       # K1 4 + K3 17 + K4 5 + K5 4
-LAUNCHES_PER_STEP = 10          # K1, K2a, K2b, K3, then detect_sources: k4a, k4b, k5m, k5k, k5s, k5f (+2 memsets, not counted)
+LAUNCHES_PER_STEP = 9           # K1, K2a, K2b, then bkg_subtract_detect: k4a (fused), k4b, k5m, k5k, k5s, k5f (+2 memsets, not counted)
+LAUNCHES_PER_STEP_UNFUSED = 10  # ... K3, then detect_sources: k4a, k4b, k5m, k5k, k5s, k5f
+TILE_TRAFFIC_NCU = None         # dram__bytes_read.sum + dram__bytes_write.sum of the fused tile kernel on config 3 (profiles/)
+K3_TRAFFIC_NCU = None           # same for k3_interp_subtract
 FALLBACK_HBM_GBS = 6650.0       # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 
 
@@ -108,6 +112,7 @@ def main():
     ap.add_argument("--warmup-ref", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--unfused", action="store_true", help="time bkg_subtract + detect_sources instead of bkg_subtract_detect")
     ap.add_argument("--cat-capacity", type=int, default=1 << 20)
     args = ap.parse_args()
     cfg = CONFIGS[args.config]
@@ -161,7 +166,11 @@ def main():
               cat=torch.empty(cap * bd.SOURCE_DTYPE.itemsize, dtype=torch.uint8, device=dev),
               n_sources=torch.empty(B, dtype=torch.int64, device=dev))
 
-    def step(ev=None):
+    ev_tile = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    for e in ev_tile:
+        e.record()          # creates the handles
+
+    def step_unfused(ev=None):
         if ev: ev[0].record()
         bm, rm, cb, cr = bd.bkg_estimate(ctx, img, p, ws=ws_b)
         if ev: ev[1].record()
@@ -169,6 +178,17 @@ def main():
         if ev: ev[2].record()
         bd.detect_sources(ctx, o3["sub"], o3["rms"], o3["mask"], cfg.detect_k, cfg.min_area, cap, ws=ws_d, out=o5)
         if ev: ev[3].record()
+
+    def step_fused(ev=None):
+        if ev: ev[0].record()
+        bm, rm, cb, cr = bd.bkg_estimate(ctx, img, p, ws=ws_b)
+        if ev: ev[1].record()
+        o35 = dict(o3); o35.update(o5)
+        bd.bkg_subtract_detect(ctx, img, p.mesh_h, p.mesh_w, cb, cr, cfg.detect_k, cfg.min_area, cap, ws=ws_d, out=o35)
+        if ev: ev[2].record()
+        if ev: ev[3].record()
+
+    step = step_unfused if args.unfused else step_fused
 
     def barrier():
         if dist: dist.barrier()
@@ -189,6 +209,21 @@ def main():
     sampler.stop_flag = True
     total_ms = t_start.elapsed_time(t_end)
     stage_ms = [float(np.mean([e[i].elapsed_time(e[i + 1]) for e in evs])) for i in range(3)]
+    # outside the timed region: (i) the tile kernel alone (events recorded by the library around its launch),
+    # (ii) the three calls one by one (bkg_subtract = the K3 pass alone, for the 17 B/px figure)
+    tile_ms = []
+    bd.tile_kernel_events(ctx, ev_tile[0], ev_tile[1])
+    for _ in range(5):
+        step(); torch.cuda.synchronize()
+        tile_ms.append(ev_tile[0].elapsed_time(ev_tile[1]))
+    bd.tile_kernel_events(ctx, None, None)
+    tile_ms = float(np.mean(tile_ms))
+    ev_u = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(5)]
+    step_unfused(); torch.cuda.synchronize()
+    for k in range(5):
+        step_unfused(ev_u[k])
+    torch.cuda.synchronize()
+    unfused_ms = [float(np.mean([e[i].elapsed_time(e[i + 1]) for e in ev_u])) for i in range(3)]
     n_src = int(o5["n_sources"].sum().item())
     if dist:
         t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
@@ -224,22 +259,31 @@ def main():
         if dist: dist.destroy_process_group()
         return
     peak, peak_src = measured_peak()
-    k3_gbs = K3_BYTES_PER_PX * npx / (stage_ms[1] * 1e-3) / 1e9
+    k3_gbs = K3_BYTES_PER_PX * npx / (unfused_ms[1] * 1e-3) / 1e9
+    tile_bpp = 5.0 if args.unfused else TILE_BYTES_PER_PX
+    tile_gbs = tile_bpp * npx / (tile_ms * 1e-3) / 1e9
     line = {
         "metric": METRIC, "value": value, "unit": "Mpix/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32/f64",
         "data": "synthetic",
         "config": {"workload": cfg.name, "B": B, "H": H, "W": W, "mesh": cfg.mesh, "filter": cfg.filt, "detect_k": cfg.detect_k,
                    "min_area": cfg.min_area, "sources_found": n_src, "parallelism": f"frames x{world} (no collective)",
+                   "calls": "bkg_estimate + bkg_subtract + detect_sources" if args.unfused else "bkg_estimate + bkg_subtract_detect",
                    "l2": "input 340 MB per step > 126 MB L2 (no flush needed)" if npx * 4 > 200e6 else "inputs smaller than L2: L2-warm"},
-        "stages_ms": {"bkg_estimate": stage_ms[0], "bkg_subtract": stage_ms[1], "detect_sources": stage_ms[2]},
+        "stages_ms": ({"bkg_estimate": stage_ms[0], "bkg_subtract": stage_ms[1], "detect_sources": stage_ms[2]} if args.unfused else
+                      {"bkg_estimate": stage_ms[0], "bkg_subtract_detect": stage_ms[1]}),
+        "stages_ms_separate_calls": {"bkg_estimate": unfused_ms[0], "bkg_subtract": unfused_ms[1], "detect_sources": unfused_ms[2]},
         "chain_roofline": {"bytes_per_px": CHAIN_BYTES_PER_PX, "achieved_gbs": CHAIN_BYTES_PER_PX * npx / (ms_per_step * 1e-3) / 1e9,
                            "frac_of_measured": CHAIN_BYTES_PER_PX * npx / (ms_per_step * 1e-3) / 1e9 / peak,
                            "frac_of_8000": CHAIN_BYTES_PER_PX * npx / (ms_per_step * 1e-3) / 1e9 / 8000.0},
-        "roofline": {"kernel": "k3_interp_subtract", "bound": "hbm", "achieved": k3_gbs, "peak": peak, "unit": "GB/s",
-                     "frac": k3_gbs / peak, "frac_of_8000": k3_gbs / 8000.0, "traffic": None, "peak_source": peak_src,
-                     "bytes_per_px": K3_BYTES_PER_PX},
-        "gpu_launches": LAUNCHES_PER_STEP * args.steps,
+        "roofline": {"kernel": "k4a_tile_label" + ("" if args.unfused else "<fused: a3 + a4 + partial sums of a5>"), "bound": "hbm",
+                     "achieved": tile_gbs, "peak": peak, "unit": "GB/s", "frac": tile_gbs / peak, "frac_of_8000": tile_gbs / 8000.0,
+                     "traffic": TILE_TRAFFIC_NCU if not args.unfused and args.config == 3 else None, "peak_source": peak_src,
+                     "bytes_per_px": tile_bpp, "ms": tile_ms},
+        "roofline_k3_pass": {"kernel": "k3_interp_subtract (bkg_subtract called alone)", "bound": "hbm", "achieved": k3_gbs, "peak": peak,
+                             "unit": "GB/s", "frac": k3_gbs / peak, "frac_of_8000": k3_gbs / 8000.0, "traffic": K3_TRAFFIC_NCU if args.config == 3 else None,
+                             "bytes_per_px": K3_BYTES_PER_PX, "ms": unfused_ms[1]},
+        "gpu_launches": (LAUNCHES_PER_STEP_UNFUSED if args.unfused else LAUNCHES_PER_STEP) * args.steps,
         "clocks": sampler.summary(),
         "host": {"nproc": os.cpu_count()},
     }

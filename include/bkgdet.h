@@ -126,14 +126,29 @@ int bkg_subtract(bd_ctx *ctx, const float *d_img, int B, int H, int W, int mesh_
  * min(n_total, cat_capacity) are written.  d_n_sources: int64 [B] true per-frame counts (device).
  * Catalogue overflow is not an error: records beyond cat_capacity are dropped.
  * Sums use float64 atomics: flux/centroid/moments are not bit-reproducible run to run (labels are).
- * d_ws / ws_bytes: at least bd_detect_workspace_bytes(). */
+ * d_ws / ws_bytes: at least bd_detect_workspace_bytes() (about 26 bytes per pixel: the record table is sized for the
+ * worst case of one component per 2x2 pixels, so it cannot overflow; only the records in use are touched). */
 int detect_sources(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_t *d_mask,
                    int B, int H, int W, double detect_k, int32_t min_area,
                    int32_t *d_labels, bd_source *d_cat, int64_t cat_capacity, int64_t *d_n_sources,
                    void *d_ws, size_t ws_bytes, void *cuda_stream);
 
+/* ---- bkg_subtract_detect = a3 + a4 + a5 in one pass (fused tile kernel).  PAPER.md:80, :61-65, :153, :159. -------
+ * Same results as bkg_subtract followed by detect_sources on its mask (the two share their arithmetic: maps, mask
+ * and labels are bit-identical; catalogue sums differ only by atomic order), but the 128x64-pixel tile kernel of
+ * detect_sources evaluates the splines itself, so the streaming of the maps overlaps the labelling and neither the
+ * mask nor sub is read back from HBM.  Arguments as in the two calls: d_sub required; d_bkg, d_rms, d_mask may be
+ * NULL (not emitted).  For mesh_w < 33 (spline table too large for the tile kernel) or frames smaller than one tile the
+ * call runs the two passes one after the other (same results).
+ * d_ws / ws_bytes: at least bd_detect_workspace_bytes(). */
+int bkg_subtract_detect(bd_ctx *ctx, const float *d_img, int B, int H, int W, int mesh_h, int mesh_w,
+                        const double *d_bkg_coef, const double *d_rms_coef, double detect_k, int32_t min_area,
+                        float *d_sub, float *d_bkg, float *d_rms, uint8_t *d_mask, int32_t *d_labels,
+                        bd_source *d_cat, int64_t cat_capacity, int64_t *d_n_sources, void *d_ws, size_t ws_bytes,
+                        void *cuda_stream);
+
 /* ---- whole chain from HOST buffers (pinned or pageable), synchronous. ----------------------------------
- * Copies h_img to the device, runs bkg_estimate -> bkg_subtract -> detect_sources, copies the
+ * Copies h_img to the device, runs bkg_estimate -> bkg_subtract_detect, copies the
  * catalogue and the per-frame counts back, and waits.  Device buffers are cached in ctx between calls.
  * h_cat: [cat_capacity] records; h_n_sources: [B].  Returns BD_OK or an error code. */
 int bd_run_host(bd_ctx *ctx, const float *h_img, int B, int H, int W, const bd_bkg_params *p,

@@ -16,11 +16,11 @@ import torch
 from . import _build
 
 __all__ = ["BkgParams", "Context", "SOURCE_DTYPE", "bkg_estimate", "bkg_subtract", "detect_sources", "mesh_stats",
-           "grid_filter_spline", "run_host", "grid_shape", "load_library", "EXPORTS"]
+           "grid_filter_spline", "bkg_subtract_detect", "run_host", "grid_shape", "load_library", "EXPORTS"]
 
 EXPORTS = ["bd_create", "bd_destroy", "bd_last_error", "bd_default_bkg_params", "bd_grid_shape",
            "bd_bkg_workspace_bytes", "bd_detect_workspace_bytes", "bd_mesh_stats", "bd_grid_filter_spline",
-           "bkg_estimate", "bkg_subtract", "detect_sources", "bd_run_host"]
+           "bkg_estimate", "bkg_subtract", "detect_sources", "bkg_subtract_detect", "bd_run_host"]
 
 
 class _CParams(C.Structure):
@@ -139,6 +139,14 @@ def k1_force_slow(ctx: "Context", on: bool) -> None:
     ctx.check(ctx.lib.bd_debug_k1_force_slow(ctx.h, C.c_int(1 if on else 0)))
 
 
+def tile_kernel_events(ctx: "Context", ev_before, ev_after) -> None:
+    """Diagnostics: torch.cuda.Event pair (already recorded once, so that their handles exist) that the library records
+    right before / after the tile kernel of detect_sources / bkg_subtract_detect; (None, None) switches it off."""
+    h0 = C.c_void_p(0 if ev_before is None else ev_before.cuda_event)
+    h1 = C.c_void_p(0 if ev_after is None else ev_after.cuda_event)
+    ctx.check(ctx.lib.bd_debug_tile_kernel_events(ctx.h, h0, h1))
+
+
 def _dev(ctx):
     return torch.device("cuda", ctx.device)
 
@@ -215,6 +223,31 @@ def detect_sources(ctx: Context, sub: torch.Tensor, rms: torch.Tensor | None, ma
                                      C.c_int32(min_area), _ptr(labels), _ptr(cat), C.c_int64(cat_capacity), _ptr(nsrc),
                                      _ptr(ws), C.c_size_t(ws.numel()), _stream()))
     return dict(labels=labels, cat=cat, n_sources=nsrc)
+
+
+def bkg_subtract_detect(ctx: Context, img: torch.Tensor, mesh_h: int, mesh_w: int, bkg_coef: torch.Tensor,
+                        rms_coef: torch.Tensor, detect_k: float, min_area: int, cat_capacity: int,
+                        want_bkg: bool = True, want_rms: bool = True, want_mask: bool = True,
+                        ws: torch.Tensor | None = None, out: dict | None = None):
+    """a3 + a4 + a5 in one pass.  -> dict(sub, bkg, rms, mask, labels, cat, n_sources)."""
+    B, H, W = img.shape
+    dev = _dev(ctx)
+    o = out or {}
+    def buf(key, dtype, want=True):
+        if not want:
+            return None
+        return o.get(key) if o.get(key) is not None else torch.empty((B, H, W), dtype=dtype, device=dev)
+    sub = buf("sub", torch.float32); bkg = buf("bkg", torch.float32, want_bkg); rms = buf("rms", torch.float32, want_rms)
+    mask = buf("mask", torch.uint8, want_mask); labels = buf("labels", torch.int32)
+    cat = o.get("cat") if o.get("cat") is not None else torch.empty(max(cat_capacity, 1) * SOURCE_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+    nsrc = o.get("n_sources") if o.get("n_sources") is not None else torch.empty(B, dtype=torch.int64, device=dev)
+    if ws is None:
+        ws = torch.empty(ctx.detect_workspace_bytes(B, H, W, cat_capacity), dtype=torch.uint8, device=dev)
+    ctx.check(ctx.lib.bkg_subtract_detect(ctx.h, _ptr(img), B, H, W, mesh_h, mesh_w, _ptr(bkg_coef), _ptr(rms_coef),
+                                          C.c_double(detect_k), C.c_int32(min_area), _ptr(sub), _ptr(bkg), _ptr(rms),
+                                          _ptr(mask), _ptr(labels), _ptr(cat), C.c_int64(cat_capacity), _ptr(nsrc),
+                                          _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+    return dict(sub=sub, bkg=bkg, rms=rms, mask=mask, labels=labels, cat=cat, n_sources=nsrc)
 
 
 def catalogue_to_numpy(cat: torch.Tensor, n_sources: torch.Tensor, cat_capacity: int) -> np.ndarray:

@@ -172,7 +172,38 @@ int detect_sources(bd_ctx *ctx, const float *d_sub, const float *d_rms, const ui
     if (!aligned16(d_sub) || !aligned16(d_labels) || !aligned16(d_mask) || !aligned16(d_rms))
         return bd_set_error(ctx, BD_EINVAL, "misaligned pointer (16 bytes required)");
     return k45_launch(ctx, d_sub, d_rms, d_mask, B, H, W, detect_k, min_area, d_labels, d_cat, cat_capacity, d_n_sources,
-                      d_ws, ws_bytes, (cudaStream_t)cuda_stream);
+                      d_ws, ws_bytes, (cudaStream_t)cuda_stream, nullptr);
+}
+
+int bkg_subtract_detect(bd_ctx *ctx, const float *d_img, int B, int H, int W, int mesh_h, int mesh_w, const double *d_bkg_coef,
+                        const double *d_rms_coef, double detect_k, int32_t min_area, float *d_sub, float *d_bkg, float *d_rms,
+                        uint8_t *d_mask, int32_t *d_labels, bd_source *d_cat, int64_t cat_capacity, int64_t *d_n_sources,
+                        void *d_ws, size_t ws_bytes, void *cuda_stream) {
+    int rc = check_frame(ctx, B, H, W);
+    if (rc) return rc;
+    if (mesh_h <= 0 || mesh_w <= 0) return bd_set_error(ctx, BD_EINVAL, "mesh size must be positive");
+    if (!d_img || !d_bkg_coef || !d_rms_coef || !d_sub || !d_labels || !d_n_sources || !d_ws)
+        return bd_set_error(ctx, BD_EINVAL, "null pointer");
+    if (!(detect_k > 0.0)) return bd_set_error(ctx, BD_EINVAL, "detect_k must be > 0");
+    if (cat_capacity < 0 || (cat_capacity > 0 && !d_cat)) return bd_set_error(ctx, BD_EINVAL, "bad catalogue buffer");
+    if (!aligned16(d_img) || !aligned16(d_sub) || !aligned16(d_bkg) || !aligned16(d_rms) || !aligned16(d_mask) || !aligned16(d_labels))
+        return bd_set_error(ctx, BD_EINVAL, "misaligned pointer (16 bytes required)");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (!k45_can_fuse(ctx, H, W, mesh_w)) {   // frame smaller than a tile, or mesh too narrow for the tile kernel's spline table:
+        size_t need = 0;                      // the two passes one after the other (the mask goes through the workspace if need be)
+        bd_detect_workspace_bytes(ctx, B, H, W, cat_capacity, &need);
+        if (ws_bytes < need) return bd_set_error(ctx, BD_EWORKSPACE, "detect workspace: need %zu bytes, got %zu", need, ws_bytes);
+        uint8_t *mask = d_mask ? d_mask : k45_ws_maskbuf(d_ws, B, H, W);
+        rc = k3_launch(ctx, d_img, B, H, W, mesh_h, mesh_w, d_bkg_coef, d_rms_coef, detect_k, d_sub, d_bkg, d_rms, mask, st);
+        if (rc) return rc;
+        return k45_launch(ctx, d_sub, d_rms, mask, B, H, W, detect_k, min_area, d_labels, d_cat, cat_capacity, d_n_sources, d_ws,
+                          ws_bytes, st, nullptr);
+    }
+    K45Fused fz;
+    fz.img = d_img; fz.bcoef = d_bkg_coef; fz.rcoef = d_rms_coef;
+    fz.sub = d_sub; fz.bkg = d_bkg; fz.rms = d_rms; fz.mask = d_mask; fz.mh = mesh_h; fz.mw = mesh_w;
+    return k45_launch(ctx, d_sub, d_rms, nullptr, B, H, W, detect_k, min_area, d_labels, d_cat, cat_capacity, d_n_sources, d_ws,
+                      ws_bytes, st, &fz);
 }
 
 int bd_run_host(bd_ctx *ctx, const float *h_img, int B, int H, int W, const bd_bkg_params *p, double detect_k,
@@ -207,13 +238,10 @@ int bd_run_host(bd_ctx *ctx, const float *h_img, int B, int H, int W, const bd_b
     rc = bkg_estimate(ctx, (const float *)(d + o_img), B, H, W, p, nullptr, nullptr, (double *)(d + o_cb), (double *)(d + o_cr),
                       d + o_wsb, ws_b, st);
     if (rc) return rc;
-    rc = bkg_subtract(ctx, (const float *)(d + o_img), B, H, W, p->mesh_h, p->mesh_w, (const double *)(d + o_cb),
-                      (const double *)(d + o_cr), detect_k, (float *)(d + o_sub), nullptr, (float *)(d + o_rms),
-                      (uint8_t *)(d + o_mask), st);
-    if (rc) return rc;
-    rc = detect_sources(ctx, (const float *)(d + o_sub), (const float *)(d + o_rms), (const uint8_t *)(d + o_mask), B, H, W,
-                        detect_k, min_area, (int32_t *)(d + o_lab), (bd_source *)(d + o_cat), cat_capacity,
-                        (int64_t *)(d + o_n), d + o_wsd, ws_d, st);
+    rc = bkg_subtract_detect(ctx, (const float *)(d + o_img), B, H, W, p->mesh_h, p->mesh_w, (const double *)(d + o_cb),
+                             (const double *)(d + o_cr), detect_k, min_area, (float *)(d + o_sub), nullptr, (float *)(d + o_rms),
+                             (uint8_t *)(d + o_mask), (int32_t *)(d + o_lab), (bd_source *)(d + o_cat), cat_capacity,
+                             (int64_t *)(d + o_n), d + o_wsd, ws_d, st);
     if (rc) return rc;
     BD_CUDA_CHECK(ctx, cudaMemcpyAsync(h_n_sources, d + o_n, (size_t)B * 8, cudaMemcpyDeviceToHost, st));
     BD_CUDA_CHECK(ctx, cudaStreamSynchronize(st));

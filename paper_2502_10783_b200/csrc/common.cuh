@@ -14,6 +14,7 @@ struct bd_ctx {
     size_t smem_optin;
     char err[512];
     int k1_force_slow;   // diagnostics: K1 skips its fast path
+    cudaEvent_t dbg_ev0, dbg_ev1;   // diagnostics: recorded around the tile kernel of detect_sources / bkg_subtract_detect
     // cuTensorMapEncodeTiled, fetched through the runtime (no -lcuda link dependency)
     CUresult (*encode_tiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                              const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
@@ -64,9 +65,19 @@ int k3_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, int mh, int 
               cudaStream_t st);
 
 size_t k45_workspace_bytes(int B, int H, int W, int64_t cat_capacity);
+// fused step a3 + a4 + a5: the tile kernel evaluates the splines itself (no mask / sub input)
+struct K45Fused {
+    const float *img;
+    const double *bcoef, *rcoef;
+    float *sub, *bkg, *rms;   // sub required; bkg, rms may be null
+    uint8_t *mask;            // may be null
+    int mh, mw;
+};
+bool k45_can_fuse(const bd_ctx *ctx, int H, int W, int mesh_w);
+uint8_t *k45_ws_maskbuf(void *d_ws, int B, int H, int W);
 int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_t *d_mask, int B, int H, int W,
                double detect_k, int min_area, int32_t *d_labels, bd_source *d_cat, int64_t cat_capacity,
-               int64_t *d_n_sources, void *d_ws, size_t ws_bytes, cudaStream_t st);
+               int64_t *d_n_sources, void *d_ws, size_t ws_bytes, cudaStream_t st, const K45Fused *fz);
 
 // ---- small device helpers ------------------------------------------------------------------------------
 #ifdef __CUDACC__

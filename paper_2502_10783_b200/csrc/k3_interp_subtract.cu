@@ -18,6 +18,7 @@
 // instruction runs per pixel.  (The float32 ulp at ~1000 ADU, 6e-5, would not be good enough for the
 // 1e-5*sigma mask agreement if bkg itself were accumulated in float32.)
 #include "common.cuh"
+#include "spline_eval.cuh"
 
 namespace {
 
@@ -33,24 +34,8 @@ constexpr int K3_PX = 4;     // pixels per thread per row (one float4)
 #define K3_STRIP_ROWS 32
 #endif
 constexpr int K3_R = K3_ROWS_IN_FLIGHT;   // rows whose loads are in flight per thread
-constexpr int K3_ENT = 12;   // floats per table entry (48 B: three 128-bit shared loads)
+constexpr int K3_ENT = SPL_ENT;   // floats per table entry (48 B: three 128-bit shared loads)
 constexpr int K3_TABLE_BYTES = 40 * 1024;
-
-__device__ __forceinline__ void bspline_weights(double t, double w[4]) {
-    // beta3 at distances 1+t, t, 1-t, 2-t  (t in [0,1))
-    double omt = 1.0 - t;
-    w[0] = omt * omt * omt / 6.0;
-    w[1] = (4.0 - 6.0 * t * t + 3.0 * t * t * t) / 6.0;
-    w[2] = (4.0 - 6.0 * omt * omt + 3.0 * omt * omt * omt) / 6.0;
-    w[3] = t * t * t / 6.0;
-}
-
-__device__ __forceinline__ int reflect_idx(int k, int n) {   // half-sample symmetric: -1->0, n->n-1, period 2n
-    int p = 2 * n;
-    k %= p;
-    if (k < 0) k += p;
-    return k < n ? k : p - 1 - k;
-}
 
 struct K3Args {
     const float *img;
@@ -76,39 +61,14 @@ __global__ void __launch_bounds__(K3_NT, K3_MIN_CTAS) k3_interp_subtract(K3Args 
     const size_t frame_off = (size_t)frame * a.H * a.W;
     const double *bc = a.bcoef + (size_t)frame * a.ny * a.nx;
     const double *rc = a.rcoef + (size_t)frame * a.ny * a.nx;
-    const double inv_mw = 1.0 / (double)a.mw, inv_mh = 1.0 / (double)a.mh;
-    // floor((x + 0.5)/mw - 0.5) with exact integer arithmetic: floor((2x + 1 - mw) / (2 mw))
-    auto cell_of = [](int x, int m) { int num = 2 * x + 1 - m, den = 2 * m; return num >= 0 ? num / den : -((-num + den - 1) / den); };
-    const int i0_first = cell_of(xc0, a.mw);
-    const int n_i0 = cell_of(xc1, a.mw) - i0_first + 1;
+    const int i0_first = spl_cell_of(xc0, a.mw);
+    const int n_i0 = spl_cell_of(xc1, a.mw) - i0_first + 1;
 
     // ---- table: one entry per (row, i0) --------------------------------------------------------------
     const int n_ent = (y_end - y_begin) * n_i0;
     for (int e = threadIdx.x; e < n_ent; e += K3_NT) {
         const int r = e / n_i0, ii = e - r * n_i0;
-        const int y = y_begin + r, i0 = i0_first + ii;
-        const int j0 = cell_of(y, a.mh);
-        double wy[4];
-        bspline_weights(((double)y + 0.5) * inv_mh - 0.5 - (double)j0, wy);
-        double hb[4] = {0, 0, 0, 0}, hr[4] = {0, 0, 0, 0};
-#pragma unroll
-        for (int rr = 0; rr < 4; ++rr) {
-            const size_t row = (size_t)reflect_idx(j0 - 1 + rr, a.ny) * a.nx;
-#pragma unroll
-            for (int d = 0; d < 4; ++d) {
-                const int ci = reflect_idx(i0 - 1 + d, a.nx);
-                hb[d] = fma(wy[rr], __ldg(bc + row + ci), hb[d]);
-                hr[d] = fma(wy[rr], __ldg(rc + row + ci), hr[d]);
-            }
-        }
-        float *t = table + (size_t)e * K3_ENT;
-        const float hi = (float)hb[1];
-        t[0] = hi;
-        t[1] = (float)(hb[1] - (double)hi);
-        t[2] = (float)(hb[0] - hb[1]);
-        t[3] = (float)(hb[2] - hb[1]);
-        t[4] = (float)(hb[3] - hb[1]);
-        t[5] = (float)hr[0]; t[6] = (float)hr[1]; t[7] = (float)hr[2]; t[8] = (float)hr[3];
+        spl_table_entry(bc, rc, a.ny, a.nx, a.mh, y_begin + r, i0_first + ii, table + (size_t)e * K3_ENT);
     }
     __syncthreads();
     if (x0 >= a.W) return;
@@ -118,10 +78,8 @@ __global__ void __launch_bounds__(K3_NT, K3_MIN_CTAS) k3_interp_subtract(K3Args 
     int ent_off[K3_PX];
 #pragma unroll
     for (int q = 0; q < K3_PX; ++q) {
-        const int i0 = cell_of(x0 + q, a.mw);
-        double w[4];
-        bspline_weights(((double)(x0 + q) + 0.5) * inv_mw - 0.5 - (double)i0, w);
-        wx[q][0] = (float)w[0]; wx[q][1] = (float)w[1]; wx[q][2] = (float)w[2]; wx[q][3] = (float)w[3];
+        const int i0 = spl_cell_of(x0 + q, a.mw);
+        spl_x_weights(x0 + q, a.mw, i0, wx[q]);
         ent_off[q] = (i0 - i0_first) * K3_ENT;
     }
     const int row_stride = n_i0 * K3_ENT;
@@ -156,20 +114,7 @@ __global__ void __launch_bounds__(K3_NT, K3_MIN_CTAS) k3_interp_subtract(K3Args 
                     t1 = *reinterpret_cast<const float4 *>(t + 4);
                     t8 = t[8];
                 }
-                // t0 = {hi, lo, e_-1, e_+1}, t1 = {e_+2, r_-1, r_0, r_+1}, t8 = r_+2
-                float rel = wx[q][0] * t0.z;
-                rel = fmaf(wx[q][2], t0.w, rel);
-                rel = fmaf(wx[q][3], t1.x, rel);
-                rel += t0.y;
-                float s = wx[q][0] * t1.y;
-                s = fmaf(wx[q][1], t1.z, s);
-                s = fmaf(wx[q][2], t1.w, s);
-                s = fmaf(wx[q][3], t8, s);
-                const float d = (in[q] - t0.x) - rel;
-                o_sub[q] = d;
-                o_bkg[q] = t0.x + rel;
-                o_rms[q] = s;
-                const bool fg = (s > 0.0f) && (d > a.k_d * s);
+                const bool fg = spl_pixel(t0, t1, t8, wx[q], in[q], a.k_d, o_sub[q], o_bkg[q], o_rms[q]);
                 mbits |= (fg ? 1u : 0u) << (8 * q);
             }
             const size_t off = frame_off + (size_t)y * a.W + x0;

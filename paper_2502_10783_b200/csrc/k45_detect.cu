@@ -27,6 +27,7 @@
 // one: they would be 8-adjacent), so no allocation can overflow; only the touched entries cost traffic.
 // Labels are bit-exact by construction; float sums depend on atomic order (not bit-reproducible).
 #include "common.cuh"
+#include "spline_eval.cuh"
 
 namespace {
 
@@ -146,6 +147,13 @@ struct K4Args {
     uint32_t *recidx;
     uint32_t *counters;
     int skip_isolated;   // min_area > 1: pixels without any foreground neighbour never enter the list
+    // fused mode (FUSED = true): phase A evaluates the background / RMS splines itself (step a3) instead of reading a mask
+    const float *img;
+    const double *bcoef, *rcoef;
+    float *sub_out, *bkg, *rms;
+    uint8_t *mask_out;
+    int mh, mw, ny, nx, uniform;
+    float k_d;
 };
 
 constexpr int SM_LAB = 0;
@@ -188,7 +196,9 @@ __device__ __forceinline__ uint32_t raw_to_word(const Raw8 &r) {
     return word;
 }
 
-__global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant__ CUtensorMap tmap_lab, K4Args a) {
+template <bool FUSED>
+__global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant__ CUtensorMap tmap_lab,
+                                                               const __grid_constant__ CUtensorMap tmap_img, K4Args a) {
     extern __shared__ __align__(128) unsigned char sm[];
     uint32_t *lab = reinterpret_cast<uint32_t *>(sm + SM_LAB);
     uint16_t *list = reinterpret_cast<uint16_t *>(sm + SM_LIST);
@@ -208,24 +218,153 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
 #endif
 
     // ---- A: zero the label tile, mask bytes -> bit rows with a 1-pixel halo -------------------------------
-#pragma unroll
-    for (int k = 0; k < TPX / 4 / K4_NT; ++k) reinterpret_cast<uint4 *>(lab)[k * K4_NT + tid] = make_uint4(0, 0, 0, 0);
     if (tid == 0) { wsum[8] = 0; wsum[10] = 0; }
-    const Raw8 raw_m = load_mask_raw(a, fbase, y0 + row_w, x0 + 32 * w_w);
-    Raw8 raw_h;
-    uint32_t hbit = 0;
-    const int hcol = tid - 8;   // halo column element (if 0 <= hcol < 2 * BROWS)
-    if (tid < 8) {              // halo rows y0-1 and y0+TH
-        raw_h = load_mask_raw(a, fbase, y0 - 1 + (tid < 4 ? 0 : BROWS - 1), x0 + 32 * (tid & 3));
-    } else if (hcol < BROWS * 2) {   // halo columns x0-1 and x0+TW
-        const int y = y0 - 1 + (hcol >> 1), x = (hcol & 1) ? x0 + TW : x0 - 1;
-        if (y >= 0 && y < H && x >= 0 && x < W) hbit = __ldg(a.mask + fbase + (size_t)y * W + x) ? 1u : 0u;
+    if constexpr (FUSED) {
+        // the tile's image pixels: one TMA bulk-tensor load into the label buffer (unused until phase B), in flight
+        // while the spline table is built; rows / columns past the frame edge are zero-filled and never used
+        if (tid == 0) {
+            const uint32_t bar = smem_u32(&wsum[12]);
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"((uint32_t)(TPX * 4)) : "memory");
+            asm volatile(
+                "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                ::"r"(smem_u32(lab)), "l"(&tmap_img), "r"(x0), "r"(y0), "r"(frame), "r"(bar)
+                : "memory");
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < TPX / 4 / K4_NT; ++k) reinterpret_cast<uint4 *>(lab)[k * K4_NT + tid] = make_uint4(0, 0, 0, 0);
     }
-    const uint32_t M = raw_to_word(raw_m);
-    bits[row_w + 1][1 + w_w] = M;
-    if (tid < 8) bits[tid < 4 ? 0 : BROWS - 1][1 + (tid & 3)] = raw_to_word(raw_h);
-    else if (hcol < BROWS * 2) bits[hcol >> 1][(hcol & 1) ? 5 : 0] = (hcol & 1) ? hbit : hbit << 31;
+    uint32_t M;
+    if constexpr (FUSED) {
+        // ---- A (fused): step a3 for the tile and its 1-pixel halo: spline table -> sub, bkg, rms (written out),
+        //      threshold bits.  Arithmetic shared with K3 (spline_eval.cuh): bit-identical maps and mask.
+        float *table = reinterpret_cast<float *>(sm + SM_LIST);   // aliases the list (built in B)
+        const double *bc = a.bcoef + (size_t)frame * a.ny * a.nx, *rc = a.rcoef + (size_t)frame * a.ny * a.nx;
+        const int ry0 = max(y0 - 1, 0), ry1 = min(y0 + TH, H - 1), cx0 = max(x0 - 1, 0), cx1 = min(x0 + TW, W - 1);
+        const int i0_first = spl_cell_of(cx0, a.mw), n_i0 = spl_cell_of(cx1, a.mw) - i0_first + 1;
+        const int row_stride = n_i0 * SPL_ENT;
+        const int xt = x0 + 4 * lane;                // this thread's four columns
+        const bool col_ok = xt < W;
+        const float *img = a.img + fbase;
+        // halo loads first (the tile itself arrives by TMA): the halo row of warps 0 / 1, one halo-column pixel
+        const int yh = warp == 0 ? y0 - 1 : y0 + TH;   // halo row of warp 0 / warp 1
+        const bool hrow_ok = warp < 2 && col_ok && yh >= 0 && yh < H;
+        float4 pixh = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (hrow_ok) pixh = __ldg(reinterpret_cast<const float4 *>(img + (size_t)yh * W + xt));
+        const int hcy = y0 - 1 + (tid >> 1), hcx = (tid & 1) ? x0 + TW : x0 - 1;   // halo-column pixel of threads < 2 * BROWS
+        const bool hcol_ok = tid < 2 * BROWS && hcy >= 0 && hcy < H && hcx >= 0 && hcx < W;
+        float pixc = 0.f;
+        if (hcol_ok) pixc = __ldg(img + (size_t)hcy * W + hcx);
+        // table: one entry per (row, grid cell) of the halo region
+        const int n_ent = (ry1 - ry0 + 1) * n_i0;
+        for (int e = tid; e < n_ent; e += K4_NT) {
+            const int r = e / n_i0, ii = e - r * n_i0;
+            spl_table_entry(bc, rc, a.ny, a.nx, a.mh, ry0 + r, i0_first + ii, table + (size_t)e * SPL_ENT);
+        }
+        float wx[4][4];
+        int ent_off[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int i0 = spl_cell_of(min(xt + q, W - 1), a.mw);
+            spl_x_weights(xt + q, a.mw, i0, wx[q]);
+            ent_off[q] = (i0 - i0_first) * SPL_ENT;
+        }
+        __syncthreads();
+        auto eval4 = [&](const float4 &px, int y, float o_sub[4], float o_bkg[4], float o_rms[4]) -> uint32_t {
+            const float *trow = table + (size_t)(y - ry0) * row_stride;
+            const float in[4] = {px.x, px.y, px.z, px.w};
+            uint32_t nib = 0;
+            float4 t0, t1;
+            float t8;
+            if (a.uniform) {
+                const float *t = trow + ent_off[0];
+                t0 = *reinterpret_cast<const float4 *>(t); t1 = *reinterpret_cast<const float4 *>(t + 4); t8 = t[8];
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                if (!a.uniform) {
+                    const float *t = trow + ent_off[q];
+                    t0 = *reinterpret_cast<const float4 *>(t); t1 = *reinterpret_cast<const float4 *>(t + 4); t8 = t[8];
+                }
+                nib |= (spl_pixel(t0, t1, t8, wx[q], in[q], a.k_d, o_sub[q], o_bkg[q], o_rms[q]) ? 1u : 0u) << q;
+            }
+            return nib;
+        };
+        auto put_bits = [&](uint32_t nib, int hr) {   // 8 lanes x 4 bits -> one word of bit row hr
+            uint32_t word = nib << (4 * (lane & 7));
+            word |= __shfl_xor_sync(0xffffffffu, word, 1);
+            word |= __shfl_xor_sync(0xffffffffu, word, 2);
+            word |= __shfl_xor_sync(0xffffffffu, word, 4);
+            if ((lane & 7) == 0) bits[hr][1 + (lane >> 3)] = word;
+        };
+        {   // wait for the tile
+            const uint32_t bar = smem_u32(&wsum[12]);
+            uint32_t done = 0;
+            while (!done)
+                asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
+                             : "=r"(done) : "r"(bar) : "memory");
+        }
+        const float4 *tile4 = reinterpret_cast<const float4 *>(lab);
+#pragma unroll 2
+        for (int k = 0; k < TH / 8; ++k) {
+            const int row = warp + 8 * k, y = y0 + row;
+            uint32_t nib = 0;
+            if (col_ok && y < H) {
+                float o_sub[4], o_bkg[4], o_rms[4];
+                nib = eval4(tile4[row * (TW / 4) + lane], y, o_sub, o_bkg, o_rms);
+                const size_t off = fbase + (size_t)y * W + xt;
+                *reinterpret_cast<float4 *>(a.sub_out + off) = make_float4(o_sub[0], o_sub[1], o_sub[2], o_sub[3]);
+                if (a.bkg) __stcs(reinterpret_cast<float4 *>(a.bkg + off), make_float4(o_bkg[0], o_bkg[1], o_bkg[2], o_bkg[3]));
+                if (a.rms) __stcs(reinterpret_cast<float4 *>(a.rms + off), make_float4(o_rms[0], o_rms[1], o_rms[2], o_rms[3]));
+                if (a.mask_out)
+                    __stcs(reinterpret_cast<uint32_t *>(a.mask_out + off),
+                           (nib & 1u) | (nib & 2u) << 7 | (nib & 4u) << 14 | (nib & 8u) << 21);
+            }
+            put_bits(nib, row + 1);
+        }
+        if (warp < 2) {   // halo rows: bits only
+            uint32_t nib = 0;
+            if (hrow_ok) {
+                float o_sub[4], o_bkg[4], o_rms[4];
+                nib = eval4(pixh, yh, o_sub, o_bkg, o_rms);
+            }
+            put_bits(nib, warp == 0 ? 0 : BROWS - 1);
+        }
+        if (tid < 2 * BROWS) {   // halo columns: one pixel each
+            uint32_t bit = 0;
+            if (hcol_ok) {
+                const int i0 = spl_cell_of(hcx, a.mw);
+                float wxc[4], o_s, o_b, o_r;
+                spl_x_weights(hcx, a.mw, i0, wxc);
+                const float *t = table + (size_t)(hcy - ry0) * row_stride + (i0 - i0_first) * SPL_ENT;
+                bit = spl_pixel(*reinterpret_cast<const float4 *>(t), *reinterpret_cast<const float4 *>(t + 4), t[8], wxc, pixc, a.k_d,
+                                o_s, o_b, o_r) ? 1u : 0u;
+            }
+            bits[tid >> 1][(tid & 1) ? 5 : 0] = (tid & 1) ? bit : bit << 31;
+        }
+        __syncthreads();   // every pixel of the tile buffer has been consumed: it becomes the label array
+#pragma unroll
+        for (int k = 0; k < TPX / 4 / K4_NT; ++k) reinterpret_cast<uint4 *>(lab)[k * K4_NT + tid] = make_uint4(0, 0, 0, 0);
+        M = bits[row_w + 1][1 + w_w];
+    } else {
+        const Raw8 raw_m = load_mask_raw(a, fbase, y0 + row_w, x0 + 32 * w_w);
+        Raw8 raw_h;
+        uint32_t hbit = 0;
+        const int hcol = tid - 8;   // halo column element (if 0 <= hcol < 2 * BROWS)
+        if (tid < 8) {              // halo rows y0-1 and y0+TH
+            raw_h = load_mask_raw(a, fbase, y0 - 1 + (tid < 4 ? 0 : BROWS - 1), x0 + 32 * (tid & 3));
+        } else if (hcol < BROWS * 2) {   // halo columns x0-1 and x0+TW
+            const int y = y0 - 1 + (hcol >> 1), x = (hcol & 1) ? x0 + TW : x0 - 1;
+            if (y >= 0 && y < H && x >= 0 && x < W) hbit = __ldg(a.mask + fbase + (size_t)y * W + x) ? 1u : 0u;
+        }
+        M = raw_to_word(raw_m);
+        bits[row_w + 1][1 + w_w] = M;
+        if (tid < 8) bits[tid < 4 ? 0 : BROWS - 1][1 + (tid & 3)] = raw_to_word(raw_h);
+        else if (hcol < BROWS * 2) bits[hcol >> 1][(hcol & 1) ? 5 : 0] = (hcol & 1) ? hbit : hbit << 31;
 
+    }
     __syncthreads();
     K4_T(0);
 
@@ -302,7 +441,8 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
         float I_pre = 0.f;
         if (tid < n) {
             const uint32_t p = list[tid];
-            I_pre = __ldg(a.sub + fbase + (size_t)(y0 + (int)(p >> 7)) * W + x0 + (int)(p & 127));
+            const float *ps = a.sub + fbase + (size_t)(y0 + (int)(p >> 7)) * W + x0 + (int)(p & 127);
+            I_pre = FUSED ? __ldcg(ps) : __ldg(ps);   // fused: sub was written by this CTA in phase A (L2-coherent load)
         }
         // ---- C: vertical / diagonal links inside the tile.  Rules (w, a, b, c = W, NW, N, NE neighbours):
         //      b && !w -> N;  !b && a && !w -> NW;  !b && c -> NE.  In-tile bits only (a halo pixel never prunes an
@@ -433,7 +573,7 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
                         row = (int)(p >> 7); x = (int)(p & 127);
                         key = (r << 6) | (uint32_t)row;
                         const int gidx = (y0 + row) * W + x0 + x;
-                        const float I = e0 == 0 ? I_pre : __ldg(a.sub + fbase + (size_t)gidx);
+                        const float I = e0 == 0 ? I_pre : (FUSED ? __ldcg(a.sub + fbase + (size_t)gidx) : __ldg(a.sub + fbase + (size_t)gidx));
                         const double dx = (double)(x - (int)(r & 127));
                         S0 = (double)I; S1 = S0 * dx; S2 = S1 * dx;
                         pk = ((u64)f32_to_key(I) << 32) | (u64)(0xFFFFFFFFu - (uint32_t)gidx);
@@ -803,9 +943,21 @@ size_t k45_workspace_bytes(int B, int H, int W, int64_t cat_capacity) {
     return carve(w, nullptr, B, H, W) + 256;
 }
 
+// the fused tile kernel keeps its spline table (66 rows x cells x 48 B) in the 16 KiB the list occupies later
+// and stages the image tile with a TMA box of TW x TH pixels
+bool k45_can_fuse(const bd_ctx *ctx, int H, int W, int mesh_w) {
+    return ctx->encode_tiled && W >= TW && H >= TH && BROWS * ((TW + 2) / mesh_w + 2) * SPL_ENT * (int)sizeof(float) <= TPX * 2;
+}
+// the P bytes of the detect workspace that hold a mask when the caller passes none
+uint8_t *k45_ws_maskbuf(void *d_ws, int B, int H, int W) {
+    Ws w;
+    carve(w, (char *)bd_align_up((size_t)d_ws, 256), B, H, W);
+    return w.maskbuf;
+}
+
 int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_t *d_mask, int B, int H, int W,
                double detect_k, int min_area, int32_t *d_labels, bd_source *d_cat, int64_t cat_capacity,
-               int64_t *d_n_sources, void *d_ws, size_t ws_bytes, cudaStream_t st) {
+               int64_t *d_n_sources, void *d_ws, size_t ws_bytes, cudaStream_t st, const K45Fused *fz) {
     Ws w;
     char *base = (char *)bd_align_up((size_t)d_ws, 256);
     size_t need = carve(w, base, B, H, W);
@@ -814,7 +966,7 @@ int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_
     const size_t P = w.P;
 
     const uint8_t *mask = d_mask;
-    if (!mask) {
+    if (!mask && !fz) {
         size_t n4 = P / 4;
         k_make_mask<<<(unsigned)((n4 + 255) / 256), 256, 0, st>>>(d_sub, d_rms, n4, detect_k, w.maskbuf);
         mask = w.maskbuf;
@@ -824,10 +976,19 @@ int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_
 
     const int TX = (W + TW - 1) / TW, TY = (H + TH - 1) / TH;
     K4Args a;
+    memset(&a, 0, sizeof(a));
     a.mask = mask; a.sub = d_sub; a.H = H; a.W = W; a.min_area = min_area;
     a.vec16 = (W % 16 == 0 && ((uintptr_t)mask & 15) == 0) ? 1 : 0;
     a.labels = d_labels; a.edges = w.edges; a.rec = w.rec; a.recidx = w.recidx; a.counters = w.counters;
     a.skip_isolated = min_area > 1 ? 1 : 0;
+    if (fz) {
+        a.img = fz->img; a.bcoef = fz->bcoef; a.rcoef = fz->rcoef;
+        a.sub_out = fz->sub; a.bkg = fz->bkg; a.rms = fz->rms; a.mask_out = fz->mask;
+        a.mh = fz->mh; a.mw = fz->mw; a.ny = (H + fz->mh - 1) / fz->mh; a.nx = (W + fz->mw - 1) / fz->mw;
+        a.uniform = fz->mw % 8 == 0 ? 1 : 0;
+        a.k_d = (float)detect_k;
+        a.sub = fz->sub;
+    }
     a.use_tma = (W >= TW && H >= TH && ctx->encode_tiled) ? 1 : 0;
     CUtensorMap tmap;
     memset(&tmap, 0, sizeof(tmap));
@@ -841,8 +1002,27 @@ int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_
                                        CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return bd_set_error(ctx, BD_ECUDA, "cuTensorMapEncodeTiled(labels) failed (%d)", (int)r);
     }
-    BD_CUDA_CHECK(ctx, cudaFuncSetAttribute(k4a_tile_label, cudaFuncAttributeMaxDynamicSharedMemorySize, K4_SMEM));
-    k4a_tile_label<<<dim3(TX, TY, B), K4_NT, K4_SMEM, st>>>(tmap, a);
+    if (ctx->dbg_ev0) cudaEventRecord(ctx->dbg_ev0, st);
+    CUtensorMap tmap_img;
+    memset(&tmap_img, 0, sizeof(tmap_img));
+    if (fz) {
+        cuuint64_t dims[3] = {(cuuint64_t)W, (cuuint64_t)H, (cuuint64_t)B};
+        cuuint64_t strides[2] = {(cuuint64_t)W * sizeof(float), (cuuint64_t)W * H * sizeof(float)};
+        cuuint32_t box[3] = {TW, TH, 1};
+        cuuint32_t estr[3] = {1, 1, 1};
+        CUresult r = ctx->encode_tiled(&tmap_img, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)fz->img, dims, strides, box, estr,
+                                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                       CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return bd_set_error(ctx, BD_ECUDA, "cuTensorMapEncodeTiled(img) failed (%d)", (int)r);
+    }
+    if (fz) {
+        BD_CUDA_CHECK(ctx, cudaFuncSetAttribute(k4a_tile_label<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, K4_SMEM));
+        k4a_tile_label<true><<<dim3(TX, TY, B), K4_NT, K4_SMEM, st>>>(tmap, tmap_img, a);
+    } else {
+        BD_CUDA_CHECK(ctx, cudaFuncSetAttribute(k4a_tile_label<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, K4_SMEM));
+        k4a_tile_label<false><<<dim3(TX, TY, B), K4_NT, K4_SMEM, st>>>(tmap, tmap_img, a);
+    }
+    if (ctx->dbg_ev1) cudaEventRecord(ctx->dbg_ev1, st);
     if (TX > 1 || TY > 1) {
         const size_t n_units = w.ntiles * 6;
         k4b_seams<<<(unsigned)((n_units + 7) / 8), 256, 0, st>>>(w.edges, d_labels, H, W, TX, TY, n_units);
@@ -866,3 +1046,12 @@ extern "C" int bd_debug_k4_timing(unsigned long long *out16, int reset) {
     return BD_OK;
 }
 #endif
+
+// diagnostics (not part of include/bkgdet.h): CUDA events (cudaEvent_t as void*, 0 = off) that the next calls record
+// on their stream immediately before and after the tile kernel, so a caller can time that kernel alone
+extern "C" int bd_debug_tile_kernel_events(bd_ctx *ctx, void *ev_before, void *ev_after) {
+    if (!ctx) return BD_EINVAL;
+    ctx->dbg_ev0 = (cudaEvent_t)ev_before;
+    ctx->dbg_ev1 = (cudaEvent_t)ev_after;
+    return BD_OK;
+}

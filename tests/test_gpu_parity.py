@@ -255,6 +255,12 @@ def check_chain(bd, ctx, img, p, k, min_area, frames=None):
     bm, rm, o, det = run_chain(bd, ctx, img, p, k, min_area, cap)
     cat = bd.catalogue_to_numpy(det["cat"], det["n_sources"], cap)
     n = det["n_sources"].cpu().numpy()
+    fz = bd.bkg_subtract_detect(ctx, dev(img), p.mesh_h, p.mesh_w, *bd.bkg_estimate(ctx, dev(img), p)[2:], k, min_area, cap)
+    torch.cuda.synchronize()
+    for key in ("sub", "bkg", "rms", "mask"):
+        assert torch.equal(fz[key], o[key]), f"fused {key} differs from bkg_subtract"
+    assert torch.equal(fz["labels"], det["labels"]) and torch.equal(fz["n_sources"], det["n_sources"])
+    del fz
     report = {}
     for f in (range(B) if frames is None else frames):
         r = oracle.chain(img[f], to_oracle_params(p), k, min_area)
@@ -290,6 +296,38 @@ def test_chain_configs_reduced(bd, ctx, cid, H, W, B):
     img = make_frames(cfg, H=H, W=W, B=B)
     rep = check_chain(bd, ctx, img, params_for(bd, cfg), cfg.detect_k, cfg.min_area)
     assert all(v["n_sources"] > 0 for v in rep.values())
+
+
+@pytest.mark.parametrize("cid,H,W,B,mesh", [(1, 512, 512, 1, 64), (3, 528, 768, 1, 256), (5, 300, 388, 2, 64), (2, 200, 260, 1, 50),
+                                            (1, 97, 132, 1, 36), (1, 64, 64, 1, 20)])
+def test_fused_subtract_detect_equals_two_passes(bd, ctx, cid, H, W, B, mesh):
+    """bkg_subtract_detect (fused tile kernel) against bkg_subtract + detect_sources: maps, mask and labels bit-identical,
+    catalogue equal up to the order of the float64 atomics.  mesh 36/50: four columns of a thread straddle grid cells;
+    mesh 20: the documented fallback to the two passes; ragged tiles and frame edges in all of them."""
+    cfg = CONFIGS[cid]
+    img = make_frames(cfg, H=H, W=W, B=B)
+    p = params_for(bd, cfg, mesh_h=mesh, mesh_w=mesh)
+    d_img = dev(img)
+    bm, rm, cb, cr = bd.bkg_estimate(ctx, d_img, p)
+    cap = 1 << 16
+    o = bd.bkg_subtract(ctx, d_img, p.mesh_h, p.mesh_w, cb, cr, cfg.detect_k)
+    det = bd.detect_sources(ctx, o["sub"], o["rms"], o["mask"], cfg.detect_k, cfg.min_area, cap)
+    f = bd.bkg_subtract_detect(ctx, d_img, p.mesh_h, p.mesh_w, cb, cr, cfg.detect_k, cfg.min_area, cap)
+    torch.cuda.synchronize()
+    for k in ("sub", "bkg", "rms", "mask"):
+        assert torch.equal(f[k], o[k]), k
+    assert torch.equal(f["labels"], det["labels"]) and torch.equal(f["n_sources"], det["n_sources"])
+    c1 = bd.catalogue_to_numpy(det["cat"], det["n_sources"], cap); c2 = bd.catalogue_to_numpy(f["cat"], f["n_sources"], cap)
+    assert len(c1) == len(c2) and len(c1) > 0
+    for k in ("frame", "label", "npix", "xmin", "xmax", "ymin", "ymax", "xpeak", "ypeak", "peak"):
+        assert np.array_equal(c1[k], c2[k]), k
+    for k in ("flux", "x", "y", "x2", "y2", "xy"):
+        assert np.allclose(c1[k], c2[k], rtol=1e-9, atol=1e-9), k
+    # without the optional outputs
+    f2 = bd.bkg_subtract_detect(ctx, d_img, p.mesh_h, p.mesh_w, cb, cr, cfg.detect_k, cfg.min_area, cap, want_bkg=False,
+                                want_rms=False, want_mask=False)
+    torch.cuda.synchronize()
+    assert f2["bkg"] is None and torch.equal(f2["labels"], det["labels"]) and torch.equal(f2["sub"], o["sub"])
 
 
 def test_chain_constant_frame(bd, ctx):
