@@ -68,6 +68,9 @@ struct Ws {
     uint32_t *keptbits;     // [NWk] one bit per pixel  |
     uint32_t *blkcnt;       // [NB + 1] per 4096 px     |  zeroed together every call
     uint32_t *blkprefix;    // [NB + 2]
+    float *wx_tab;          // [W][4] float32 x-weights of every image column  | fused mode: filled by k_spline_tabs
+    double *wy_tab;         // [H][4] float64 y-weights of every image row     |
+    int32_t *i0_tab, *j0_tab;   // [W], [H] grid cells                          |
     Rec *rec;               // [nblk2] records, compact: 0 .. n_rec-1 (capacity = one per 2x2 block, the worst case)
     size_t P, nblk2, NWk, NB, ntiles;
     size_t zero_bytes;      // bytes from keptbits to the end of blkcnt
@@ -91,6 +94,10 @@ size_t carve(Ws &w, void *base, int B, int H, int W) {
     w.blkcnt = (uint32_t *)take((w.NB + 8) * sizeof(uint32_t));
     w.zero_bytes = (size_t)((char *)w.blkcnt - (char *)w.keptbits) + (w.NB + 1) * sizeof(uint32_t);
     w.blkprefix = (uint32_t *)take((w.NB + 8) * sizeof(uint32_t));
+    w.wx_tab = (float *)take((size_t)W * 4 * sizeof(float));
+    w.wy_tab = (double *)take((size_t)H * 4 * sizeof(double));
+    w.i0_tab = (int32_t *)take((size_t)W * sizeof(int32_t));
+    w.j0_tab = (int32_t *)take((size_t)H * sizeof(int32_t));
     w.rec = (Rec *)take(w.nblk2 * sizeof(Rec));
     w.total = off;
     return off;
@@ -115,6 +122,27 @@ __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)_
 __device__ __forceinline__ uint32_t bytes_to_nibble(uint32_t v) {
     const uint32_t nz = ((((v & 0x7F7F7F7Fu) + 0x7F7F7F7Fu) | v) & 0x80808080u) >> 7;   // bits 0, 8, 16, 24
     return (nz * 0x00204081u >> 21) & 0xFu;
+}
+
+// ------------------------------------------------------------------------------------------------ spline weights
+// The x-weights of a column and the y-weights of a row are the same for every tile that contains them: computed once
+// per call (fused mode) with the functions K3 uses, instead of 5 float64 polynomial evaluations per thread per tile.
+__global__ void k_spline_tabs(int H, int W, int mh, int mw, float *wx_tab, double *wy_tab, int32_t *i0_tab, int32_t *j0_tab) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < W) {
+        const int i0 = spl_cell_of(t, mw);
+        float wx[4];
+        spl_x_weights(t, mw, i0, wx);
+        reinterpret_cast<float4 *>(wx_tab)[t] = make_float4(wx[0], wx[1], wx[2], wx[3]);
+        i0_tab[t] = i0;
+    }
+    if (t < H) {
+        const int j0 = spl_cell_of(t, mh);
+        double wy[4];
+        spl_y_weights(t, mh, j0, wy);
+        wy_tab[4 * t + 0] = wy[0]; wy_tab[4 * t + 1] = wy[1]; wy_tab[4 * t + 2] = wy[2]; wy_tab[4 * t + 3] = wy[3];
+        j0_tab[t] = j0;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------ K4a
@@ -154,6 +182,9 @@ struct K4Args {
     uint8_t *mask_out;
     int mh, mw, ny, nx, uniform;
     float k_d;
+    const float *wx_tab;
+    const double *wy_tab;
+    const int32_t *i0_tab, *j0_tab;
 };
 
 constexpr int SM_LAB = 0;
@@ -260,18 +291,23 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
         // table: one entry per (row, grid cell) of the halo region
         const int n_ent = (ry1 - ry0 + 1) * n_i0;
         for (int e = tid; e < n_ent; e += K4_NT) {
-            const int r = e / n_i0, ii = e - r * n_i0;
-            spl_table_entry(bc, rc, a.ny, a.nx, a.mh, ry0 + r, i0_first + ii, table + (size_t)e * SPL_ENT);
+            const int r = e / n_i0, ii = e - r * n_i0, y = ry0 + r;
+            double wy[4];
+            wy[0] = __ldg(a.wy_tab + 4 * y); wy[1] = __ldg(a.wy_tab + 4 * y + 1); wy[2] = __ldg(a.wy_tab + 4 * y + 2); wy[3] = __ldg(a.wy_tab + 4 * y + 3);
+            spl_table_entry_w(bc, rc, a.ny, a.nx, __ldg(a.j0_tab + y), wy, i0_first + ii, table + (size_t)e * SPL_ENT);
         }
         float wx[4][4];
         int ent_off[4];
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-            const int i0 = spl_cell_of(min(xt + q, W - 1), a.mw);
-            spl_x_weights(xt + q, a.mw, i0, wx[q]);
-            ent_off[q] = (i0 - i0_first) * SPL_ENT;
+            const int xq = min(xt + q, W - 1);
+            const float4 wv = __ldg(reinterpret_cast<const float4 *>(a.wx_tab) + xq);
+            wx[q][0] = wv.x; wx[q][1] = wv.y; wx[q][2] = wv.z; wx[q][3] = wv.w;
+            ent_off[q] = (__ldg(a.i0_tab + xq) - i0_first) * SPL_ENT;
         }
+        K4_T(11);
         __syncthreads();
+        K4_T(12);
         auto eval4 = [&](const float4 &px, int y, float o_sub[4], float o_bkg[4], float o_rms[4]) -> uint32_t {
             const float *trow = table + (size_t)(y - ry0) * row_stride;
             const float in[4] = {px.x, px.y, px.z, px.w};
@@ -306,6 +342,7 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
                 asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
                              : "=r"(done) : "r"(bar) : "memory");
         }
+        K4_T(13);
         const float4 *tile4 = reinterpret_cast<const float4 *>(lab);
 #pragma unroll 2
         for (int k = 0; k < TH / 8; ++k) {
@@ -324,6 +361,7 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
             }
             put_bits(nib, row + 1);
         }
+        K4_T(14);
         if (warp < 2) {   // halo rows: bits only
             uint32_t nib = 0;
             if (hrow_ok) {
@@ -335,9 +373,10 @@ __global__ void __launch_bounds__(K4_NT, 4) k4a_tile_label(const __grid_constant
         if (tid < 2 * BROWS) {   // halo columns: one pixel each
             uint32_t bit = 0;
             if (hcol_ok) {
-                const int i0 = spl_cell_of(hcx, a.mw);
-                float wxc[4], o_s, o_b, o_r;
-                spl_x_weights(hcx, a.mw, i0, wxc);
+                const int i0 = __ldg(a.i0_tab + hcx);
+                const float4 wv = __ldg(reinterpret_cast<const float4 *>(a.wx_tab) + hcx);
+                const float wxc[4] = {wv.x, wv.y, wv.z, wv.w};
+                float o_s, o_b, o_r;
                 const float *t = table + (size_t)(hcy - ry0) * row_stride + (i0 - i0_first) * SPL_ENT;
                 bit = spl_pixel(*reinterpret_cast<const float4 *>(t), *reinterpret_cast<const float4 *>(t + 4), t[8], wxc, pixc, a.k_d,
                                 o_s, o_b, o_r) ? 1u : 0u;
@@ -988,6 +1027,9 @@ int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_
         a.uniform = fz->mw % 8 == 0 ? 1 : 0;
         a.k_d = (float)detect_k;
         a.sub = fz->sub;
+        a.wx_tab = w.wx_tab; a.wy_tab = w.wy_tab; a.i0_tab = w.i0_tab; a.j0_tab = w.j0_tab;
+        const int nt_tabs = W > H ? W : H;
+        k_spline_tabs<<<(nt_tabs + 255) / 256, 256, 0, st>>>(H, W, fz->mh, fz->mw, w.wx_tab, w.wy_tab, w.i0_tab, w.j0_tab);
     }
     a.use_tma = (W >= TW && H >= TH && ctx->encode_tiled) ? 1 : 0;
     CUtensorMap tmap;
