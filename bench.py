@@ -1,14 +1,18 @@
 #!/usr/bin/env python
 """bench.py -- background + detection throughput on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--unfused] [--impl reference]
 
-One "step" = one pass of the whole hot path (bkg_estimate -> bkg_subtract -> detect_sources, steps a1..a5)
-over one synthetic frame batch of the chosen BASELINE.json config (default: config 3, the 9216x9232 frame the
-metric's targets are quoted on).  `value` is Mpix/s with the frame resident in HBM; `e2e` is the same metric
-through bd_run_host with HOST buffers (H2D of the frame and D2H of the catalogue inside the timed region).
-`roofline` is for the dominant kernel (K3, the fused interpolate/subtract/threshold pass): algorithmic bytes
-(17 B/px) / its CUDA-event duration, against MEASURED_PEAKS.json's HBM copy bandwidth.
+One "step" = one pass of the whole hot path (steps a1..a5) over one synthetic frame batch of the chosen
+BASELINE.json config (default: config 3, the 9216x9232 frame the metric's targets are quoted on), through the C ABI:
+bkg_estimate -> bkg_subtract_detect (the fused a3+a4+a5 call; --unfused times bkg_subtract -> detect_sources).
+`value` is Mpix/s with the frame resident in HBM; `e2e` is the same metric through bd_run_host with HOST buffers
+(H2D of the frame and D2H of the catalogue inside the timed region).
+`roofline` is for the dominant kernel, the fused tile kernel k4a_tile_label<fused> (pass a3 + pass a4 + the partial
+sums of a5): algorithmic bytes 22 B/px (17 + 5) / its duration, taken with CUDA events that the
+library records on the launching stream right before and after that kernel (outside the timed steps, same inputs),
+against MEASURED_PEAKS.json's HBM copy bandwidth.  `roofline_k3_pass` is the stand-alone K3 pass (bkg_subtract),
+the "fused interpolate/subtract/threshold pass" BASELINE.json's 70 % target names.
 With N > 1 (torchrun) every rank processes its own frame (frames are independent units: no data-path
 collective); value = all ranks' pixels / max-over-ranks time.
 `--impl reference` times the CPU oracle, as it stands, on a bounded crop of the same workload.
@@ -36,8 +40,9 @@ TILE_BYTES_PER_PX = 22.0        # fused tile kernel = pass a3 (17) + pass a4 (ma
 CHAIN_BYTES_PER_PX = 30.0       # K1 4 + K3 17 + K4 5 + K5 4
 LAUNCHES_PER_STEP = 9           # K1, K2a, K2b, then bkg_subtract_detect: k4a (fused), k4b, k5m, k5k, k5s, k5f (+2 memsets, not counted)
 LAUNCHES_PER_STEP_UNFUSED = 10  # ... K3, then detect_sources: k4a, k4b, k5m, k5k, k5s, k5f
-TILE_TRAFFIC_NCU = None         # dram__bytes_read.sum + dram__bytes_write.sum of the fused tile kernel on config 3 (profiles/)
-K3_TRAFFIC_NCU = None           # same for k3_interp_subtract
+TILE_TRAFFIC_NCU = 1.8018e9     # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused tile kernel on config 3
+                                # (351.2 MB + 1450.6 MB, profiles/r1_c_fused.md; algorithmic 22 B/px = 1.872 GB)
+K3_TRAFFIC_NCU = 1.3888e9       # same for k3_interp_subtract (340.4 MB + 1048.4 MB; algorithmic 17 B/px = 1.446 GB)
 FALLBACK_HBM_GBS = 6650.0       # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 
 
