@@ -142,6 +142,7 @@ def main():
 
     import torch
     import paper_2502_10783_b200 as bd
+    from paper_2502_10783_b200 import shard
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
@@ -153,7 +154,7 @@ def main():
 
     # ---- workload: each rank its own frame batch (seed offset by rank) -------------------------------
     from dataclasses import replace
-    my_cfg = replace(cfg, seed=cfg.seed + 7919 * rank) if rank else cfg
+    my_cfg = replace(cfg, seed=shard.rank_seed(cfg.seed, rank)) if rank else cfg
     img_h = make_frames(my_cfg)
     B, H, W = img_h.shape
     npx = B * H * W
@@ -230,12 +231,9 @@ def main():
     torch.cuda.synchronize()
     unfused_ms = [float(np.mean([e[i].elapsed_time(e[i + 1]) for e in ev_u])) for i in range(3)]
     n_src = int(o5["n_sources"].sum().item())
-    if dist:
-        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = shard.max_over_ranks(total_ms, dist, dev)
     ms_per_step = total_ms / args.steps
-    value = world * npx / (ms_per_step * 1e-3) / 1e6
+    value = shard.whole_job_value(shard.sum_over_ranks(npx, dist, dev), ms_per_step * 1e-3) / 1e6
 
     # ---- end to end through bd_run_host: pinned host frame in, catalogue out, every step -------------
     e2e = None
@@ -252,10 +250,7 @@ def main():
             recs, nn = bd.run_host(ctx, host_img, p, cfg.detect_k, cfg.min_area, cap, cat=cat_h)
         torch.cuda.synchronize()
         dt = (time.perf_counter() - t0) / n_e2e
-        if dist:
-            t = torch.tensor([dt], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = shard.max_over_ranks(dt, dist, dev)
         e2e = {"value": world * npx / dt / 1e6, "unit": "Mpix/s", "h2d_bytes_per_step": int(npx * 4),
                "d2h_bytes_per_step": int(len(recs) * bd.SOURCE_DTYPE.itemsize + B * 8), "ms_per_step": dt * 1e3,
                "api": "bd_run_host (pinned host frame -> catalogue on host)"}
