@@ -42,8 +42,11 @@ constexpr int K1_T1 = 512;         // slow path: stop refining when the target b
 constexpr int K1_LISTCAP = 4096;   // candidate window capacity (team total) with >= 512 threads; 2048 with 256
 constexpr int K1_MAXWARPS = 16;
 constexpr int K1_MAXC = 8;
-constexpr int K1_FAST_MIN_PX = 8192;   // below this the fixed costs of the fast path exceed the sweeps it saves
-                                       // (and the dead slab must hold the 12 KiB of sort arrays)
+#ifndef K1_FAST_MIN
+#define K1_FAST_MIN 4096
+#endif
+constexpr int K1_FAST_MIN_PX = K1_FAST_MIN;   // smallest mesh for the fast path (measured: 64x64 meshes gain 25 % from it;
+                                       // the dead slab of a 64x64 mesh, 16 KiB, exactly holds the sort arrays)
 
 __device__ unsigned long long g_k1_slow_meshes;   // diagnostic: meshes that took the slow path
 __device__ unsigned long long g_k1_reason[8];     // diagnostic: why (1 sample, 2 tails, 3 rank/bin, 4 window, 5 round window, 6 bound)
@@ -941,9 +944,13 @@ static size_t k1_rowwalk_per_thread(int mesh_h, int mesh_w, int threads) {
 }
 
 int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan) {
-    const size_t soft = 64 * 1024;
+#ifndef K1_SOFT_KB
+#define K1_SOFT_KB 48
+#endif
+    const size_t soft = K1_SOFT_KB * 1024;
     plan->stream = 0;
-    // (1) The mesh fits one CTA's slab (<= 64 KiB): slab mode, one TMA load, every sweep in shared memory.
+    // (1) The mesh fits one CTA's slab (<= 48 KiB; a 64 KiB slab leaves room for one CTA per SM only and was 30 % slower
+    //     than stream mode on 128x128 meshes): slab mode, one TMA load, every sweep in shared memory.
     // (2) Larger meshes with mesh_w % 4 == 0: stream mode -- one CTA per mesh, no slab; the two sweeps of the fast
     //     path read global memory (the second one from L2) with 8 x 128-bit loads in flight per thread.  (The first
     //     version gave such a mesh to a cluster of 4 CTAs with DSMEM exchanges: 570 us on config 3, two thirds of
