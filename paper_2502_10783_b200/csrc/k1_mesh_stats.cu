@@ -91,6 +91,13 @@ struct Smem {   // fixed-size part of shared memory; follows the slab
     // the work area follows: sample keys -> per-thread byte histograms -> tail pixels
 };
 
+// bytes of Smem in use: with fewer than 512 threads only the first 2048 entries of list[] (the last member) are used, and
+// the work area starts right after them
+__host__ __device__ inline size_t k1_smem_fixed_bytes(int threads) {
+    const size_t cut = threads >= 512 ? 0 : (size_t)(K1_LISTCAP - 2048) * sizeof(uint32_t);
+    return (sizeof(Smem) - cut + 127) & ~(size_t)127;
+}
+
 template <int C>
 struct Team {
     __device__ static void sync() {
@@ -572,7 +579,7 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
     float *slab = reinterpret_cast<float *>(smem_raw);   // [slab_rows * mw], 128-B aligned for TMA
     const size_t slab_bytes = (size_t)a.slab_bytes;
     Smem &s = *reinterpret_cast<Smem *>(smem_raw + slab_bytes);
-    unsigned char *area = smem_raw + slab_bytes + ((sizeof(Smem) + 127) & ~(size_t)127);
+    unsigned char *area = smem_raw + slab_bytes + k1_smem_fixed_bytes((int)blockDim.x);
     uint8_t *hist8 = area;                                  // [K1_NBIN][nt] byte counters
     uint32_t *samp = reinterpret_cast<uint32_t *>(area);    // sample keys (before the histogram)
     float *tail = reinterpret_cast<float *>(area);          // tail pixels (after the histogram)
@@ -931,8 +938,10 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
 
 // ---- host side ------------------------------------------------------------------------------------------
 static size_t k1_smem_bytes(int slab_rows, int mw, int threads) {
-    size_t area = (size_t)K1_NBIN * threads;   // byte histograms; also holds the sample (<= 4 KiB) and the tails
-    return bd_align_up((size_t)slab_rows * mw * sizeof(float), 128) + bd_align_up(sizeof(Smem), 128) + area + 128;
+    size_t area = (size_t)K1_NBIN * threads;   // byte histograms; also holds the sample (<= 4 KiB) and the tails,
+    const size_t sort_bytes = 2 * (size_t)(threads >= 512 ? K1_LISTCAP : 2048) * sizeof(uint32_t);
+    if (area < sort_bytes) area = sort_bytes;   // and the general path's sort arrays
+    return bd_align_up((size_t)slab_rows * mw * sizeof(float), 128) + k1_smem_fixed_bytes(threads) + area + 128;
 }
 
 // what one thread of a lone CTA sees of the whole mesh when it walks it row by row in global memory (slow path)
@@ -965,7 +974,7 @@ int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan) {
             if (walk > per_thread) per_thread = walk;
             const size_t slab_bytes = bd_align_up(2 * K1_LISTCAP * sizeof(uint32_t), 128);   // sort arrays
             const size_t area = 56 * 1024;   // byte histograms (32 KiB), then up to 14336 tail pixels
-            const size_t smem = slab_bytes + bd_align_up(sizeof(Smem), 128) + area + 128;
+            const size_t smem = slab_bytes + k1_smem_fixed_bytes(threads) + area + 128;
             if (per_thread <= 255 && smem <= ctx->smem_optin) {
                 plan->cluster = 1;
                 plan->slab_rows = mesh_h;
@@ -984,7 +993,10 @@ int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan) {
             int rows = (mesh_h + c - 1) / c;
             size_t px = (size_t)rows * mesh_w;
             size_t slab = px * sizeof(float);
-            int threads = px >= 16384 ? 512 : 256;
+#ifndef K1_SMALL_NT
+#define K1_SMALL_NT 128
+#endif
+            int threads = px >= 16384 ? 512 : (px > 4096 ? 256 : K1_SMALL_NT);   // small meshes: more, smaller CTAs per SM
             size_t smem = k1_smem_bytes(rows, mesh_w, threads);
             bool ok = pass == 0 ? slab <= soft : true;
             // byte counters: what one thread can see of (a) its slab, (b) the whole mesh read from global
