@@ -48,6 +48,12 @@ constexpr int K1_MAXC = 8;
 constexpr int K1_FAST_MIN_PX = K1_FAST_MIN;   // smallest mesh for the fast path (measured: 64x64 meshes gain 25 % from it;
                                        // the dead slab of a 64x64 mesh, 16 KiB, exactly holds the sort arrays)
 
+#ifdef K1_TIMING
+__device__ unsigned long long g_k1_t[16];
+#define K1_T(i) do { if (tid == 0) { const long long t_ = clock64(); atomicAdd(&g_k1_t[i], (unsigned long long)(t_ - t_prev)); t_prev = t_; } } while (0)
+#else
+#define K1_T(i) do { } while (0)
+#endif
 __device__ unsigned long long g_k1_slow_meshes;   // diagnostic: meshes that took the slow path
 __device__ unsigned long long g_k1_reason[8];     // diagnostic: why (1 sample, 2 tails, 3 rank/bin, 4 window, 5 round window, 6 bound)
 
@@ -297,10 +303,11 @@ __device__ void grow_window(Smem &s, const uint32_t *cnt, int nb, uint32_t b, ui
 // by key, shared-memory atomics on m <= 2048 elements only, then an insertion sort inside the (tiny) bins that
 // hold more than one key.  fcur is scratch [K1_FB].
 #ifndef K1_FB_DIV
-#define K1_FB_DIV 4
+#define K1_FB_DIV 1
 #endif
-// fine bins of the counting sort: listcap / K1_FB_DIV are used (more bins made tie-heavy integer frames 1.8x
-// slower and changed nothing on continuous data: measured on configs 2 and 3)
+// fine bins of the counting sort: listcap / K1_FB_DIV are used.  The per-bin insertion sort (one thread per bin) was
+// 15 k cycles per mesh with 4-6 keys per bin; with as many bins as candidates it is ~1.4 keys per bin on continuous
+// data, and bins of equal keys (integer-valued frames) are skipped
 struct SortArea {   // carved from a dead region of shared memory: 2 * listcap words
     uint32_t *sorted;   // [listcap]
     uint32_t *fcur;     // [listcap]
@@ -314,13 +321,21 @@ __device__ __forceinline__ SortArea make_sort_area(void *base) {
 }
 __device__ void sort_candidates(Smem &s, const uint32_t *list, uint32_t m, uint32_t kga, uint32_t gspan, const SortArea &srt) {
     const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31;
+#ifdef K1_TIMING
+    long long c_ = clock64();
+#define K1_TS(i) do { if (tid == 0) { const long long t_ = clock64(); atomicAdd(&g_k1_t[i], (unsigned long long)(t_ - c_)); c_ = t_; } } while (0)
+#else
+#define K1_TS(i) do { } while (0)
+#endif
     int fshift = 0;
     while ((gspan >> fshift) >= k1_listcap() / K1_FB_DIV) ++fshift;
     const int nfb = (int)(gspan >> fshift) + 1;
     for (int i = tid; i < nfb; i += nt) srt.fcur[i] = 0;
     __syncthreads();
+    K1_TS(11);
     for (uint32_t i = tid; i < m; i += nt) atomicAdd(&srt.fcur[(list[i] - kga) >> fshift], 1u);
     __syncthreads();
+    K1_TS(12);
     {   // exclusive scan of fcur[0..nfb), in place
         const int per = (nfb + nt - 1) / nt, f0 = tid * per;
         uint32_t local = 0;
@@ -343,14 +358,22 @@ __device__ void sort_candidates(Smem &s, const uint32_t *list, uint32_t m, uint3
         }
     }
     __syncthreads();
+    K1_TS(13);
     for (uint32_t i = tid; i < m; i += nt) {
         const uint32_t k = list[i];
         srt.sorted[atomicAdd(&srt.fcur[(k - kga) >> fshift], 1u)] = k;
     }
     __syncthreads();
+    K1_TS(14);
     if (fshift > 0) {   // fcur[f] is now the end of bin f = the start of bin f + 1
         for (int f = tid; f < nfb; f += nt) {
             const uint32_t lo = f ? srt.fcur[f - 1] : 0u, hi = srt.fcur[f];
+            if (hi - lo < 2) continue;
+            if (hi - lo > 4) {   // a bin of equal keys (integer-valued frames: hundreds of copies) needs no sorting
+                uint32_t kmin = 0xFFFFFFFFu, kmax = 0;
+                for (uint32_t i = lo; i < hi; ++i) { const uint32_t k = srt.sorted[i]; kmin = min(kmin, k); kmax = max(kmax, k); }
+                if (kmin == kmax) continue;
+            }
             for (uint32_t i = lo + 1; i < hi; ++i) {
                 const uint32_t k = srt.sorted[i];
                 uint32_t j = i;
@@ -360,6 +383,7 @@ __device__ void sort_candidates(Smem &s, const uint32_t *list, uint32_t m, uint3
         }
         __syncthreads();
     }
+    K1_TS(15);
 }
 
 // ---- pixel source of the slow path: the slab in shared memory (C = 1) or the mesh in global memory ---------
@@ -596,6 +620,9 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
     const int n_tot = vh * vw;
     const float *mesh_ptr = a.img + (size_t)frame * a.H * a.W + (size_t)y0 * a.W + x0;
     const int tid = threadIdx.x, nt = blockDim.x;
+#ifdef K1_TIMING
+    long long t_prev = clock64();
+#endif
 
     // ---- stage the slab ---------------------------------------------------------------------------------
     const bool stream = C == 1 && a.stream;
@@ -626,7 +653,9 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
             samp[e] = f32_to_key(__ldg(mesh_ptr + (size_t)y * a.W + x));
         }
         __syncthreads();
+        K1_T(0);
         bitonic_sort(samp, M_S);
+        K1_T(1);
     }
     // sample quantiles, averaged over the team -> pivot, core interval [A, B], median bracket [ka, kb]
     double pivot = 0.0;
@@ -670,6 +699,7 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
     }
     __syncthreads();   // the sample is dead: the work area becomes the byte histogram
 
+    K1_T(2);
     if (tma) {
         uint32_t bar = smem_u32(&s.mbar), done = 0;
         while (!done) {
@@ -747,6 +777,7 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
         int c_core = 0, c_tail = 0;
         uint32_t below = 0;
         uint8_t *col = hist8 + tid;
+        K1_T(3);
         const uint32_t col_s = smem_u32(col);
         K1_SWEEP_ANY({
             const uint32_t k = f32_to_key(e);
@@ -767,7 +798,9 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
             block_reduce_stats(s, t1, t2, c_core, ct);
             if (tid == 0) { s.xch.s1 = t1; s.xch.s2 = t2; s.xch.n_core = c_core; s.xch.n_tail = ct; s.xch.below = below; }
         }
+        K1_T(4);
         Team<C>::sync();   // #1: every CTA's xch is published
+        K1_T(5);
         if (tid == 0) {
             double q1 = 0, q2 = 0;
             int nc = 0, ntl = 0;
@@ -814,6 +847,7 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
             uint32_t packed_tot;
             const uint32_t packed = block_scan_excl(s, mycnt | ((uint32_t)c_tail << 16), packed_tot);
             uint32_t pos_c = packed & 0xFFFFu, pos_t = packed >> 16;   // (the scan's barriers: histogram is dead)
+            K1_T(6);
             uint32_t addr_c = smem_u32(&s.list[pos_c]), addr_t = smem_u32(&tail[pos_t]);
             K1_SWEEP_ANY({
                 k1_push_u32_if_le(addr_c, f32_to_key(e) - kga, gspan, f32_to_key(e));
@@ -821,6 +855,7 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
             })
             if (tid == 0) { s.xch.m_cand = packed_tot & 0xFFFFu; s.xch.m_tail = packed_tot >> 16; }
         }
+        K1_T(7);
         Team<C>::sync();   // #2: lists published (or: everybody is done reading the peers' xch)
         if (!ok) {
             fast = false;
@@ -845,7 +880,9 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
             __syncthreads();
             const SortArea srt = make_sort_area(slab);   // the slab is dead from here on
             slab_dirty = true;
+            K1_T(8);
             sort_candidates(s, s.list, m_tot, kga, gspan, srt);
+            K1_T(9);
             // ---- clipping rounds on the tail list --------------------------------------------------------
             const double A_d = (double)A_f, B_d = (double)B_f;
             auto tail_stats = [&](double lo, double hi, double &q1, double &q2, int &c_in, int &c_below) {
@@ -920,6 +957,7 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
         k1_slow_path(src, s, hist8, n_tot, a.k_c, a.iters, med, mu, sd, n_final);
     }
 
+    K1_T(10);
     if (tid == 0) {
         double bkg = a.median_factor * med - a.mean_factor * mu;
         if (a.skew_guard) {
@@ -1100,3 +1138,12 @@ extern "C" int bd_debug_k1_force_slow(bd_ctx *ctx, int on) {
     ctx->k1_force_slow = on ? 1 : 0;
     return BD_OK;
 }
+
+#ifdef K1_TIMING
+extern "C" int bd_debug_k1_timing(unsigned long long *out16, int reset) {
+    unsigned long long z[16] = {0};
+    if (cudaMemcpyFromSymbol(out16, g_k1_t, sizeof(z)) != cudaSuccess) return BD_ECUDA;
+    if (reset && cudaMemcpyToSymbol(g_k1_t, z, sizeof(z)) != cudaSuccess) return BD_ECUDA;
+    return BD_OK;
+}
+#endif
