@@ -330,6 +330,39 @@ def test_fused_subtract_detect_equals_two_passes(bd, ctx, cid, H, W, B, mesh):
     assert f2["bkg"] is None and torch.equal(f2["labels"], det["labels"]) and torch.equal(f2["sub"], o["sub"])
 
 
+@pytest.mark.parametrize("H,W,B,mesh", [(97, 132, 2, 36), (130, 260, 1, 64), (64, 128, 3, 64), (200, 516, 1, 128)])
+def test_no_writes_outside_the_outputs(bd, ctx, H, W, B, mesh):
+    """Guard bands around every output buffer of both detection paths stay untouched (ragged tiles, frame edges, TMA
+    label-tile stores clipped at the frame edge)."""
+    cfg = CONFIGS[1]
+    img = make_frames(cfg, H=H, W=W, B=B)
+    p = params_for(bd, cfg, mesh_h=mesh, mesh_w=mesh)
+    d_img = dev(img)
+    bm, rm, cb, cr = bd.bkg_estimate(ctx, d_img, p)
+    G, P, cap = 4096, B * H * W, 512
+    def guarded(dtype, n, fill):
+        flat = torch.full((n + 2 * G,), fill, dtype=dtype, device="cuda")
+        return flat, flat[G:G + n]
+    for fused in (True, False):
+        bufs = {k: guarded(torch.float32, P, -777.0) for k in ("sub", "bkg", "rms")}
+        bufs["mask"] = guarded(torch.uint8, P, 0xAB)
+        bufs["labels"] = guarded(torch.int32, P, -5)
+        bufs["cat"] = guarded(torch.uint8, cap * bd.SOURCE_DTYPE.itemsize, 0xCD)
+        bufs["n_sources"] = guarded(torch.int64, B, -9)
+        out = {k: (v[1].view(B, H, W) if k in ("sub", "bkg", "rms", "mask", "labels") else v[1]) for k, v in bufs.items()}
+        if fused:
+            bd.bkg_subtract_detect(ctx, d_img, p.mesh_h, p.mesh_w, cb, cr, cfg.detect_k, cfg.min_area, cap, out=out)
+        else:
+            bd.bkg_subtract(ctx, d_img, p.mesh_h, p.mesh_w, cb, cr, cfg.detect_k, out=out)
+            bd.detect_sources(ctx, out["sub"], out["rms"], out["mask"], cfg.detect_k, cfg.min_area, cap, out=out)
+        torch.cuda.synchronize()
+        for k, (flat, view) in bufs.items():
+            n = view.numel()
+            fill = flat[0].item()
+            assert bool((flat[:G] == fill).all()) and bool((flat[G + n:] == fill).all()), f"{k}: guard band overwritten (fused={fused})"
+        assert int(out["labels"].min()) >= 0 and int(out["n_sources"].min()) >= 0
+
+
 def test_chain_constant_frame(bd, ctx):
     img = np.full((1, 256, 320), 4321.0, dtype=np.float32)
     p = bd.BkgParams()
