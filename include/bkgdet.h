@@ -64,6 +64,25 @@ typedef struct {
     double x2, y2, xy;                  /* central second moments  sum(I*(x-xc)^2)/sum(I) ... */
 } bd_source;
 
+/* Parameters of aperture / auto photometry (readings A23-A27; the paper, names the methods only). */
+typedef struct {
+    double r_aper;            /* radius of the circular aperture in pixels; default 5.0                        A23 */
+    double kron_factor;       /* auto aperture = kron_factor * first-moment radius; default 2.5               A25 */
+    double kron_min_radius;   /* lower limit of the auto radius, in units of the object's 1-sigma ellipse; 3.5    */
+    double kron_search;       /* the first-moment radius is measured inside this many sigma; default 6.0          */
+    int32_t subpix;           /* sub-pixel samples per axis for the pixels on the aperture's rim; default 5    A23 */
+    int32_t pad;
+} bd_phot_params;
+
+/* One photometry record per catalogue record (same index).  56 bytes. */
+typedef struct {
+    double flux_aper, fluxerr_aper, area_aper;   /* sum w*sub, sqrt(sum w*rms^2), sum w over the circular aperture */
+    double kron_radius;                          /* in units of the 1-sigma ellipse of the second moments          */
+    double flux_auto, fluxerr_auto;              /* sum sub, sqrt(sum rms^2) over the ellipse of kron_radius       */
+    int32_t npix_auto;                           /* pixels in that ellipse                                          */
+    int32_t flags;                               /* bit 0: aperture cut by the frame edge; bit 1: an ellipse's box is */
+} bd_phot;
+
 /* ---- context ------------------------------------------------------------------------------------ */
 int bd_create(bd_ctx **ctx, int device);   /* binds to CUDA device `device`; returns BD_ECUDA if none */
 void bd_destroy(bd_ctx *ctx);
@@ -146,6 +165,20 @@ int bkg_subtract_detect(bd_ctx *ctx, const float *d_img, int B, int H, int W, in
                         float *d_sub, float *d_bkg, float *d_rms, uint8_t *d_mask, int32_t *d_labels,
                         bd_source *d_cat, int64_t cat_capacity, int64_t *d_n_sources, void *d_ws, size_t ws_bytes,
                         void *cuda_stream);
+
+/* ---- photometry = SURVEY 8(f) NEXT-2: aperture and auto (Kron-like) photometry of every catalogue record (kernel K6).
+ * PAPER.md:159 (aperture, isophotal and auto photometry, one object per thread; isophotal = bd_source.flux).
+ * d_sub, d_rms: float32 [B,H,W] maps of bkg_subtract; d_cat / d_n_sources: the outputs of detect_sources (records in
+ * catalogue order, per-frame counts on the device); the first min(sum n_sources, cat_capacity) records are measured and
+ * d_phot[i] belongs to d_cat[i].  Aperture: circle of r_aper about the centroid, rim pixels weighted by the fraction of
+ * their subpix^2 sub-pixel centres inside (A23).  Auto: ellipse of the second moments (A24; 1/12 added to x2, y2 of
+ * degenerate objects), first-moment radius r1 = sum r*sub / sum sub inside kron_search sigma, kron_radius =
+ * max(kron_factor*r1, kron_min_radius) (A25), flux inside that ellipse with a hard edge (A26).  No neighbour masking
+ * (A27).  Deterministic (fixed summation order).  Pixels outside the frame contribute nothing (flags). */
+void bd_default_phot_params(bd_phot_params *p);
+int photometry(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H, int W, const bd_source *d_cat,
+               const int64_t *d_n_sources, int64_t cat_capacity, const bd_phot_params *p, bd_phot *d_phot,
+               void *cuda_stream);
 
 /* ---- whole chain from HOST buffers (pinned or pageable), synchronous. ----------------------------------
  * Copies h_img to the device, runs bkg_estimate -> bkg_subtract_detect, copies the

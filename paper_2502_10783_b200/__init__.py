@@ -16,11 +16,12 @@ import torch
 from . import _build
 
 __all__ = ["BkgParams", "Context", "SOURCE_DTYPE", "bkg_estimate", "bkg_subtract", "detect_sources", "mesh_stats",
-           "grid_filter_spline", "bkg_subtract_detect", "run_host", "grid_shape", "load_library", "EXPORTS"]
+           "grid_filter_spline", "bkg_subtract_detect", "photometry", "PhotParams", "PHOT_DTYPE", "run_host", "grid_shape", "load_library", "EXPORTS"]
 
 EXPORTS = ["bd_create", "bd_destroy", "bd_last_error", "bd_default_bkg_params", "bd_grid_shape",
            "bd_bkg_workspace_bytes", "bd_detect_workspace_bytes", "bd_mesh_stats", "bd_grid_filter_spline",
-           "bkg_estimate", "bkg_subtract", "detect_sources", "bkg_subtract_detect", "bd_run_host"]
+           "bkg_estimate", "bkg_subtract", "detect_sources", "bkg_subtract_detect", "bd_default_phot_params", "photometry",
+           "bd_run_host"]
 
 
 class _CParams(C.Structure):
@@ -248,6 +249,49 @@ def bkg_subtract_detect(ctx: Context, img: torch.Tensor, mesh_h: int, mesh_w: in
                                           _ptr(mask), _ptr(labels), _ptr(cat), C.c_int64(cat_capacity), _ptr(nsrc),
                                           _ptr(ws), C.c_size_t(ws.numel()), _stream()))
     return dict(sub=sub, bkg=bkg, rms=rms, mask=mask, labels=labels, cat=cat, n_sources=nsrc)
+
+
+PHOT_DTYPE = np.dtype([("flux_aper", np.float64), ("fluxerr_aper", np.float64), ("area_aper", np.float64),
+                       ("kron_radius", np.float64), ("flux_auto", np.float64), ("fluxerr_auto", np.float64),
+                       ("npix_auto", np.int32), ("flags", np.int32)], align=True)
+
+
+class _CPhotParams(C.Structure):
+    _fields_ = [("r_aper", C.c_double), ("kron_factor", C.c_double), ("kron_min_radius", C.c_double),
+                ("kron_search", C.c_double), ("subpix", C.c_int32), ("pad", C.c_int32)]
+
+
+class PhotParams:
+    """bd_phot_params (defaults from bd_default_phot_params)."""
+
+    def __init__(self, **kw):
+        c = _CPhotParams()
+        load_library().bd_default_phot_params(C.byref(c))
+        for k, v in kw.items():
+            if not hasattr(c, k):
+                raise TypeError(f"unknown photometry parameter {k}")
+            setattr(c, k, v)
+        self._c = c
+
+    def __getattr__(self, k):
+        return getattr(self._c, k)
+
+
+def photometry(ctx: Context, sub: torch.Tensor, rms: torch.Tensor, cat: torch.Tensor, n_sources: torch.Tensor,
+               cat_capacity: int, p: "PhotParams | None" = None, out: torch.Tensor | None = None) -> torch.Tensor:
+    """NEXT-2 (K6): aperture + auto photometry of the catalogue records.  -> uint8 [cap*56] device bytes (PHOT_DTYPE)."""
+    B, H, W = sub.shape
+    p = p or PhotParams()
+    if out is None:
+        out = torch.zeros(max(cat_capacity, 1) * PHOT_DTYPE.itemsize, dtype=torch.uint8, device=_dev(ctx))
+    ctx.check(ctx.lib.photometry(ctx.h, _ptr(sub), _ptr(rms), B, H, W, _ptr(cat), _ptr(n_sources), C.c_int64(cat_capacity),
+                                 C.byref(p._c), _ptr(out), _stream()))
+    return out
+
+
+def phot_to_numpy(phot: torch.Tensor, n_sources: torch.Tensor, cat_capacity: int) -> np.ndarray:
+    n = int(min(int(n_sources.sum().item()), cat_capacity))
+    return phot[: n * PHOT_DTYPE.itemsize].cpu().numpy().view(PHOT_DTYPE).copy()
 
 
 def catalogue_to_numpy(cat: torch.Tensor, n_sources: torch.Tensor, cat_capacity: int) -> np.ndarray:

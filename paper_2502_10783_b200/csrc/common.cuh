@@ -79,6 +79,9 @@ int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_
                double detect_k, int min_area, int32_t *d_labels, bd_source *d_cat, int64_t cat_capacity,
                int64_t *d_n_sources, void *d_ws, size_t ws_bytes, cudaStream_t st, const K45Fused *fz);
 
+int k6_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H, int W, const bd_source *d_cat,
+              const int64_t *d_n_sources, int64_t cat_capacity, const bd_phot_params *p, bd_phot *d_phot, cudaStream_t st);
+
 // ---- small device helpers ------------------------------------------------------------------------------
 #ifdef __CUDACC__
 __device__ __forceinline__ uint32_t f32_to_key(float f) {   // order-preserving map float32 -> uint32

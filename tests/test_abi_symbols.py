@@ -36,6 +36,7 @@ def test_struct_layouts_match_header():
     import paper_2502_10783_b200 as m
     assert m.SOURCE_DTYPE.itemsize == 88 and m.SOURCE_DTYPE.fields["flux"][1] == 40
     assert ctypes.sizeof(m._CParams) == 48   # 4 x i32, f64, 2 x i32, 2 x f64
+    assert m.PHOT_DTYPE.itemsize == 56 and m.PHOT_DTYPE.fields["npix_auto"][1] == 48 and ctypes.sizeof(m._CPhotParams) == 40
 
 
 def test_no_gpu_no_fallback():

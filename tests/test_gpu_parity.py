@@ -402,6 +402,64 @@ def test_run_host_matches_device_path(bd, ctx):
     assert np.allclose(cat_h["flux"], cat_d["flux"], rtol=1e-12)
 
 
+# ------------------------------------------------------------------------------------------- NEXT-2: photometry (K6)
+from oracle import photometry as oph  # noqa: E402
+
+
+@pytest.mark.parametrize("cid,H,W,B,kw", [(1, 512, 512, 1, {}), (3, 528, 768, 1, dict(r_aper=3.0, subpix=7)),
+                                           (5, 300, 388, 2, dict(r_aper=8.5, kron_min_radius=0.5)),
+                                           (2, 260, 260, 1, dict(r_aper=12.0, kron_factor=2.0, kron_search=4.0, subpix=1))])
+def test_k6_photometry_against_oracle(bd, ctx, cid, H, W, B, kw):
+    """Stage parity: the oracle measures the GPU's own sub / rms maps and catalogue.  Pixel membership (npix_auto, flags)
+    exact; sums to 1e-9 relative (float64 on both sides, only the summation order differs)."""
+    cfg = CONFIGS[cid]
+    img = make_frames(cfg, H=H, W=W, B=B)
+    p = params_for(bd, cfg)
+    cap = 1 << 15
+    bm, rm, o, det = run_chain(bd, ctx, img, p, cfg.detect_k, cfg.min_area, cap)
+    pp = bd.PhotParams(**kw)
+    ph = bd.photometry(ctx, o["sub"], o["rms"], det["cat"], det["n_sources"], cap, pp)
+    ph2 = bd.photometry(ctx, o["sub"], o["rms"], det["cat"], det["n_sources"], cap, pp)
+    torch.cuda.synchronize()
+    assert torch.equal(ph, ph2), "photometry is not bit-reproducible"
+    cat = bd.catalogue_to_numpy(det["cat"], det["n_sources"], cap)
+    got = bd.phot_to_numpy(ph, det["n_sources"], cap)
+    assert len(got) == len(cat) > 0
+    op = oph.PhotParams(r_aper=pp.r_aper, kron_factor=pp.kron_factor, kron_min_radius=pp.kron_min_radius,
+                        kron_search=pp.kron_search, subpix=pp.subpix)
+    for f in range(B):
+        sel = cat["frame"] == f
+        want = oph.photometry(o["sub"][f].cpu().numpy(), o["rms"][f].cpu().numpy(), cat[sel], op)
+        g = got[sel]
+        assert np.array_equal(g["npix_auto"], want["npix_auto"]) and np.array_equal(g["flags"], want["flags"])
+        assert np.allclose(g["kron_radius"], want["kron_radius"], rtol=1e-12, atol=0)
+        for k in ("flux_aper", "fluxerr_aper", "area_aper", "flux_auto", "fluxerr_auto"):
+            assert np.allclose(g[k], want[k], rtol=1e-9, atol=1e-6), f"{k}: worst {np.max(np.abs(g[k] - want[k]))}"
+        assert (want["flags"] != 0).any() or cid == 1          # the reduced frames have sources at their edges
+
+
+def test_k6_isolated_gaussian_and_errors(bd, ctx):
+    """An analytic source through the GPU path alone: encircled energy and the Kron radius of a Gaussian."""
+    H = W = 128
+    yy, xx = np.mgrid[:H, :W].astype(np.float64)
+    F, sig, xc, yc = 2.0e4, 2.0, 63.3, 64.6
+    sub = (F / (2 * np.pi * sig**2) * np.exp(-0.5 * ((xx - xc) ** 2 + (yy - yc) ** 2) / sig**2)).astype(np.float32)[None]
+    rms = np.ones_like(sub)
+    cat = np.zeros(1, dtype=bd.SOURCE_DTYPE)
+    cat["x"], cat["y"], cat["x2"], cat["y2"], cat["xy"] = xc, yc, sig**2, sig**2, 0.0
+    d_cat = torch.from_numpy(cat.view(np.uint8)).cuda(); n = torch.tensor([1], dtype=torch.int64, device="cuda")
+    ph = bd.photometry(ctx, dev(sub), dev(rms), d_cat, n, 4, bd.PhotParams(r_aper=5.0, kron_min_radius=0.1))
+    torch.cuda.synchronize()
+    g = bd.phot_to_numpy(ph, n, 4)[0]
+    assert g["flux_aper"] == pytest.approx(F * (1 - np.exp(-25 / (2 * sig**2))), rel=1.2e-2)
+    assert g["kron_radius"] == pytest.approx(2.5 * np.sqrt(np.pi / 2), rel=2e-2)
+    assert g["flux_auto"] == pytest.approx(F * (1 - np.exp(-0.5 * g["kron_radius"] ** 2)), rel=5e-3) and g["flags"] == 0
+    with pytest.raises(bd.BkgdetError):
+        bd.photometry(ctx, dev(sub), dev(rms), d_cat, n, 4, bd.PhotParams(r_aper=-1.0))
+    with pytest.raises(bd.BkgdetError):
+        bd.photometry(ctx, dev(sub), dev(rms), d_cat, n, 4, bd.PhotParams(subpix=0))
+
+
 # ------------------------------------------------------------------------------------------- errors
 def test_error_codes(bd, ctx):
     img = torch.zeros((1, 64, 66), dtype=torch.float32, device="cuda")     # W % 4 != 0
