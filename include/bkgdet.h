@@ -174,11 +174,14 @@ int bkg_subtract_detect(bd_ctx *ctx, const float *d_img, int B, int H, int W, in
  * their subpix^2 sub-pixel centres inside (A23).  Auto: ellipse of the second moments (A24; 1/12 added to x2, y2 of
  * degenerate objects), first-moment radius r1 = sum r*sub / sum sub inside kron_search sigma, kron_radius =
  * max(kron_factor*r1, kron_min_radius) (A25), flux inside that ellipse with a hard edge (A26).  No neighbour masking
- * (A27).  Deterministic (fixed summation order).  Pixels outside the frame contribute nothing (flags). */
+ * (A27).  Deterministic (fixed summation order).  Pixels outside the frame contribute nothing (flags).
+ * One warp per object; objects whose search ellipse covers more than 4096 pixels are queued in the workspace and
+ * measured by one thread block each.  d_ws / ws_bytes: at least bd_phot_workspace_bytes(cat_capacity). */
 void bd_default_phot_params(bd_phot_params *p);
+int bd_phot_workspace_bytes(const bd_ctx *ctx, int64_t cat_capacity, size_t *bytes);
 int photometry(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H, int W, const bd_source *d_cat,
                const int64_t *d_n_sources, int64_t cat_capacity, const bd_phot_params *p, bd_phot *d_phot,
-               void *cuda_stream);
+               void *d_ws, size_t ws_bytes, void *cuda_stream);
 
 /* ---- whole chain from HOST buffers (pinned or pageable), synchronous. ----------------------------------
  * Copies h_img to the device, runs bkg_estimate -> bkg_subtract_detect, copies the

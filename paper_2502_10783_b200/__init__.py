@@ -20,7 +20,7 @@ __all__ = ["BkgParams", "Context", "SOURCE_DTYPE", "bkg_estimate", "bkg_subtract
 
 EXPORTS = ["bd_create", "bd_destroy", "bd_last_error", "bd_default_bkg_params", "bd_grid_shape",
            "bd_bkg_workspace_bytes", "bd_detect_workspace_bytes", "bd_mesh_stats", "bd_grid_filter_spline",
-           "bkg_estimate", "bkg_subtract", "detect_sources", "bkg_subtract_detect", "bd_default_phot_params", "photometry",
+           "bkg_estimate", "bkg_subtract", "detect_sources", "bkg_subtract_detect", "bd_default_phot_params", "bd_phot_workspace_bytes", "photometry",
            "bd_run_host"]
 
 
@@ -278,14 +278,19 @@ class PhotParams:
 
 
 def photometry(ctx: Context, sub: torch.Tensor, rms: torch.Tensor, cat: torch.Tensor, n_sources: torch.Tensor,
-               cat_capacity: int, p: "PhotParams | None" = None, out: torch.Tensor | None = None) -> torch.Tensor:
+               cat_capacity: int, p: "PhotParams | None" = None, out: torch.Tensor | None = None,
+               ws: torch.Tensor | None = None) -> torch.Tensor:
     """NEXT-2 (K6): aperture + auto photometry of the catalogue records.  -> uint8 [cap*56] device bytes (PHOT_DTYPE)."""
     B, H, W = sub.shape
     p = p or PhotParams()
     if out is None:
         out = torch.zeros(max(cat_capacity, 1) * PHOT_DTYPE.itemsize, dtype=torch.uint8, device=_dev(ctx))
+    if ws is None:
+        nb = C.c_size_t()
+        ctx.check(ctx.lib.bd_phot_workspace_bytes(ctx.h, C.c_int64(cat_capacity), C.byref(nb)))
+        ws = torch.empty(nb.value, dtype=torch.uint8, device=_dev(ctx))
     ctx.check(ctx.lib.photometry(ctx.h, _ptr(sub), _ptr(rms), B, H, W, _ptr(cat), _ptr(n_sources), C.c_int64(cat_capacity),
-                                 C.byref(p._c), _ptr(out), _stream()))
+                                 C.byref(p._c), _ptr(out), _ptr(ws), C.c_size_t(ws.numel()), _stream()))
     return out
 
 

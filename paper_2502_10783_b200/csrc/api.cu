@@ -206,22 +206,29 @@ int bkg_subtract_detect(bd_ctx *ctx, const float *d_img, int B, int H, int W, in
                       ws_bytes, st, &fz);
 }
 
+int bd_phot_workspace_bytes(const bd_ctx *ctx, int64_t cat_capacity, size_t *bytes) {
+    if (!ctx || !bytes || cat_capacity < 0) return BD_EINVAL;
+    *bytes = k6_workspace_bytes(cat_capacity);
+    return BD_OK;
+}
+
 void bd_default_phot_params(bd_phot_params *p) {
     if (!p) return;
     p->r_aper = 5.0; p->kron_factor = 2.5; p->kron_min_radius = 3.5; p->kron_search = 6.0; p->subpix = 5; p->pad = 0;
 }
 
 int photometry(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H, int W, const bd_source *d_cat,
-               const int64_t *d_n_sources, int64_t cat_capacity, const bd_phot_params *p, bd_phot *d_phot, void *cuda_stream) {
+               const int64_t *d_n_sources, int64_t cat_capacity, const bd_phot_params *p, bd_phot *d_phot, void *d_ws,
+               size_t ws_bytes, void *cuda_stream) {
     int rc = check_frame(ctx, B, H, W);
     if (rc) return rc;
-    if (!d_sub || !d_rms || !d_cat || !d_n_sources || !d_phot || !p) return bd_set_error(ctx, BD_EINVAL, "null pointer");
+    if (!d_sub || !d_rms || !d_cat || !d_n_sources || !d_phot || !p || !d_ws) return bd_set_error(ctx, BD_EINVAL, "null pointer");
     if (cat_capacity < 0) return bd_set_error(ctx, BD_EINVAL, "bad catalogue capacity");
     if (!(p->r_aper > 0.0) || !(p->kron_factor > 0.0) || !(p->kron_min_radius > 0.0) || !(p->kron_search > 0.0) || p->subpix < 1 ||
         p->subpix > 16)
         return bd_set_error(ctx, BD_EINVAL, "photometry parameters must be positive, subpix in 1..16");
     if (cat_capacity == 0) return BD_OK;
-    return k6_launch(ctx, d_sub, d_rms, B, H, W, d_cat, d_n_sources, cat_capacity, p, d_phot, (cudaStream_t)cuda_stream);
+    return k6_launch(ctx, d_sub, d_rms, B, H, W, d_cat, d_n_sources, cat_capacity, p, d_phot, d_ws, ws_bytes, (cudaStream_t)cuda_stream);
 }
 
 int bd_run_host(bd_ctx *ctx, const float *h_img, int B, int H, int W, const bd_bkg_params *p, double detect_k,

@@ -80,7 +80,9 @@ int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_
                int64_t *d_n_sources, void *d_ws, size_t ws_bytes, cudaStream_t st, const K45Fused *fz);
 
 int k6_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H, int W, const bd_source *d_cat,
-              const int64_t *d_n_sources, int64_t cat_capacity, const bd_phot_params *p, bd_phot *d_phot, cudaStream_t st);
+              const int64_t *d_n_sources, int64_t cat_capacity, const bd_phot_params *p, bd_phot *d_phot, void *d_ws,
+              size_t ws_bytes, cudaStream_t st);
+size_t k6_workspace_bytes(int64_t cat_capacity);
 
 // ---- small device helpers ------------------------------------------------------------------------------
 #ifdef __CUDACC__

@@ -438,6 +438,41 @@ def test_k6_photometry_against_oracle(bd, ctx, cid, H, W, B, kw):
         assert (want["flags"] != 0).any() or cid == 1          # the reduced frames have sources at their edges
 
 
+def test_k6_large_objects_take_the_block_path(bd, ctx):
+    """Objects whose search ellipse covers more than 4096 px are queued and measured by one thread block each: same
+    membership and sums as the oracle, mixed with small objects, at the frame edge, in the second frame of a batch."""
+    rng = np.random.default_rng(11)
+    B, H, W = 2, 300, 420
+    sub = rng.normal(0, 1, (B, H, W)).astype(np.float32); rms = rng.uniform(0.8, 1.3, (B, H, W)).astype(np.float32)
+    yy, xx = np.mgrid[:H, :W].astype(np.float64)
+    objs = [(0, 150.3, 140.7, 15.0, 9.0, 0.5), (0, 30.2, 25.5, 2.0, 1.5, 0.1), (1, 400.6, 10.2, 20.0, 20.0, 0.0),
+            (1, 200.1, 150.9, 40.0, 3.0, -0.7), (1, 100.0, 250.0, 1.2, 1.2, 0.0), (0, 300.5, 200.5, 11.0, 10.5, 1.2)]
+    cat = np.zeros(len(objs), dtype=bd.SOURCE_DTYPE)
+    objs.sort(key=lambda o: o[0])
+    for i, (f, xc, yc, sx, sy, th) in enumerate(objs):
+        c, s_ = np.cos(th), np.sin(th)
+        u = (xx - xc) * c + (yy - yc) * s_; v = -(xx - xc) * s_ + (yy - yc) * c
+        sub[f] += (5e4 / (2 * np.pi * sx * sy) * np.exp(-0.5 * (u * u / sx**2 + v * v / sy**2))).astype(np.float32)
+        cat[i]["frame"], cat[i]["x"], cat[i]["y"] = f, xc, yc
+        cat[i]["x2"] = sx**2 * c * c + sy**2 * s_ * s_; cat[i]["y2"] = sx**2 * s_ * s_ + sy**2 * c * c
+        cat[i]["xy"] = (sx**2 - sy**2) * s_ * c
+    n = torch.tensor([sum(o[0] == 0 for o in objs), sum(o[0] == 1 for o in objs)], dtype=torch.int64, device="cuda")
+    d_cat = torch.from_numpy(cat.view(np.uint8)).cuda()
+    ph = bd.photometry(ctx, dev(sub), dev(rms), d_cat, n, 16)
+    ph2 = bd.photometry(ctx, dev(sub), dev(rms), d_cat, n, 16)
+    torch.cuda.synchronize()
+    assert torch.equal(ph, ph2)
+    got = bd.phot_to_numpy(ph, n, 16)
+    for f in range(B):
+        sel = cat["frame"] == f
+        want = oph.photometry(sub[f], rms[f], cat[sel], oph.PhotParams())
+        g = got[sel]
+        assert np.array_equal(g["npix_auto"], want["npix_auto"]) and np.array_equal(g["flags"], want["flags"])
+        assert want["npix_auto"].max() > 4096
+        for k in ("flux_aper", "fluxerr_aper", "area_aper", "kron_radius", "flux_auto", "fluxerr_auto"):
+            assert np.allclose(g[k], want[k], rtol=1e-9, atol=1e-6), k
+
+
 def test_k6_isolated_gaussian_and_errors(bd, ctx):
     """An analytic source through the GPU path alone: encircled energy and the Kron radius of a Gaussian."""
     H = W = 128
