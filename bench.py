@@ -38,7 +38,8 @@ METRIC = "Mpix/s background+detection per frame"
 K3_BYTES_PER_PX = 17.0          # img 4 read; sub 4 + bkg 4 + rms 4 + mask 1 written
 TILE_BYTES_PER_PX = 22.0        # fused tile kernel = pass a3 (17) + pass a4 (mask 1 read, labels 4 written)
 CHAIN_BYTES_PER_PX = 30.0       # K1 4 + K3 17 + K4 5 + K5 4
-LAUNCHES_PER_STEP = 9           # K1, K2a, K2b, then bkg_subtract_detect: k4a (fused), k4b, k5m, k5k, k5s, k5f (+2 memsets, not counted)
+LAUNCHES_PER_STEP = 10          # K1, K2a, K2b, then bkg_subtract_detect: k_spline_tabs, k4a (fused), k4b, k5m, k5k, k5s, k5f
+                                # (+2 memsets, not counted)
 LAUNCHES_PER_STEP_UNFUSED = 10  # ... K3, then detect_sources: k4a, k4b, k5m, k5k, k5s, k5f
 TILE_TRAFFIC_NCU = 1.8018e9     # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused tile kernel on config 3
                                 # (351.2 MB + 1450.6 MB, profiles/r1_c_fused.md; algorithmic 22 B/px = 1.872 GB)
