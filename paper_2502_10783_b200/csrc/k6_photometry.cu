@@ -64,13 +64,15 @@ __device__ __forceinline__ bool ellipse_box(const Ellipse &e, double R, int H, i
 }
 __device__ __forceinline__ long long box_area(const Box &b) { return (long long)(b.x_hi - b.x_lo + 1) * (b.y_hi - b.y_lo + 1); }
 // this thread's share (pixels t, t + nt, ... of the box) of  S0 = sum I, S1 = sum r I, V = sum rms^2, N = count  over r <= R
-__device__ __forceinline__ void ellipse_partial(const Ellipse &e, const Box &b, double R, const float *sub, const float *rms, int W,
-                                                int t, int nt, double &S0, double &S1, double &V, int &N) {
-    S0 = 0.0; S1 = 0.0; V = 0.0; N = 0;
-    const int bw = b.x_hi - b.x_lo + 1;
-    const long long n = box_area(b);
-    for (long long k = t; k < n; k += nt) {
-        const int yy = b.y_lo + (int)(k / bw), xx = b.x_lo + (int)(k % bw);
+// (IDX = int for boxes below 2^31 pixels: a 64-bit division per pixel costs more than the rest of the loop body)
+template <typename IDX>
+__device__ __forceinline__ void ellipse_partial_t(const Ellipse &e, const Box &b, double R, const float *sub, const float *rms, int W,
+                                                  int t, int nt, double &S0, double &S1, double &V, int &N) {
+    const IDX bw = (IDX)(b.x_hi - b.x_lo + 1);
+    const IDX n = (IDX)box_area(b);
+    for (IDX k = (IDX)t; k < n; k += (IDX)nt) {
+        const IDX row = k / bw;
+        const int yy = b.y_lo + (int)row, xx = b.x_lo + (int)(k - row * bw);
         const double dx = (double)xx - e.xc, dy = (double)yy - e.yc;
         const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(__dmul_rn(e.cxx, dx), dx), __dmul_rn(__dmul_rn(e.cyy, dy), dy)),
                                     __dmul_rn(__dmul_rn(e.cxy, dx), dy));
@@ -80,6 +82,12 @@ __device__ __forceinline__ void ellipse_partial(const Ellipse &e, const Box &b, 
             S0 += I; S1 += rad * I; V += q * q; ++N;
         }
     }
+}
+__device__ __forceinline__ void ellipse_partial(const Ellipse &e, const Box &b, double R, const float *sub, const float *rms, int W,
+                                                int t, int nt, double &S0, double &S1, double &V, int &N) {
+    S0 = 0.0; S1 = 0.0; V = 0.0; N = 0;
+    if (box_area(b) < 0x7FFF0000ll) ellipse_partial_t<int>(e, b, R, sub, rms, W, t, nt, S0, S1, V, N);
+    else ellipse_partial_t<long long>(e, b, R, sub, rms, W, t, nt, S0, S1, V, N);
 }
 __device__ __forceinline__ double kron_radius_of(const bd_phot_params &p, double S0, double S1) {   // A25
     if (S0 > 0.0 && S1 > 0.0) return fmax(__dmul_rn(p.kron_factor, S1) / S0, p.kron_min_radius);
