@@ -7,24 +7,28 @@
 // tiles and labelling and reduction are ONE pass over the tile (the first version labelled, flattened and then
 // re-read labels and sub twice more: 1.38 ms on 9216x9232; ncu showed the tile kernel instruction-bound on
 // divergent per-pixel loops and the re-read passes latency-bound):
-//   K4a  per tile: mask bytes -> bit rows (+1-pixel halo) in shared memory; a COMPACT list of the tile's
-//        foreground pixels, so every later phase runs dense; union-find on the list (parent = start of the
-//        horizontal run, vertical/diagonal links with the usual pruning, union by minimum index); per-component
-//        pixel counts; components that can matter (count >= min_area, or touching a foreground pixel of
-//        another tile) get partial sums (npix, flux, first/second moments about the tile-local root, peak,
-//        bbox) reduced in shared memory with warp-segmented shuffles, and are written as one 96-byte record
-//        each; the label tile (1 + raster index of the tile-local root, 0 = background) is assembled in
-//        shared memory and leaves with one TMA bulk-tensor store; the tile's border bit rows/columns are
-//        exported (48 B per tile).
+//   K4a  per tile (256 threads, one per 32-pixel bit word): mask bytes -> bit rows (+1-pixel halo) in shared memory --
+//        or, in FUSED mode (bkg_subtract_detect), the spline evaluation of step a3 itself: the image tile arrives by one
+//        TMA load into the label buffer, sub / bkg / rms are written out and the threshold bits go straight into the bit
+//        rows; pixels without any foreground neighbour are complete components (labelled on the spot, dropped when
+//        min_area > 1); a COMPACT list of the other foreground pixels, so every later phase runs dense; union-find on
+//        the list (parent = start of the horizontal run, vertical/diagonal links with the usual pruning, union by
+//        minimum index); per-component pixel counts; components that can matter (count >= min_area, or touching a
+//        foreground pixel of another tile) get a 96-byte record in a contiguous range the tile reserves with one atomic;
+//        partial sums (npix, flux, first/second moments about the tile-local root, peak, bbox) are reduced over the
+//        list entries of one (component, row) with a segmented shuffle reduction and added to the record with RED
+//        atomics; the label tile (1 + raster index of the tile-local root, 0 = background) is assembled in shared memory
+//        and leaves with one TMA bulk-tensor store; the tile's border bit rows/columns are exported (48 B per tile).
 //   K4b  seam merge from the exported border bits alone: only real cross-tile links touch the label array
 //        (union by atomicMin on the root's label word).
 //   K5m  for every record whose tile-local root is no longer a root: add it to the final root's record
 //        (float64 atomics, moments shifted to the new origin) and relabel the pixels of its bounding box.
 //   K5k  records that are final roots with npix >= min_area set their bit in a per-pixel bitmap and count into
-//        1024-pixel blocks;  K5s scans the block counts;  K5f ranks every kept root (= catalogue slot in
+//        4096-pixel blocks;  K5s scans the block counts;  K5f ranks every kept root (= catalogue slot in
 //        ascending (frame, label) order) and writes its record.
-// Records live in a direct-mapped table indexed by the 2x2-pixel block of the root (two roots can never share
-// one: they would be 8-adjacent), so no allocation can overflow; only the touched entries cost traffic.
+// Records are a compact array (capacity: one per 2x2-pixel block, the worst case, so nothing can overflow; only the
+// records in use are touched); a direct-mapped index by the 2x2 block of the root (two roots can never share one: they
+// would be 8-adjacent) finds the record of a root when two records merge.
 // Labels are bit-exact by construction; float sums depend on atomic order (not bit-reproducible).
 #include "common.cuh"
 #include "spline_eval.cuh"
