@@ -80,7 +80,10 @@ typedef struct {
     double kron_radius;                          /* in units of the 1-sigma ellipse of the second moments          */
     double flux_auto, fluxerr_auto;              /* sum sub, sqrt(sum rms^2) over the ellipse of kron_radius       */
     int32_t npix_auto;                           /* pixels in that ellipse                                          */
-    int32_t flags;                               /* bit 0: aperture cut by the frame edge; bit 1: an ellipse's box is */
+    int32_t flags;                               /* bit 0: the circular aperture is cut by the frame edge; bit 1: the
+                                                    bounding box of the search or Kron ellipse leaves the frame; bit 2:
+                                                    degenerate record (non-finite centroid / moments or flux <= 0): all
+                                                    sums are 0 and nothing was measured                                */
 } bd_phot;
 
 /* ---- context ------------------------------------------------------------------------------------ */
@@ -101,8 +104,10 @@ int bd_detect_workspace_bytes(const bd_ctx *ctx, int B, int H, int W, int64_t ca
  * the survivor sets equal the float64 definition's.
  * Outputs, each [B, ny, nx], any may be NULL:  d_bkg_raw = median_factor*median - mean_factor*mean
  * (float64), d_rms_raw = std (float64), d_median, d_mean (float64), d_n_kept (int32 survivors).
- * Limits: mesh_w % 4 == 0 and mesh_w <= 256 use the TMA loader, other widths a plain loader; a mesh
- * must fit the shared memory of one thread-block cluster (<= 8 CTAs x 200 KiB) else BD_EUNSUPPORTED. */
+ * Limits: a mesh may hold at most 255 * 512 = 130 560 pixels (the sweeps count into per-thread 8-bit histogram
+ * columns, 512 threads per mesh), i.e. up to 361 x 361; larger meshes return BD_EUNSUPPORTED.  Meshes of at
+ * most 4096 pixels with mesh_w % 4 == 0 are held in the registers of one warp; larger ones are staged in shared
+ * memory by TMA (<= 48 KiB) or streamed from global memory / L2 (mesh_w % 4 == 0), other widths use a plain loader. */
 int bd_mesh_stats(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg_params *p,
                   double *d_bkg_raw, double *d_rms_raw, double *d_median, double *d_mean,
                   int32_t *d_n_kept, void *cuda_stream);
@@ -128,7 +133,10 @@ int bkg_estimate(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_
  * resolution), :61-65 (removal), :153 (threshold scan). -------------------------------------------------
  * Per pixel: bkg, rms = cubic B-spline value of the coefficient grids at u=(x+1/2)/mesh_w-1/2,
  * v=(y+1/2)/mesh_h-1/2 (A14);  sub = img - bkg;  mask = rms > 0 && sub > detect_k*rms (strict, A15).
- * The background and the comparison are evaluated in float64; outputs are rounded to float32.
+ * Arithmetic: the y-collapsed spline coefficients of every (row, grid cell) are formed in float64 and split into a
+ * float32 hi/lo pair; a pixel is then float32 FMAs with sub = (img - hi) - (lo + sum), which agrees with the float64
+ * definition to ~1e-6 ADU.  The comparison is float32 on the float32 outputs: sub > (float)detect_k * rms, one
+ * rounded product (the same rule in bkg_subtract, bkg_subtract_detect and detect_sources without a mask).
  * d_sub (required), d_bkg, d_rms: float32 [B,H,W]; d_mask: uint8 [B,H,W] (0/1).  d_bkg, d_rms, d_mask may be
  * NULL (not emitted); detect_k <= 0 with d_mask != NULL is BD_EINVAL. */
 int bkg_subtract(bd_ctx *ctx, const float *d_img, int B, int H, int W, int mesh_h, int mesh_w,
@@ -137,8 +145,8 @@ int bkg_subtract(bd_ctx *ctx, const float *d_img, int B, int H, int W, int mesh_
 
 /* ---- detect_sources = a4 + a5 (kernels K4, K5).  PAPER.md:153 (connect pixels above the main
  * threshold into candidates; peak and total flux per candidate), :159 (isophotal flux). ------------------
- * d_mask: uint8 [B,H,W], non-zero = foreground.  If NULL the mask is computed from
- * (d_sub, d_rms, detect_k) with the bkg_subtract rule in float64 on the float32 inputs.
+ * d_mask: uint8 [B,H,W], non-zero = foreground.  If NULL the mask is computed from (d_sub, d_rms, detect_k) with
+ * the bkg_subtract rule (float32: rms > 0 && sub > (float)detect_k * rms), so it equals bkg_subtract's mask bit for bit.
  * d_labels: int32 [B,H,W] out; 8-connected components (A16), label = 1 + minimum raster index of the
  * component within its frame, 0 = background; all components are labelled (A20).
  * d_cat: records of components with npix >= min_area (A19), ascending (frame, label); the first

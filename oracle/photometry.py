@@ -20,7 +20,9 @@ A25  Kron radius: r1 = sum r * sub / sum sub over the pixels with r <= kron_sear
 A26  auto: flux_auto = sum of sub over the pixels with r <= kron_radius (hard edge, pixel centres), npix_auto their
      number, fluxerr_auto = sqrt(sum rms^2).  Flag bit 1: the bounding box of either ellipse leaves the frame (the sums
      then run over the part inside).
-A27  no masking of neighbours and no deblending (SURVEY.md NEXT-1 is not built).
+A27  no masking of neighbours (the measurement follows whatever catalogue it is given: raw, deblended or cleaned).
+A28  a record whose centroid or moments are not finite, or whose (regularised) moments define no ellipse (D <= 0, x2 <= 0
+     or y2 <= 0), is not measured: every output 0, flags = 4.
 """
 from __future__ import annotations
 
@@ -79,6 +81,13 @@ def measure_one(sub: np.ndarray, rms: np.ndarray, src, p: PhotParams):
     H, W = sub.shape
     xc, yc = float(src["x"]), float(src["y"])
     flags = 0
+    # ---- A28 degenerate record
+    m = [xc, yc, float(src["x2"]), float(src["y2"]), float(src["xy"])]
+    if not all(np.isfinite(v) for v in m):
+        return 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0, 4
+    _x2, _y2 = (m[2] + 1.0 / 12.0, m[3] + 1.0 / 12.0) if m[2] * m[3] - m[4] * m[4] < 0.00694 else (m[2], m[3])
+    if not (_x2 * _y2 - m[4] * m[4] > 0.0 and _x2 > 0.0 and _y2 > 0.0):
+        return 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0, 4
     # ---- A23 aperture
     x_lo, x_hi, cx = _box(xc, p.r_aper + 1.0, W)
     y_lo, y_hi, cy = _box(yc, p.r_aper + 1.0, H)

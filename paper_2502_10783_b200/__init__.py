@@ -22,6 +22,7 @@ EXPORTS = ["bd_create", "bd_destroy", "bd_last_error", "bd_default_bkg_params", 
            "bd_bkg_workspace_bytes", "bd_detect_workspace_bytes", "bd_mesh_stats", "bd_grid_filter_spline",
            "bkg_estimate", "bkg_subtract", "detect_sources", "bkg_subtract_detect", "bd_default_phot_params", "bd_phot_workspace_bytes", "photometry",
            "bd_run_host"]
+DEBUG_EXPORTS = ["bd_debug_k1_slow_meshes", "bd_debug_k1_reasons", "bd_debug_k1_force_slow", "bd_debug_tile_kernel_events"]
 
 
 class _CParams(C.Structure):
@@ -65,7 +66,7 @@ def load_library(build: bool = True):
         path = _build.build() if build else _build.LIB
         lib = C.CDLL(path)
         lib.bd_last_error.restype = C.c_char_p
-        for name in EXPORTS:
+        for name in EXPORTS + DEBUG_EXPORTS:
             getattr(lib, name)          # fail loudly if a declared symbol is missing
         _lib = lib
     return _lib
@@ -83,8 +84,25 @@ def _ptr(t):
     return C.c_void_p(0 if t is None else t.data_ptr())
 
 
-def _stream():
-    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+def _chk(ctx, t, dtype, name, shape=None, optional=False):
+    """A tensor handed to the C ABI must be what its signature says: on ctx's device, of the right dtype, contiguous."""
+    if t is None:
+        if optional:
+            return None
+        raise BkgdetError(f"{name}: tensor required")
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.device.index != ctx.device:
+        raise BkgdetError(f"{name}: expected a CUDA tensor on device {ctx.device}, got {getattr(t, 'device', type(t))}")
+    if dtype is not None and t.dtype != dtype:
+        raise BkgdetError(f"{name}: expected dtype {dtype}, got {t.dtype}")
+    if not t.is_contiguous():
+        raise BkgdetError(f"{name}: tensor must be contiguous")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise BkgdetError(f"{name}: expected shape {tuple(shape)}, got {tuple(t.shape)}")
+    return t
+
+
+def _stream(ctx):
+    return C.c_void_p(torch.cuda.current_stream(ctx.device).cuda_stream)
 
 
 class Context:
@@ -152,8 +170,30 @@ def _dev(ctx):
     return torch.device("cuda", ctx.device)
 
 
+_OUT_DTYPES = dict(sub=torch.float32, bkg=torch.float32, rms=torch.float32, mask=torch.uint8, labels=torch.int32)
+
+
+def _check_out(ctx, B, H, W, out):
+    for k, t in (out or {}).items():
+        if t is None:
+            continue
+        if k in _OUT_DTYPES:
+            _chk(ctx, t, _OUT_DTYPES[k], f"out[{k}]", (B, H, W))
+        elif k == "cat":
+            _chk(ctx, t, torch.uint8, "out[cat]")
+        elif k == "n_sources":
+            _chk(ctx, t, torch.int64, "out[n_sources]", (B,))
+
+
+def _check_coef_and_out(ctx, B, H, W, mesh_h, mesh_w, bkg_coef, rms_coef, out):
+    ny, nx = grid_shape(H, W, mesh_h, mesh_w)
+    _chk(ctx, bkg_coef, torch.float64, "bkg_coef", (B, ny, nx)); _chk(ctx, rms_coef, torch.float64, "rms_coef", (B, ny, nx))
+    _check_out(ctx, B, H, W, out)
+
+
 def mesh_stats(ctx: Context, img: torch.Tensor, p: BkgParams):
     """a1 (K1).  img float32 [B,H,W] on the device -> dict of [B,ny,nx] tensors."""
+    _chk(ctx, img, torch.float32, "img")
     B, H, W = img.shape
     ny, nx = grid_shape(H, W, p.mesh_h, p.mesh_w)
     dev = _dev(ctx)
@@ -161,24 +201,26 @@ def mesh_stats(ctx: Context, img: torch.Tensor, p: BkgParams):
     out["n_kept"] = torch.empty((B, ny, nx), dtype=torch.int32, device=dev)
     cp = p.c()
     ctx.check(ctx.lib.bd_mesh_stats(ctx.h, _ptr(img), B, H, W, C.byref(cp), _ptr(out["bkg"]), _ptr(out["rms"]),
-                                    _ptr(out["median"]), _ptr(out["mean"]), _ptr(out["n_kept"]), _stream()))
+                                    _ptr(out["median"]), _ptr(out["mean"]), _ptr(out["n_kept"]), _stream(ctx)))
     return out
 
 
 def grid_filter_spline(ctx: Context, bkg_raw: torch.Tensor, rms_raw: torch.Tensor, filt_h: int, filt_w: int):
     """a2 (K2).  raw grids float64 [B,ny,nx] -> (bkg_mesh f32, rms_mesh f32, bkg_coef f64, rms_coef f64)."""
+    _chk(ctx, bkg_raw, torch.float64, "bkg_raw"); _chk(ctx, rms_raw, torch.float64, "rms_raw", bkg_raw.shape)
     B, ny, nx = bkg_raw.shape
     dev = _dev(ctx)
     bm = torch.empty((B, ny, nx), dtype=torch.float32, device=dev); rm = torch.empty_like(bm)
     cb = torch.empty((B, ny, nx), dtype=torch.float64, device=dev); cr = torch.empty_like(cb)
     ws = torch.empty(4 * B * (ny + nx) + 32, dtype=torch.float64, device=dev)
     ctx.check(ctx.lib.bd_grid_filter_spline(ctx.h, _ptr(bkg_raw), _ptr(rms_raw), B, ny, nx, filt_h, filt_w, _ptr(bm),
-                                            _ptr(rm), _ptr(cb), _ptr(cr), _ptr(ws), C.c_size_t(ws.numel() * 8), _stream()))
+                                            _ptr(rm), _ptr(cb), _ptr(cr), _ptr(ws), C.c_size_t(ws.numel() * 8), _stream(ctx)))
     return bm, rm, cb, cr
 
 
 def bkg_estimate(ctx: Context, img: torch.Tensor, p: BkgParams, ws: torch.Tensor | None = None):
     """a1 + a2.  -> (bkg_mesh f32, rms_mesh f32, bkg_coef f64, rms_coef f64), each [B,ny,nx]."""
+    _chk(ctx, img, torch.float32, "img"); _chk(ctx, ws, torch.uint8, "ws", optional=True)
     B, H, W = img.shape
     ny, nx = grid_shape(H, W, p.mesh_h, p.mesh_w)
     dev = _dev(ctx)
@@ -188,7 +230,7 @@ def bkg_estimate(ctx: Context, img: torch.Tensor, p: BkgParams, ws: torch.Tensor
         ws = torch.empty(ctx.bkg_workspace_bytes(B, H, W, p), dtype=torch.uint8, device=dev)
     cp = p.c()
     ctx.check(ctx.lib.bkg_estimate(ctx.h, _ptr(img), B, H, W, C.byref(cp), _ptr(bm), _ptr(rm), _ptr(cb), _ptr(cr),
-                                   _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+                                   _ptr(ws), C.c_size_t(ws.numel()), _stream(ctx)))
     return bm, rm, cb, cr
 
 
@@ -196,7 +238,9 @@ def bkg_subtract(ctx: Context, img: torch.Tensor, mesh_h: int, mesh_w: int, bkg_
                  rms_coef: torch.Tensor, detect_k: float, want_bkg: bool = True, want_rms: bool = True,
                  want_mask: bool = True, out: dict | None = None):
     """a3 (K3).  -> dict(sub, bkg, rms float32 [B,H,W]; mask uint8 [B,H,W]); absent outputs are None."""
+    _chk(ctx, img, torch.float32, "img")
     B, H, W = img.shape
+    _check_coef_and_out(ctx, B, H, W, mesh_h, mesh_w, bkg_coef, rms_coef, out)
     dev = _dev(ctx)
     o = out or {}
     sub = o.get("sub") if o.get("sub") is not None else torch.empty((B, H, W), dtype=torch.float32, device=dev)
@@ -204,7 +248,7 @@ def bkg_subtract(ctx: Context, img: torch.Tensor, mesh_h: int, mesh_w: int, bkg_
     rms = (o.get("rms") if o.get("rms") is not None else torch.empty_like(sub)) if want_rms else None
     mask = (o.get("mask") if o.get("mask") is not None else torch.empty((B, H, W), dtype=torch.uint8, device=dev)) if want_mask else None
     ctx.check(ctx.lib.bkg_subtract(ctx.h, _ptr(img), B, H, W, mesh_h, mesh_w, _ptr(bkg_coef), _ptr(rms_coef),
-                                   C.c_double(detect_k), _ptr(sub), _ptr(bkg), _ptr(rms), _ptr(mask), _stream()))
+                                   C.c_double(detect_k), _ptr(sub), _ptr(bkg), _ptr(rms), _ptr(mask), _stream(ctx)))
     return dict(sub=sub, bkg=bkg, rms=rms, mask=mask)
 
 
@@ -212,7 +256,11 @@ def detect_sources(ctx: Context, sub: torch.Tensor, rms: torch.Tensor | None, ma
                    detect_k: float, min_area: int, cat_capacity: int, ws: torch.Tensor | None = None,
                    out: dict | None = None):
     """a4 + a5 (K4, K5).  -> dict(labels int32 [B,H,W], cat uint8 [cap*88] (device), n_sources int64 [B])."""
+    _chk(ctx, sub, torch.float32, "sub")
     B, H, W = sub.shape
+    _chk(ctx, rms, torch.float32, "rms", (B, H, W), optional=True); _chk(ctx, mask, torch.uint8, "mask", (B, H, W), optional=True)
+    _chk(ctx, ws, torch.uint8, "ws", optional=True)
+    _check_out(ctx, B, H, W, out)
     dev = _dev(ctx)
     o = out or {}
     labels = o.get("labels") if o.get("labels") is not None else torch.empty((B, H, W), dtype=torch.int32, device=dev)
@@ -222,7 +270,7 @@ def detect_sources(ctx: Context, sub: torch.Tensor, rms: torch.Tensor | None, ma
         ws = torch.empty(ctx.detect_workspace_bytes(B, H, W, cat_capacity), dtype=torch.uint8, device=dev)
     ctx.check(ctx.lib.detect_sources(ctx.h, _ptr(sub), _ptr(rms), _ptr(mask), B, H, W, C.c_double(detect_k),
                                      C.c_int32(min_area), _ptr(labels), _ptr(cat), C.c_int64(cat_capacity), _ptr(nsrc),
-                                     _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+                                     _ptr(ws), C.c_size_t(ws.numel()), _stream(ctx)))
     return dict(labels=labels, cat=cat, n_sources=nsrc)
 
 
@@ -231,7 +279,9 @@ def bkg_subtract_detect(ctx: Context, img: torch.Tensor, mesh_h: int, mesh_w: in
                         want_bkg: bool = True, want_rms: bool = True, want_mask: bool = True,
                         ws: torch.Tensor | None = None, out: dict | None = None):
     """a3 + a4 + a5 in one pass.  -> dict(sub, bkg, rms, mask, labels, cat, n_sources)."""
+    _chk(ctx, img, torch.float32, "img"); _chk(ctx, ws, torch.uint8, "ws", optional=True)
     B, H, W = img.shape
+    _check_coef_and_out(ctx, B, H, W, mesh_h, mesh_w, bkg_coef, rms_coef, out)
     dev = _dev(ctx)
     o = out or {}
     def buf(key, dtype, want=True):
@@ -247,7 +297,7 @@ def bkg_subtract_detect(ctx: Context, img: torch.Tensor, mesh_h: int, mesh_w: in
     ctx.check(ctx.lib.bkg_subtract_detect(ctx.h, _ptr(img), B, H, W, mesh_h, mesh_w, _ptr(bkg_coef), _ptr(rms_coef),
                                           C.c_double(detect_k), C.c_int32(min_area), _ptr(sub), _ptr(bkg), _ptr(rms),
                                           _ptr(mask), _ptr(labels), _ptr(cat), C.c_int64(cat_capacity), _ptr(nsrc),
-                                          _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+                                          _ptr(ws), C.c_size_t(ws.numel()), _stream(ctx)))
     return dict(sub=sub, bkg=bkg, rms=rms, mask=mask, labels=labels, cat=cat, n_sources=nsrc)
 
 
@@ -281,7 +331,10 @@ def photometry(ctx: Context, sub: torch.Tensor, rms: torch.Tensor, cat: torch.Te
                cat_capacity: int, p: "PhotParams | None" = None, out: torch.Tensor | None = None,
                ws: torch.Tensor | None = None) -> torch.Tensor:
     """NEXT-2 (K6): aperture + auto photometry of the catalogue records.  -> uint8 [cap*56] device bytes (PHOT_DTYPE)."""
+    _chk(ctx, sub, torch.float32, "sub")
     B, H, W = sub.shape
+    _chk(ctx, rms, torch.float32, "rms", (B, H, W)); _chk(ctx, cat, torch.uint8, "cat"); _chk(ctx, n_sources, torch.int64, "n_sources", (B,))
+    _chk(ctx, out, torch.uint8, "out", optional=True); _chk(ctx, ws, torch.uint8, "ws", optional=True)
     p = p or PhotParams()
     if out is None:
         out = torch.zeros(max(cat_capacity, 1) * PHOT_DTYPE.itemsize, dtype=torch.uint8, device=_dev(ctx))
@@ -290,7 +343,7 @@ def photometry(ctx: Context, sub: torch.Tensor, rms: torch.Tensor, cat: torch.Te
         ctx.check(ctx.lib.bd_phot_workspace_bytes(ctx.h, C.c_int64(cat_capacity), C.byref(nb)))
         ws = torch.empty(nb.value, dtype=torch.uint8, device=_dev(ctx))
     ctx.check(ctx.lib.photometry(ctx.h, _ptr(sub), _ptr(rms), B, H, W, _ptr(cat), _ptr(n_sources), C.c_int64(cat_capacity),
-                                 C.byref(p._c), _ptr(out), _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+                                 C.byref(p._c), _ptr(out), _ptr(ws), C.c_size_t(ws.numel()), _stream(ctx)))
     return out
 
 

@@ -24,30 +24,34 @@ int bd_create(bd_ctx **out, int device) {
     *out = nullptr;
     int n = 0;
     if (cudaGetDeviceCount(&n) != cudaSuccess || n <= 0 || device < 0 || device >= n) return BD_ECUDA;
-    if (cudaSetDevice(device) != cudaSuccess) return BD_ECUDA;
     bd_ctx *c = (bd_ctx *)calloc(1, sizeof(bd_ctx));
     if (!c) return BD_ECUDA;
     c->device = device;
-    cudaDeviceProp prop;
-    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { free(c); return BD_ECUDA; }
-    c->num_sms = prop.multiProcessorCount;
-    c->smem_optin = prop.sharedMemPerBlockOptin;
-    void *fn = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) == cudaSuccess &&
-        qres == cudaDriverEntryPointSuccess)
-        c->encode_tiled = (decltype(c->encode_tiled))fn;
-    cudaGetLastError();
+    {
+        BdDeviceGuard guard(c);   // the caller's current device is put back on return
+        if (guard.err != cudaSuccess) { free(c); return BD_ECUDA; }
+        cudaDeviceProp prop;
+        if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { free(c); return BD_ECUDA; }
+        c->num_sms = prop.multiProcessorCount;
+        c->smem_optin = prop.sharedMemPerBlockOptin;
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            c->encode_tiled = (decltype(c->encode_tiled))fn;
+        cudaGetLastError();
+    }
     *out = c;
     return BD_OK;
 }
 
 void bd_destroy(bd_ctx *ctx) {
     if (!ctx) return;
-    cudaSetDevice(ctx->device);
-    if (ctx->host_dev) cudaFree(ctx->host_dev);
-    if (ctx->host_pinned) cudaFreeHost(ctx->host_pinned);
-    if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
+    {
+        BdDeviceGuard guard(ctx);
+        if (ctx->host_dev) cudaFree(ctx->host_dev);
+        if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
+    }
     free(ctx);
 }
 
@@ -106,6 +110,7 @@ int bd_mesh_stats(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd
                   double *d_rms_raw, double *d_median, double *d_mean, int32_t *d_n_kept, void *cuda_stream) {
     int rc = check_frame(ctx, B, H, W);
     if (rc) return rc;
+    BD_BIND_DEVICE(ctx);
     if ((rc = check_params(ctx, p))) return rc;
     if (!d_img || !aligned16(d_img)) return bd_set_error(ctx, BD_EINVAL, "d_img null or misaligned");
     return k1_launch(ctx, d_img, B, H, W, p, d_bkg_raw, d_rms_raw, d_median, d_mean, d_n_kept, (cudaStream_t)cuda_stream);
@@ -117,6 +122,7 @@ int bd_grid_filter_spline(bd_ctx *ctx, const double *d_bkg_raw, const double *d_
     if (!ctx) return BD_EINVAL;
     if (!d_bkg_raw || !d_rms_raw || !d_bkg_coef || !d_rms_coef || !d_ws) return bd_set_error(ctx, BD_EINVAL, "null pointer");
     if (B <= 0 || ny <= 0 || nx <= 0 || B > 65535) return bd_set_error(ctx, BD_EINVAL, "bad grid shape");
+    BD_BIND_DEVICE(ctx);
     if (filt_h < 1 || filt_w < 1 || !(filt_h & 1) || !(filt_w & 1) || filt_h > 11 || filt_w > 11)
         return bd_set_error(ctx, BD_EINVAL, "filter size must be odd and in 1..11");
     size_t need = 2 * (size_t)B * k2_scratch_per_grid(ny, nx) * sizeof(double);
@@ -130,6 +136,7 @@ int bkg_estimate(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_
                  void *cuda_stream) {
     int rc = check_frame(ctx, B, H, W);
     if (rc) return rc;
+    BD_BIND_DEVICE(ctx);
     if ((rc = check_params(ctx, p))) return rc;
     if (!d_img || !aligned16(d_img)) return bd_set_error(ctx, BD_EINVAL, "d_img null or misaligned");
     if (!d_bkg_coef || !d_rms_coef || !d_ws) return bd_set_error(ctx, BD_EINVAL, "null coefficient or workspace pointer");
@@ -152,6 +159,7 @@ int bkg_subtract(bd_ctx *ctx, const float *d_img, int B, int H, int W, int mesh_
                  void *cuda_stream) {
     int rc = check_frame(ctx, B, H, W);
     if (rc) return rc;
+    BD_BIND_DEVICE(ctx);
     if (mesh_h <= 0 || mesh_w <= 0) return bd_set_error(ctx, BD_EINVAL, "mesh size must be positive");
     if (!d_img || !d_bkg_coef || !d_rms_coef || !d_sub) return bd_set_error(ctx, BD_EINVAL, "null pointer");
     if (!aligned16(d_img) || !aligned16(d_sub) || !aligned16(d_bkg) || !aligned16(d_rms) || !aligned16(d_mask))
@@ -166,6 +174,7 @@ int detect_sources(bd_ctx *ctx, const float *d_sub, const float *d_rms, const ui
                    int64_t *d_n_sources, void *d_ws, size_t ws_bytes, void *cuda_stream) {
     int rc = check_frame(ctx, B, H, W);
     if (rc) return rc;
+    BD_BIND_DEVICE(ctx);
     if (!d_sub || !d_labels || !d_n_sources || !d_ws) return bd_set_error(ctx, BD_EINVAL, "null pointer");
     if (!d_mask && (!d_rms || !(detect_k > 0.0))) return bd_set_error(ctx, BD_EINVAL, "no mask: d_rms and detect_k > 0 required");
     if (cat_capacity < 0 || (cat_capacity > 0 && !d_cat)) return bd_set_error(ctx, BD_EINVAL, "bad catalogue buffer");
@@ -181,6 +190,7 @@ int bkg_subtract_detect(bd_ctx *ctx, const float *d_img, int B, int H, int W, in
                         void *d_ws, size_t ws_bytes, void *cuda_stream) {
     int rc = check_frame(ctx, B, H, W);
     if (rc) return rc;
+    BD_BIND_DEVICE(ctx);
     if (mesh_h <= 0 || mesh_w <= 0) return bd_set_error(ctx, BD_EINVAL, "mesh size must be positive");
     if (!d_img || !d_bkg_coef || !d_rms_coef || !d_sub || !d_labels || !d_n_sources || !d_ws)
         return bd_set_error(ctx, BD_EINVAL, "null pointer");
@@ -222,11 +232,14 @@ int photometry(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H
                size_t ws_bytes, void *cuda_stream) {
     int rc = check_frame(ctx, B, H, W);
     if (rc) return rc;
+    BD_BIND_DEVICE(ctx);
     if (!d_sub || !d_rms || !d_cat || !d_n_sources || !d_phot || !p || !d_ws) return bd_set_error(ctx, BD_EINVAL, "null pointer");
     if (cat_capacity < 0) return bd_set_error(ctx, BD_EINVAL, "bad catalogue capacity");
     if (!(p->r_aper > 0.0) || !(p->kron_factor > 0.0) || !(p->kron_min_radius > 0.0) || !(p->kron_search > 0.0) || p->subpix < 1 ||
         p->subpix > 16)
         return bd_set_error(ctx, BD_EINVAL, "photometry parameters must be positive, subpix in 1..16");
+    if (!(p->r_aper <= 1024.0) || !(p->kron_factor <= 1024.0) || !(p->kron_min_radius <= 1024.0) || !(p->kron_search <= 1024.0))
+        return bd_set_error(ctx, BD_EINVAL, "photometry radii / factors must be <= 1024");
     if (cat_capacity == 0) return BD_OK;
     return k6_launch(ctx, d_sub, d_rms, B, H, W, d_cat, d_n_sources, cat_capacity, p, d_phot, d_ws, ws_bytes, (cudaStream_t)cuda_stream);
 }
@@ -235,10 +248,10 @@ int bd_run_host(bd_ctx *ctx, const float *h_img, int B, int H, int W, const bd_b
                 int32_t min_area, bd_source *h_cat, int64_t cat_capacity, int64_t *h_n_sources) {
     int rc = check_frame(ctx, B, H, W);
     if (rc) return rc;
+    BD_BIND_DEVICE(ctx);
     if ((rc = check_params(ctx, p))) return rc;
     if (!h_img || !h_n_sources || cat_capacity < 0 || (cat_capacity > 0 && !h_cat))
         return bd_set_error(ctx, BD_EINVAL, "null host pointer");
-    BD_CUDA_CHECK(ctx, cudaSetDevice(ctx->device));
     if (!ctx->host_stream) BD_CUDA_CHECK(ctx, cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking));
     cudaStream_t st = ctx->host_stream;
     const size_t P = (size_t)B * H * W;

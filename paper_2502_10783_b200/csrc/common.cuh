@@ -22,12 +22,29 @@ struct bd_ctx {
     // bd_run_host cache
     void *host_dev;
     size_t host_dev_bytes;
-    void *host_pinned;
-    size_t host_pinned_bytes;
     cudaStream_t host_stream;
 };
 
 int bd_set_error(bd_ctx *ctx, int code, const char *fmt, ...);
+
+// Every entry point that touches the device runs with ctx->device current and puts the caller's device back.
+struct BdDeviceGuard {
+    int prev = -1;
+    bool changed = false;
+    cudaError_t err;
+    explicit BdDeviceGuard(const bd_ctx *ctx) {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != ctx->device) {
+            err = cudaSetDevice(ctx->device);
+            changed = err == cudaSuccess;
+        }
+    }
+    ~BdDeviceGuard() { if (changed) cudaSetDevice(prev); }
+};
+#define BD_BIND_DEVICE(ctx)                                                                             \
+    BdDeviceGuard _bd_guard(ctx);                                                                       \
+    if (_bd_guard.err != cudaSuccess)                                                                   \
+        return bd_set_error((ctx), BD_ECUDA, "cannot bind CUDA device %d: %s", (ctx)->device, cudaGetErrorString(_bd_guard.err))
 
 #define BD_CUDA_CHECK(ctx, expr)                                                                       \
     do {                                                                                               \

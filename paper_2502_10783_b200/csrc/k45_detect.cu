@@ -108,15 +108,16 @@ size_t carve(Ws &w, void *base, int B, int H, int W) {
 }
 
 // ------------------------------------------------------------------------------------------------ mask
-__global__ void k_make_mask(const float *sub, const float *rms, size_t n4, double k_d, uint8_t *mask) {
+// (the same float32 rule as K3 / the fused kernel: spl_above)
+__global__ void k_make_mask(const float *sub, const float *rms, size_t n4, float k_d, uint8_t *mask) {
     size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n4) return;
     float4 s = reinterpret_cast<const float4 *>(sub)[i], r = reinterpret_cast<const float4 *>(rms)[i];
     uint32_t m = 0;
-    m |= (r.x > 0.f && (double)s.x > k_d * (double)r.x) ? 1u : 0u;
-    m |= (r.y > 0.f && (double)s.y > k_d * (double)r.y) ? 1u << 8 : 0u;
-    m |= (r.z > 0.f && (double)s.z > k_d * (double)r.z) ? 1u << 16 : 0u;
-    m |= (r.w > 0.f && (double)s.w > k_d * (double)r.w) ? 1u << 24 : 0u;
+    m |= spl_above(s.x, r.x, k_d) ? 1u : 0u;
+    m |= spl_above(s.y, r.y, k_d) ? 1u << 8 : 0u;
+    m |= spl_above(s.z, r.z, k_d) ? 1u << 16 : 0u;
+    m |= spl_above(s.w, r.w, k_d) ? 1u << 24 : 0u;
     reinterpret_cast<uint32_t *>(mask)[i] = m;
 }
 
@@ -1011,7 +1012,7 @@ int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_
     const uint8_t *mask = d_mask;
     if (!mask && !fz) {
         size_t n4 = P / 4;
-        k_make_mask<<<(unsigned)((n4 + 255) / 256), 256, 0, st>>>(d_sub, d_rms, n4, detect_k, w.maskbuf);
+        k_make_mask<<<(unsigned)((n4 + 255) / 256), 256, 0, st>>>(d_sub, d_rms, n4, (float)detect_k, w.maskbuf);
         mask = w.maskbuf;
     }
     BD_CUDA_CHECK(ctx, cudaMemsetAsync(w.counters, 0, 64 * sizeof(uint32_t), st));

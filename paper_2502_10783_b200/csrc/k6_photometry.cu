@@ -41,7 +41,7 @@ __device__ __forceinline__ int warp_sum_i(int v) {
 __device__ __forceinline__ double sq2(double x, double y) { return __dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)); }
 
 // A24: ellipse metric of an object (1/12 added to the moments of degenerate objects)
-struct Ellipse { double xc, yc, cxx, cyy, cxy, sx2, sy2; };
+struct Ellipse { double xc, yc, cxx, cyy, cxy, sx2, sy2; bool ok; };
 __device__ __forceinline__ Ellipse make_ellipse(const bd_source &s) {
     Ellipse e;
     double x2 = s.x2, y2 = s.y2;
@@ -49,6 +49,8 @@ __device__ __forceinline__ Ellipse make_ellipse(const bd_source &s) {
     if (__dsub_rn(__dmul_rn(x2, y2), __dmul_rn(xy, xy)) < 0.00694) { x2 = x2 + 1.0 / 12.0; y2 = y2 + 1.0 / 12.0; }
     const double det = __dsub_rn(__dmul_rn(x2, y2), __dmul_rn(xy, xy));
     e.xc = s.x; e.yc = s.y;
+    // A28: a record with a non-finite centroid or moments, or moments that define no ellipse, is not measured
+    e.ok = isfinite(s.x) && isfinite(s.y) && isfinite(x2) && isfinite(y2) && isfinite(xy) && det > 0.0 && x2 > 0.0 && y2 > 0.0;
     e.cxx = y2 / det; e.cyy = x2 / det; e.cxy = __dmul_rn(-2.0, xy) / det;
     e.sx2 = sqrt(x2); e.sy2 = sqrt(y2);
     return e;
@@ -64,14 +66,14 @@ __device__ __forceinline__ bool ellipse_box(const Ellipse &e, double R, int H, i
 }
 __device__ __forceinline__ long long box_area(const Box &b) { return (long long)(b.x_hi - b.x_lo + 1) * (b.y_hi - b.y_lo + 1); }
 // this thread's share (pixels t, t + nt, ... of the box) of  S0 = sum I, S1 = sum r I, V = sum rms^2, N = count  over r <= R
-// (IDX = int for boxes below 2^31 pixels: a 64-bit division per pixel costs more than the rest of the loop body)
-template <typename IDX>
-__device__ __forceinline__ void ellipse_partial_t(const Ellipse &e, const Box &b, double R, const float *sub, const float *rms, int W,
-                                                  int t, int nt, double &S0, double &S1, double &V, int &N) {
-    const IDX bw = (IDX)(b.x_hi - b.x_lo + 1);
-    const IDX n = (IDX)box_area(b);
-    for (IDX k = (IDX)t; k < n; k += (IDX)nt) {
-        const IDX row = k / bw;
+// (32-bit pixel indices: the box lies inside the frame and H*W < 2^31 is enforced at the boundary)
+__device__ __forceinline__ void ellipse_partial(const Ellipse &e, const Box &b, double R, const float *sub, const float *rms, int W,
+                                                int t, int nt, double &S0, double &S1, double &V, int &N) {
+    S0 = 0.0; S1 = 0.0; V = 0.0; N = 0;
+    const int bw = b.x_hi - b.x_lo + 1;
+    const int n = (int)box_area(b);
+    for (int k = t; k < n; k += nt) {
+        const int row = k / bw;
         const int yy = b.y_lo + (int)row, xx = b.x_lo + (int)(k - row * bw);
         const double dx = (double)xx - e.xc, dy = (double)yy - e.yc;
         const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(__dmul_rn(e.cxx, dx), dx), __dmul_rn(__dmul_rn(e.cyy, dy), dy)),
@@ -82,12 +84,6 @@ __device__ __forceinline__ void ellipse_partial_t(const Ellipse &e, const Box &b
             S0 += I; S1 += rad * I; V += q * q; ++N;
         }
     }
-}
-__device__ __forceinline__ void ellipse_partial(const Ellipse &e, const Box &b, double R, const float *sub, const float *rms, int W,
-                                                int t, int nt, double &S0, double &S1, double &V, int &N) {
-    S0 = 0.0; S1 = 0.0; V = 0.0; N = 0;
-    if (box_area(b) < 0x7FFF0000ll) ellipse_partial_t<int>(e, b, R, sub, rms, W, t, nt, S0, S1, V, N);
-    else ellipse_partial_t<long long>(e, b, R, sub, rms, W, t, nt, S0, S1, V, N);
 }
 __device__ __forceinline__ double kron_radius_of(const bd_phot_params &p, double S0, double S1) {   // A25
     if (S0 > 0.0 && S1 > 0.0) return fmax(__dmul_rn(p.kron_factor, S1) / S0, p.kron_min_radius);
@@ -117,6 +113,16 @@ __global__ void __launch_bounds__(256) k6_photometry(K6Args a) {
         const float *sub = a.sub + (size_t)s.frame * HW, *rms = a.rms + (size_t)s.frame * HW;
         const double xc = s.x, yc = s.y;
         int flags = 0;
+        const Ellipse e = make_ellipse(s);
+        if (!e.ok) {   // A28: degenerate record
+            if (lane == 0) {
+                bd_phot o;
+                o.flux_aper = 0.0; o.fluxerr_aper = 0.0; o.area_aper = 0.0; o.kron_radius = 0.0; o.flux_auto = 0.0; o.fluxerr_auto = 0.0;
+                o.npix_auto = 0; o.flags = 4;
+                a.out[i] = o;
+            }
+            continue;
+        }
         // ---- A23: circular aperture with sub-pixel sampling of the rim ------------------------------------------
         double f_ap = 0.0, a_ap = 0.0, v_ap = 0.0;
         {
@@ -154,7 +160,6 @@ __global__ void __launch_bounds__(256) k6_photometry(K6Args a) {
             if (__any_sync(0xffffffffu, out_w)) flags |= 1;
         }
         // ---- A24-A26: ellipse, Kron radius, auto flux ------------------------------------------------------------------
-        const Ellipse e = make_ellipse(s);
         Box b;
         bool cut;
         double S0 = 0.0, S1 = 0.0, V = 0.0, kron = a.p.kron_min_radius;

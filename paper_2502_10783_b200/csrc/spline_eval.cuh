@@ -78,6 +78,11 @@ __device__ __forceinline__ void spl_x_weights(int x, int mw, int i0, float wx[4]
     wx[0] = (float)w[0]; wx[1] = (float)w[1]; wx[2] = (float)w[2]; wx[3] = (float)w[3];
 }
 
+// The threshold rule of the library (A15), in ONE place: float32 product, float32 compare, on the float32 sub / rms values the
+// interface materialises.  K3, the fused tile kernel and the mask-less path of detect_sources (k_make_mask) all call it,
+// so the three routes give the same mask bit for bit whatever detect_k is (k_d = (float)detect_k).
+__device__ __forceinline__ bool spl_above(float sub, float rms, float k_d) { return (rms > 0.0f) && (sub > __fmul_rn(k_d, rms)); }
+
 // one pixel: t0 = {hi, lo, e_-1, e_+1}, t1 = {e_+2, r_-1, r_0, r_+1}, t8 = r_+2
 __device__ __forceinline__ bool spl_pixel(const float4 &t0, const float4 &t1, float t8, const float wx[4], float in, float k_d,
                                           float &o_sub, float &o_bkg, float &o_rms) {
@@ -93,5 +98,5 @@ __device__ __forceinline__ bool spl_pixel(const float4 &t0, const float4 &t1, fl
     o_sub = d;
     o_bkg = t0.x + rel;
     o_rms = s;
-    return (s > 0.0f) && (d > k_d * s);
+    return spl_above(d, s, k_d);
 }

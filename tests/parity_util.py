@@ -7,9 +7,11 @@ Tolerances, written out:
   * sub: |d| <= 1e-4 * |bkg_oracle| (a relative test on a zero-mean quantity is meaningless);
   * mask: may differ only where the oracle's |sub - k*rms| <= 1e-5 * rms ("fragile" pixels);
   * labels: bit-exact against the oracle's labelling of the SAME mask;
-  * catalogue: 1:1 on (frame, label); npix, bbox, peak position exact; peak value 1e-6 relative (float32 rounding of sub);
-    flux, x, y 1e-4 relative
-    (x, y additionally 1e-3 px absolute is reported); x2, y2, xy 1e-3 relative to max(|moment|, 1e-3*(x2+y2)).
+  * catalogue: 1:1 on (frame, label); npix, bbox exact.  STAGE comparison (both sides reduce the same float32 sub map,
+    `peak_pos_exact=True`): peak position and peak value bit-exact.  CHAIN comparison (each side reduces its own sub map;
+    the two maps agree to ~1e-6 ADU): peak value 1e-6 relative, peak position may move between pixels that are equal to
+    the last bit (<= 1 % of the records).  flux, x, y 1e-4 relative (the absolute centroid error is reported);
+    x2, y2, xy 1e-3 relative to max(|moment|, 1e-3*(x2+y2) + 1e-9)  (derivation in DESIGN.md section 8).
 """
 from __future__ import annotations
 
@@ -67,9 +69,13 @@ def assert_catalogue_equal(got, want, frame=None, exempt_labels=(), peak_pos_exa
         # pixels of a component are equal to the last bit (adjacent saturated / hot pixels) the winner may
         # differ.  The peak VALUE is still compared below; such near-ties must stay rare.
         assert moved.sum() <= max(2, len(want) // 100), f"{moved.sum()} of {len(want)} peak positions differ"
-    # peak is a float32 value of sub: both sides round a value that agrees to ~1e-6 ADU, so the last bit may differ
-    perr = np.abs(got["peak"].astype(np.float64) - want["peak"]) / np.maximum(np.abs(want["peak"]), 1e-300)
-    assert np.all(perr <= REL_PEAK), f"peak: worst rel {perr.max():.3e}"
+    if peak_pos_exact:
+        # stage comparison: the peak is an element of the one float32 sub map both sides read
+        assert np.array_equal(got["peak"].astype(np.float64), want["peak"]), "peak value differs (must be bit-exact)"
+    else:
+        # chain comparison: each side rounds to float32 a value that agrees to ~1e-6 ADU, so the last bit may differ
+        perr = np.abs(got["peak"].astype(np.float64) - want["peak"]) / np.maximum(np.abs(want["peak"]), 1e-300)
+        assert np.all(perr <= REL_PEAK), f"peak: worst rel {perr.max():.3e}"
     worst = {}
     for k in ("flux", "x", "y"):
         err = np.abs(got[k] - want[k]) / np.maximum(np.abs(want[k]), 1e-300)

@@ -9,8 +9,8 @@ import pytest
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def declared_functions():
-    src = open(os.path.join(ROOT, "include", "bkgdet.h")).read()
+def declared_functions(header="bkgdet.h"):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     names = re.findall(r"^\s*(?:int|void|const char \*)\s*\**\s*([A-Za-z_]\w*)\s*\(", src, flags=re.M)
     return sorted(set(names))
@@ -30,6 +30,17 @@ def test_library_builds_loads_and_exports_all_symbols():
     for n in declared_functions():
         assert hasattr(lib, n), f"{n} declared in bkgdet.h but not exported"
     assert sorted(m.EXPORTS) == declared_functions()
+    # the diagnostic entry points have a header of their own; nothing else is exported with a bd_ / API name
+    dbg = declared_functions("bkgdet_debug.h")
+    assert len(dbg) >= 4
+    for n in dbg:
+        assert hasattr(lib, n), f"{n} declared in bkgdet_debug.h but not exported"
+    assert sorted(m.DEBUG_EXPORTS) == dbg
+    import subprocess
+    out = subprocess.run(["nm", "-D", "--defined-only", _build.LIB], capture_output=True, text=True).stdout
+    exported = {ln.split()[-1] for ln in out.splitlines() if " T " in ln}
+    plain_c = {n for n in exported if not n.startswith("_Z") and not n.startswith("__")} - {"_init", "_fini"}
+    assert plain_c == set(declared_functions()) | set(dbg), plain_c ^ (set(declared_functions()) | set(dbg))
 
 
 def test_struct_layouts_match_header():
