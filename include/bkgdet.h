@@ -104,13 +104,15 @@ int bd_detect_workspace_bytes(const bd_ctx *ctx, int B, int H, int W, int64_t ca
  * the survivor sets equal the float64 definition's.
  * Outputs, each [B, ny, nx], any may be NULL:  d_bkg_raw = median_factor*median - mean_factor*mean
  * (float64), d_rms_raw = std (float64), d_median, d_mean (float64), d_n_kept (int32 survivors).
+ * d_ws / ws_bytes: at least bd_bkg_workspace_bytes() (4 bytes per mesh are used: the list of meshes the warp-per-mesh
+ * kernel hands to the general path).
  * Limits: a mesh may hold at most 255 * 512 = 130 560 pixels (the sweeps count into per-thread 8-bit histogram
  * columns, 512 threads per mesh), i.e. up to 361 x 361; larger meshes return BD_EUNSUPPORTED.  Meshes of at
  * most 4096 pixels with mesh_w % 4 == 0 are held in the registers of one warp; larger ones are staged in shared
  * memory by TMA (<= 48 KiB) or streamed from global memory / L2 (mesh_w % 4 == 0), other widths use a plain loader. */
 int bd_mesh_stats(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg_params *p,
                   double *d_bkg_raw, double *d_rms_raw, double *d_median, double *d_mean,
-                  int32_t *d_n_kept, void *cuda_stream);
+                  int32_t *d_n_kept, void *d_ws, size_t ws_bytes, void *cuda_stream);
 
 /* ---- a2: median filter of both mesh grids + cubic B-spline prefilter (kernel K2).  PAPER.md:80. --------
  * In: raw grids float64 [B, ny, nx].  Out: filtered grids (float32, for the caller; may be NULL) and the

@@ -200,8 +200,10 @@ def mesh_stats(ctx: Context, img: torch.Tensor, p: BkgParams):
     out = {k: torch.empty((B, ny, nx), dtype=torch.float64, device=dev) for k in ("bkg", "rms", "median", "mean")}
     out["n_kept"] = torch.empty((B, ny, nx), dtype=torch.int32, device=dev)
     cp = p.c()
+    ws = torch.empty(ctx.bkg_workspace_bytes(B, H, W, p), dtype=torch.uint8, device=dev)
     ctx.check(ctx.lib.bd_mesh_stats(ctx.h, _ptr(img), B, H, W, C.byref(cp), _ptr(out["bkg"]), _ptr(out["rms"]),
-                                    _ptr(out["median"]), _ptr(out["mean"]), _ptr(out["n_kept"]), _stream(ctx)))
+                                    _ptr(out["median"]), _ptr(out["mean"]), _ptr(out["n_kept"]), _ptr(ws),
+                                    C.c_size_t(ws.numel()), _stream(ctx)))
     return out
 
 

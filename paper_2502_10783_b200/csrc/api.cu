@@ -95,8 +95,9 @@ int bd_bkg_workspace_bytes(const bd_ctx *ctx, int B, int H, int W, const bd_bkg_
     if (!ctx || !p || !bytes || B <= 0 || H <= 0 || W <= 0 || p->mesh_h <= 0 || p->mesh_w <= 0) return BD_EINVAL;
     const int ny = (H + p->mesh_h - 1) / p->mesh_h, nx = (W + p->mesh_w - 1) / p->mesh_w;
     size_t cells = (size_t)B * ny * nx;
-    // raw bkg, raw rms, then K2's scratch
-    *bytes = 2 * bd_align_up(cells * sizeof(double), 256) + 2 * (size_t)B * k2_scratch_per_grid(ny, nx) * sizeof(double) + 512;
+    // raw bkg, raw rms, K2's scratch, K1's worklist
+    *bytes = 2 * bd_align_up(cells * sizeof(double), 256) + bd_align_up(2 * (size_t)B * k2_scratch_per_grid(ny, nx) * sizeof(double), 256) +
+             k1_workspace_bytes(B, ny, nx) + 512;
     return BD_OK;
 }
 
@@ -107,13 +108,18 @@ int bd_detect_workspace_bytes(const bd_ctx *ctx, int B, int H, int W, int64_t ca
 }
 
 int bd_mesh_stats(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg_params *p, double *d_bkg_raw,
-                  double *d_rms_raw, double *d_median, double *d_mean, int32_t *d_n_kept, void *cuda_stream) {
+                  double *d_rms_raw, double *d_median, double *d_mean, int32_t *d_n_kept, void *d_ws, size_t ws_bytes,
+                  void *cuda_stream) {
     int rc = check_frame(ctx, B, H, W);
     if (rc) return rc;
     BD_BIND_DEVICE(ctx);
     if ((rc = check_params(ctx, p))) return rc;
     if (!d_img || !aligned16(d_img)) return bd_set_error(ctx, BD_EINVAL, "d_img null or misaligned");
-    return k1_launch(ctx, d_img, B, H, W, p, d_bkg_raw, d_rms_raw, d_median, d_mean, d_n_kept, (cudaStream_t)cuda_stream);
+    const int ny = (H + p->mesh_h - 1) / p->mesh_h, nx = (W + p->mesh_w - 1) / p->mesh_w;
+    const size_t need = k1_workspace_bytes(B, ny, nx) + 256;
+    if (!d_ws || ws_bytes < need) return bd_set_error(ctx, BD_EWORKSPACE, "mesh statistics workspace: need %zu bytes, got %zu", need, ws_bytes);
+    return k1_launch(ctx, d_img, B, H, W, p, d_bkg_raw, d_rms_raw, d_median, d_mean, d_n_kept, (void *)bd_align_up((size_t)d_ws, 256),
+                     (cudaStream_t)cuda_stream);
 }
 
 int bd_grid_filter_spline(bd_ctx *ctx, const double *d_bkg_raw, const double *d_rms_raw, int B, int ny, int nx,
@@ -147,8 +153,9 @@ int bkg_estimate(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_
     const size_t cells = (size_t)B * ny * nx, stride = bd_align_up(cells * sizeof(double), 256);
     char *base = (char *)bd_align_up((size_t)d_ws, 256);
     double *raw_b = (double *)base, *raw_r = (double *)(base + stride), *scratch = (double *)(base + 2 * stride);
+    void *k1_ws = base + 2 * stride + bd_align_up(2 * (size_t)B * k2_scratch_per_grid(ny, nx) * sizeof(double), 256);
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    rc = k1_launch(ctx, d_img, B, H, W, p, raw_b, raw_r, nullptr, nullptr, nullptr, st);
+    rc = k1_launch(ctx, d_img, B, H, W, p, raw_b, raw_r, nullptr, nullptr, nullptr, k1_ws, st);
     if (rc) return rc;
     return k2_launch(ctx, raw_b, raw_r, B, ny, nx, p->filt_h, p->filt_w, d_bkg_mesh, d_rms_mesh, d_bkg_coef, d_rms_coef,
                      scratch, st);

@@ -68,8 +68,10 @@ struct K1Plan {
     size_t slab_bytes;  // shared memory in front of the fixed part: the slab, or room for the sort arrays
 };
 int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan);
+// d_ws: k1_workspace_bytes() of device memory (the worklist of meshes the warp-per-mesh kernel hands to the general path)
+size_t k1_workspace_bytes(int B, int ny, int nx);
 int k1_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg_params *p, double *d_bkg_raw,
-              double *d_rms_raw, double *d_median, double *d_mean, int32_t *d_n_kept, cudaStream_t st);
+              double *d_rms_raw, double *d_median, double *d_mean, int32_t *d_n_kept, void *d_ws, cudaStream_t st);
 
 // doubles of scratch K2 needs per (frame, grid): the Thomas factors of both directions
 static inline __host__ __device__ size_t k2_scratch_per_grid(int ny, int nx) { return 2 * ((size_t)ny + (size_t)nx); }

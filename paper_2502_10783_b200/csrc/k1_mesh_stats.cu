@@ -29,7 +29,6 @@
 // the key range of [mean - sd, mean + sd] (the median lies within one standard deviation of the mean).
 // It reads the slab from shared memory when C = 1 and the mesh from global memory (L2) otherwise.
 #include <cooperative_groups.h>
-#include <stdlib.h>
 
 #include "common.cuh"
 
@@ -68,6 +67,7 @@ struct K1Args {
     double median_factor, mean_factor;
     double *bkg_raw, *rms_raw, *median, *mean;
     int32_t *n_kept;
+    const uint32_t *list_count, *list;   // list mode (C == 1): the meshes to do are list[0 .. *list_count), grid-stride
 };
 
 struct Xch {   // one CTA's contribution to the team-wide totals (peers read it through DSMEM)
@@ -89,8 +89,8 @@ struct Smem {   // fixed-size part of shared memory; follows the slab
     SampleX sx;
     Xch xch;
     Xch tot;
-    double red_d[2][K1_MAXWARPS];
-    int red_i[2][K1_MAXWARPS];
+    double red_d[2][2][K1_MAXWARPS];   // [slot set][quantity][warp], see block_reduce_stats
+    int red_i[2][2][K1_MAXWARPS];
     uint32_t red_u[K1_MAXWARPS];
     uint32_t win_b0, win_b1;
     uint32_t list[K1_LISTCAP];   // candidate keys: this CTA's during the gather; the team's (sorted) at rank 0
@@ -163,33 +163,73 @@ __device__ __forceinline__ void k1_push_f32_if_outside(uint32_t &addr, float e, 
         : "memory");
 }
 
+// ---- warp-wide helpers (also used by k1w_warp_mesh.cuh) -----------------------------------------------------
+__device__ __forceinline__ double kw_sum(double v) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ int kw_sum(int v) { return __reduce_add_sync(0xffffffffu, v); }
+
+// ascending bitonic sort of 256 keys held 8 per lane, element e = lane * 8 + r
+__device__ __forceinline__ void kw_sort256(uint32_t (&x)[8], int lane) {
+#pragma unroll
+    for (int k = 2; k <= 256; k <<= 1) {
+#pragma unroll
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            if (j >= 8) {
+                const int lm = j >> 3;
+                const bool keep_min = ((lane & lm) == 0) == (((lane * 8) & k) == 0);
+#pragma unroll
+                for (int r = 0; r < 8; ++r) {
+                    const uint32_t y = __shfl_xor_sync(0xffffffffu, x[r], lm);
+                    x[r] = keep_min ? min(x[r], y) : max(x[r], y);
+                }
+            } else {
+#pragma unroll
+                for (int r = 0; r < 8; ++r) {
+                    const int p = r ^ j;
+                    if (p > r) {
+                        const bool up = ((lane * 8 + r) & k) == 0;
+                        const uint32_t lo = min(x[r], x[p]), hi = max(x[r], x[p]);
+                        x[r] = up ? lo : hi;
+                        x[p] = up ? hi : lo;
+                    }
+                }
+            }
+        }
+    }
+}
+
 // ---- block-wide reductions (result valid in every thread) -------------------------------------------------
-__device__ void block_reduce_stats(Smem &s, double &s1, double &s2, int &n_in, int &n_below) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+// ONE barrier per call: every warp leaves its partial in the slot set `ph & 1`, and after the barrier every thread adds
+// the (<= 16) partials itself, in warp order -- the same bits in every thread.  The slot sets alternate from call to
+// call (ph counts the calls; all threads of the CTA make the same calls), so a set is rewritten only after a later
+// call's barrier, when nobody reads it any more.  (The first version used three barriers and a second shuffle tree per
+// call; with a call per clipping round that was 25 k cycles per mesh.)
+__device__ __forceinline__ void block_reduce_stats(Smem &s, int &ph, double &s1, double &s2, int &n_in, int &n_below) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5, set = ph & 1;
+    ++ph;
 #pragma unroll
     for (int o = 16; o; o >>= 1) {
+        s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+        s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+    }
+    n_in = __reduce_add_sync(0xffffffffu, n_in);
+    n_below = __reduce_add_sync(0xffffffffu, n_below);
+    if (lane == 0) { s.red_d[set][0][warp] = s1; s.red_d[set][1][warp] = s2; s.red_i[set][0][warp] = n_in; s.red_i[set][1][warp] = n_below; }
+    __syncthreads();
+    // lane l takes the partial of warp l & 15; a xor tree over 16 lanes (the same in both halves of every warp)
+    const int w = lane & 15;
+    s1 = w < nw ? s.red_d[set][0][w] : 0.0; s2 = w < nw ? s.red_d[set][1][w] : 0.0;
+    n_in = w < nw ? s.red_i[set][0][w] : 0; n_below = w < nw ? s.red_i[set][1][w] : 0;
+#pragma unroll
+    for (int o = 8; o; o >>= 1) {
         s1 += __shfl_xor_sync(0xffffffffu, s1, o);
         s2 += __shfl_xor_sync(0xffffffffu, s2, o);
         n_in += __shfl_xor_sync(0xffffffffu, n_in, o);
         n_below += __shfl_xor_sync(0xffffffffu, n_below, o);
     }
-    if (lane == 0) { s.red_d[0][warp] = s1; s.red_d[1][warp] = s2; s.red_i[0][warp] = n_in; s.red_i[1][warp] = n_below; }
-    __syncthreads();
-    if (warp == 0) {   // nw <= 16 partials: one more shuffle tree, in a fixed order
-        s1 = lane < nw ? s.red_d[0][lane] : 0.0; s2 = lane < nw ? s.red_d[1][lane] : 0.0;
-        n_in = lane < nw ? s.red_i[0][lane] : 0; n_below = lane < nw ? s.red_i[1][lane] : 0;
-#pragma unroll
-        for (int o = 8; o; o >>= 1) {
-            s1 += __shfl_xor_sync(0xffffffffu, s1, o);
-            s2 += __shfl_xor_sync(0xffffffffu, s2, o);
-            n_in += __shfl_xor_sync(0xffffffffu, n_in, o);
-            n_below += __shfl_xor_sync(0xffffffffu, n_below, o);
-        }
-        if (lane == 0) { s.red_d[0][0] = s1; s.red_d[1][0] = s2; s.red_i[0][0] = n_in; s.red_i[1][0] = n_below; }
-    }
-    __syncthreads();
-    s1 = s.red_d[0][0]; s2 = s.red_d[1][0]; n_in = s.red_i[0][0]; n_below = s.red_i[1][0];
-    __syncthreads();
 }
 
 template <bool MIN>
@@ -437,7 +477,7 @@ __device__ __forceinline__ void for_each_px(const MeshSrc &m, F f) {
 
 // ---- slow path: one CTA, general -------------------------------------------------------------------------
 // Leaves the final statistics of the survivors in med/mu/sd/n.
-__device__ __noinline__ void k1_slow_path(const MeshSrc &src, Smem &s, uint8_t *hist8, int n_tot, double k_c, int iters,
+__device__ __noinline__ void k1_slow_path(const MeshSrc &src, Smem &s, int &ph, uint8_t *hist8, int n_tot, double k_c, int iters,
                                           double &med, double &mu, double &sd, int &n_out) {
     const int tid = threadIdx.x, nt = blockDim.x;
     const SortArea srt = make_sort_area(hist8);
@@ -449,7 +489,7 @@ __device__ __noinline__ void k1_slow_path(const MeshSrc &src, Smem &s, uint8_t *
         int c = 0, z = 0;
         double z2 = 0;
         for_each_px(src, [&](float e) { t1 += (double)e; ++c; });
-        block_reduce_stats(s, t1, z2, c, z);
+        block_reduce_stats(s, ph, t1, z2, c, z);
         pivot = t1 / (double)n_tot;
     }
     double s1, s2;
@@ -457,7 +497,7 @@ __device__ __noinline__ void k1_slow_path(const MeshSrc &src, Smem &s, uint8_t *
         double t1 = 0, t2 = 0;
         int z0 = 0, z1 = 0;
         for_each_px(src, [&](float e) { const double d = (double)e - pivot; t1 += d; t2 = fma(d, d, t2); });
-        block_reduce_stats(s, t1, t2, z0, z1);
+        block_reduce_stats(s, ph, t1, t2, z0, z1);
         s1 = t1; s2 = t2;
     }
 
@@ -581,7 +621,7 @@ __device__ __noinline__ void k1_slow_path(const MeshSrc &src, Smem &s, uint8_t *
                 t2 = fma(d, d, t2);
             }
         });
-        block_reduce_stats(s, t1, t2, c_in, c_below);
+        block_reduce_stats(s, ph, t1, t2, c_in, c_below);
         if (c_in == n || c_in == 0) break;   // stable (A7) or would empty the set: keep the current statistics
         LO = lo; HI = hi;
         n = c_in; n_below = c_below; s1 = t1; s2 = t2;
@@ -590,8 +630,26 @@ __device__ __noinline__ void k1_slow_path(const MeshSrc &src, Smem &s, uint8_t *
     n_out = n;
 }
 
+// 8 x 8 lattice points x 4 consecutive pixels of the mesh rows [row0, row0 + rows), read from global memory by one warp,
+// sorted in its registers, left in samp[0..256).  Not inlined: its registers must not count against the sweeps'.
+__device__ __noinline__ void k1_sample_sort_warp(const float *mesh_ptr, int W, int row0, int rows, int vw, uint32_t *samp) {
+    const int lane = threadIdx.x & 31;
+    uint32_t xs[8];
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const int e = r * 32 + lane, pt = e >> 2, q = e & 3, i = pt >> 3, j = pt & 7;
+        const int y = row0 + ((2 * i + 1) * rows) / 16;
+        const int x = min((((2 * j + 1) * vw) / 16) & ~3, vw - 4) + q;
+        xs[r] = f32_to_key(__ldg(mesh_ptr + (size_t)y * W + x));
+    }
+    kw_sort256(xs, lane);
+#pragma unroll
+    for (int r = 0; r < 8; ++r) samp[lane * 8 + r] = xs[r];
+    __syncwarp();
+}
+
 // ---- the kernel ------------------------------------------------------------------------------------------
-template <int C>
+template <int C, bool LIST>
 #ifndef K1_MINB
 #define K1_MINB 2
 #endif
@@ -609,7 +667,12 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
     float *tail = reinterpret_cast<float *>(area);          // tail pixels (after the histogram)
 
     const unsigned rank = Team<C>::rank();
-    const int mesh = blockIdx.x / C;
+    int ph = 0;   // call counter of block_reduce_stats
+    unsigned it = blockIdx.x / C;
+    [[maybe_unused]] const unsigned n_work = LIST ? *a.list_count : 0u;
+    do {   // one pass, except in list mode (C == 1): grid-stride over the worklist
+    if constexpr (LIST) { if (it >= n_work) break; }
+    const int mesh = LIST ? (int)a.list[it] : (int)it;
     const int frame = mesh / (a.ny * a.nx);
     const int mj = (mesh / a.nx) % a.ny, mi = mesh % a.nx;
     const int y0 = mj * a.mh, x0 = mi * a.mw;
@@ -645,16 +708,20 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
     bool fast = a.allow_fast && n_tot >= K1_FAST_MIN_PX && vw >= 16;
     constexpr int M_S = 256, G_S = 8;   // 8 x 8 lattice points x 4 consecutive pixels
     if (fast && my_rows > 0) {
-        for (int e = tid; e < M_S; e += nt) {
-            const int pt = e >> 2, q = e & 3;
-            const int i = pt / G_S, j = pt - i * G_S;
-            const int y = row0 + ((2 * i + 1) * my_rows) / (2 * G_S);
-            const int x = min((((2 * j + 1) * vw) / (2 * G_S)) & ~3, vw - 4) + q;
-            samp[e] = f32_to_key(__ldg(mesh_ptr + (size_t)y * a.W + x));
+        if constexpr (C == 1) {   // one warp sorts the sample in registers: no block barrier (the CTA-wide bitonic sort
+            if (tid < 32) k1_sample_sort_warp(mesh_ptr, a.W, row0, my_rows, vw, samp);   // of 256 keys was 36 barriers, 8.5 k cycles)
+        } else {
+            for (int e = tid; e < M_S; e += nt) {
+                const int pt = e >> 2, q = e & 3;
+                const int i = pt / G_S, j = pt - i * G_S;
+                const int y = row0 + ((2 * i + 1) * my_rows) / (2 * G_S);
+                const int x = min((((2 * j + 1) * vw) / (2 * G_S)) & ~3, vw - 4) + q;
+                samp[e] = f32_to_key(__ldg(mesh_ptr + (size_t)y * a.W + x));
+            }
+            __syncthreads();
+            K1_T(0);
+            bitonic_sort(samp, M_S);
         }
-        __syncthreads();
-        K1_T(0);
-        bitonic_sort(samp, M_S);
         K1_T(1);
     }
     // sample quantiles, averaged over the team -> pivot, core interval [A, B], median bracket [ka, kb]
@@ -795,7 +862,7 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
         below = block_reduce_u32<false>(s, below);
         {
             int ct = c_tail;
-            block_reduce_stats(s, t1, t2, c_core, ct);
+            block_reduce_stats(s, ph, t1, t2, c_core, ct);
             if (tid == 0) { s.xch.s1 = t1; s.xch.s2 = t2; s.xch.n_core = c_core; s.xch.n_tail = ct; s.xch.below = below; }
         }
         K1_T(4);
@@ -883,7 +950,8 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
             K1_T(8);
             sort_candidates(s, s.list, m_tot, kga, gspan, srt);
             K1_T(9);
-            // ---- clipping rounds on the tail list --------------------------------------------------------
+            // ---- clipping rounds on the tail list (all warps: with two CTAs per SM a round run by one warp alone leaves the
+            //      SM idle -- measured 0.51 ms against 0.33 ms; one barrier per round, see block_reduce_stats) ------------
             const double A_d = (double)A_f, B_d = (double)B_f;
             auto tail_stats = [&](double lo, double hi, double &q1, double &q2, int &c_in, int &c_below) {
                 q1 = 0; q2 = 0; c_in = 0; c_below = 0;
@@ -897,7 +965,7 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
                         q2 = fma(d, d, q2);
                     }
                 }
-                block_reduce_stats(s, q1, q2, c_in, c_below);
+                block_reduce_stats(s, ph, q1, q2, c_in, c_below);
             };
             double LO = -INFINITY, HI = INFINITY, q1, q2;
             int c_in, c_below;
@@ -954,7 +1022,7 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
         src.g = mesh_ptr; src.W = a.W; src.vh = vh; src.vw = vw;
         src.vec4 = (vw % 4 == 0) && (a.mw % 4 == 0) && (a.W % 4 == 0);
         __syncthreads();
-        k1_slow_path(src, s, hist8, n_tot, a.k_c, a.iters, med, mu, sd, n_final);
+        k1_slow_path(src, s, ph, hist8, n_tot, a.k_c, a.iters, med, mu, sd, n_final);
     }
 
     K1_T(10);
@@ -970,7 +1038,12 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
         if (a.mean) a.mean[mesh] = mu;
         if (a.n_kept) a.n_kept[mesh] = n_final;
     }
+    if constexpr (LIST) { __syncthreads(); it += gridDim.x; }   // the next mesh reuses the shared memory
+    else break;
+    } while (true);
 }
+
+#include "k1w_warp_mesh.cuh"
 
 }  // namespace
 
@@ -1004,7 +1077,7 @@ int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan) {
     //     the instructions being per-mesh overhead replicated in every CTA, and rank 0 finishing alone.)
     // (3) Otherwise: a cluster of 2..8 CTAs, each with a slab of rows (plain loader), slabs up to the opt-in limit.
     const size_t mesh_bytes = (size_t)mesh_h * mesh_w * sizeof(float);
-    if (mesh_bytes > soft && mesh_w % 4 == 0 && !getenv("BKGDET_K1_NOSTREAM")) {
+    if (mesh_bytes > soft && mesh_w % 4 == 0) {
         for (int threads = 512; threads <= 512; threads *= 2) {
             const size_t n_f4 = (size_t)mesh_h * (mesh_w / 4);
             size_t per_thread = (n_f4 + threads - 1) / threads * 4;
@@ -1057,11 +1130,12 @@ int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan) {
     return BD_EUNSUPPORTED;
 }
 
-template <int C>
-static cudaError_t k1_launch_c(const CUtensorMap &tmap, const K1Args &a, const K1Plan &plan, int n_mesh, cudaStream_t st) {
-    cudaError_t e = cudaFuncSetAttribute(k1_mesh_stats<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)plan.smem_bytes);
+template <int C, bool LIST = false>
+static cudaError_t k1_launch_c(const CUtensorMap &tmap, const K1Args &a, const K1Plan &plan, int n_ctas, cudaStream_t st) {
+    const int n_mesh = n_ctas;
+    cudaError_t e = cudaFuncSetAttribute(k1_mesh_stats<C, LIST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)plan.smem_bytes);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(k1_mesh_stats<C>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    e = cudaFuncSetAttribute(k1_mesh_stats<C, LIST>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)n_mesh * C);
@@ -1075,11 +1149,13 @@ static cudaError_t k1_launch_c(const CUtensorMap &tmap, const K1Args &a, const K
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = C > 1 ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, k1_mesh_stats<C>, tmap, a);
+    return cudaLaunchKernelEx(&cfg, k1_mesh_stats<C, LIST>, tmap, a);
 }
 
+size_t k1_workspace_bytes(int B, int ny, int nx) { return 256 + (size_t)B * ny * nx * sizeof(uint32_t); }
+
 int k1_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg_params *p, double *d_bkg_raw,
-              double *d_rms_raw, double *d_median, double *d_mean, int32_t *d_n_kept, cudaStream_t st) {
+              double *d_rms_raw, double *d_median, double *d_mean, int32_t *d_n_kept, void *d_ws, cudaStream_t st) {
     K1Plan plan;
     int rc = k1_plan(ctx, p->mesh_h, p->mesh_w, &plan);
     if (rc != BD_OK) return bd_set_error(ctx, rc, "mesh %dx%d is too large for the statistics kernel", p->mesh_h, p->mesh_w);
@@ -1092,6 +1168,47 @@ int k1_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg
     a.k_c = p->clip_sigma; a.iters = p->clip_iters; a.skew_guard = p->skew_guard;
     a.median_factor = p->median_factor; a.mean_factor = p->mean_factor;
     a.bkg_raw = d_bkg_raw; a.rms_raw = d_rms_raw; a.median = d_median; a.mean = d_mean; a.n_kept = d_n_kept;
+    a.list_count = nullptr; a.list = nullptr;
+    const int n_mesh = B * a.ny * a.nx;
+
+    // Small meshes (the paper's default 64x64 and anything else up to 4096 pixels with mesh_w % 4 == 0): one warp per mesh
+    // (k1w_warp_mesh.cuh); the meshes it cannot finish go through the general path of k1_mesh_stats<1> in list mode.
+    const bool warp_mode = a.allow_fast && p->mesh_w % 4 == 0 && (long long)p->mesh_h * p->mesh_w <= 4096 &&
+                           (long long)p->mesh_h * p->mesh_w >= KW_MIN_PX && p->mesh_w >= 16 && plan.cluster == 1 && d_ws;
+    if (warp_mode) {
+        K1WArgs w;
+        w.img = d_img; w.B = B; w.H = H; w.W = W; w.mh = a.mh; w.mw = a.mw; w.ny = a.ny; w.nx = a.nx;
+        w.use_tma = (ctx->encode_tiled && a.mw <= 256 && a.mh <= 256) ? 1 : 0;
+        w.k_c = a.k_c; w.iters = a.iters; w.skew_guard = a.skew_guard; w.median_factor = a.median_factor; w.mean_factor = a.mean_factor;
+        w.bkg_raw = d_bkg_raw; w.rms_raw = d_rms_raw; w.median = d_median; w.mean = d_mean; w.n_kept = d_n_kept;
+        w.fb_count = (uint32_t *)d_ws; w.fb_list = (uint32_t *)((char *)d_ws + 256);
+        CUtensorMap tm;
+        memset(&tm, 0, sizeof(tm));
+        if (w.use_tma) {
+            cuuint64_t dims[3] = {(cuuint64_t)W, (cuuint64_t)H, (cuuint64_t)B};
+            cuuint64_t strides[2] = {(cuuint64_t)W * sizeof(float), (cuuint64_t)W * H * sizeof(float)};
+            cuuint32_t box[3] = {(cuuint32_t)a.mw, (cuuint32_t)a.mh, 1};
+            cuuint32_t estr[3] = {1, 1, 1};
+            CUresult r = ctx->encode_tiled(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)d_img, dims, strides, box, estr,
+                                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                           CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) return bd_set_error(ctx, BD_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+        }
+        BD_CUDA_CHECK(ctx, cudaMemsetAsync(w.fb_count, 0, sizeof(uint32_t), st));
+        BD_CUDA_CHECK(ctx, cudaFuncSetAttribute(k1w_warp_mesh, cudaFuncAttributeMaxDynamicSharedMemorySize, KW_SMEM));
+        BD_CUDA_CHECK(ctx, cudaFuncSetAttribute(k1w_warp_mesh, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        k1w_warp_mesh<<<(unsigned)n_mesh, 32, KW_SMEM, st>>>(tm, w);
+        BD_CUDA_CHECK(ctx, cudaGetLastError());
+        // the leftovers: general path, slab filled by the plain loader, a few persistent CTAs over the worklist
+        a.allow_fast = 0; a.use_tma = 0;
+        a.list_count = w.fb_count; a.list = w.fb_list;
+        plan.use_tma = 0;
+        CUtensorMap none;
+        memset(&none, 0, sizeof(none));
+        const int n_ctas = n_mesh < ctx->num_sms * 2 ? n_mesh : ctx->num_sms * 2;
+        BD_CUDA_CHECK(ctx, (k1_launch_c<1, true>(none, a, plan, n_ctas, st)));
+        return BD_OK;
+    }
 
     CUtensorMap tmap;
     memset(&tmap, 0, sizeof(tmap));
@@ -1106,7 +1223,6 @@ int k1_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg
                                        CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return bd_set_error(ctx, BD_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
     }
-    const int n_mesh = B * a.ny * a.nx;
     cudaError_t e;
     switch (plan.cluster) {
         case 1: e = k1_launch_c<1>(tmap, a, plan, n_mesh, st); break;
