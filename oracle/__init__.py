@@ -82,6 +82,33 @@ def mesh_stats(img: np.ndarray, p: BkgParams):
     return dict(bkg=bkg, rms=rms, n_kept=nk, median=med, mean=mean, rounds=rounds)
 
 
+@dataclass
+class BkgXParams:
+    """Background variants (readings B1-B6): PAPER.md:67 (mask-defined regions, >= 100 pixels), :181 (iteration)."""
+    min_valid_px: int = 100          # B2: a mesh with fewer unmasked pixels is invalid          PAPER.md:67
+    grow: int = 1                    # B5: Chebyshev radius by which detections are grown before they are masked
+    max_masked_frac: float = 1.0     # B2: invalid if more than this fraction of the mesh is masked (1 = never)
+    max_reject_frac: float = 1.0     # B6: invalid if the clipping rejected more than this fraction (1 = never)
+
+
+def mesh_stats_masked(img: np.ndarray, bad: np.ndarray | None, p: BkgParams, xp: BkgXParams):
+    """O1 with a bad-pixel mask and the validity rules B1, B2, B6.  Invalid meshes hold NaN (n_kept 0)."""
+    img = np.ascontiguousarray(img, dtype=np.float32)
+    H, W = img.shape
+    if bad is not None:
+        bad = np.ascontiguousarray(bad, dtype=np.uint8)
+        assert bad.shape == img.shape
+    ny, nx = grid_shape(H, W, p.mesh_h, p.mesh_w)
+    bkg = np.empty((ny, nx)); rms = np.empty((ny, nx)); med = np.empty((ny, nx)); mean = np.empty((ny, nx))
+    nk = np.empty((ny, nx), dtype=np.int32); rounds = np.empty((ny, nx), dtype=np.int32); nv = np.empty((ny, nx), dtype=np.int32)
+    lib().o1_mesh_stats_masked(_p(img), _p(bad) if bad is not None else None, C.c_int(H), C.c_int(W), C.c_int(p.mesh_h),
+                               C.c_int(p.mesh_w), C.c_double(p.clip_sigma), C.c_int(p.clip_iters), C.c_double(p.median_factor),
+                               C.c_double(p.mean_factor), C.c_int(p.skew_guard), C.c_int(xp.min_valid_px),
+                               C.c_double(xp.max_masked_frac), C.c_double(xp.max_reject_frac), _p(bkg), _p(rms), _p(nk),
+                               _p(med), _p(mean), _p(rounds), _p(nv))
+    return dict(bkg=bkg, rms=rms, n_kept=nk, median=med, mean=mean, rounds=rounds, n_valid=nv)
+
+
 def grid_median(grid: np.ndarray, fh: int, fw: int) -> np.ndarray:
     """O2."""
     grid = np.ascontiguousarray(grid, dtype=np.float64)
