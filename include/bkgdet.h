@@ -193,6 +193,51 @@ int photometry(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H
                const int64_t *d_n_sources, int64_t cat_capacity, const bd_phot_params *p, bd_phot *d_phot,
                void *d_ws, size_t ws_bytes, void *cuda_stream);
 
+/* ---- background variants.  PAPER.md:67 ("This division can be based on either predefined masks
+ * generated by the Image Quality Assessment function or rectangular regions ... each sub-region containing at least 100
+ * pixels"), :181 ("We will iterate to remove background noises with the background estimation and removal function").
+ * Readings B1-B6:
+ *   B1  d_bad: uint8 [B,H,W], non-zero = excluded; masked pixels leave a mesh's multiset before the first clipping round;
+ *   B2  a mesh that keeps fewer than min_valid_px pixels, or of which more than max_masked_frac is masked, is INVALID;
+ *   B6  so is a mesh whose clipping rejected more than max_reject_frac of its valid pixels (a crowded mesh);
+ *   B3  an invalid cell of the mesh grids takes the median of the valid cells inside the smallest square window
+ *       (2r+1)^2, r = 1, 2, ..., truncated at the grid border, that holds one (both grids; 0 if no cell is valid);
+ *       then the median filter and the spline prefilter as in bkg_estimate;
+ *   B4  bkg_iterate: estimate with the caller's mask, threshold the subtracted frame at detect_k (the bkg_subtract
+ *       rule), grow the detections (B5: dilation by the (2 grow + 1)^2 square), OR them with the caller's mask,
+ *       estimate again -- n_iter re-estimations.
+ * With a mask every mesh takes the general path of kernel K1 (a sweep per clipping round). */
+typedef struct {
+    int32_t min_valid_px;     /* default 100 */
+    int32_t grow;             /* Chebyshev radius of the dilation of the detections, 0..3; default 1           B5 */
+    double max_masked_frac;   /* default 1.0 (never)                                                           B2 */
+    double max_reject_frac;   /* default 1.0 (never)                                                           B6 */
+} bd_bkgx_params;
+void bd_default_bkgx_params(bd_bkgx_params *px);
+
+/* a1 with the variants.  Outputs as bd_mesh_stats (invalid meshes: NaN, n_kept 0) plus d_n_valid (int32 [B,ny,nx], pixels
+ * left after masking; may be NULL).  d_bad may be NULL (validity rules only).  d_ws: bd_bkg_workspace_bytes(). */
+int bd_mesh_stats_masked(bd_ctx *ctx, const float *d_img, const uint8_t *d_bad, int B, int H, int W,
+                         const bd_bkg_params *p, const bd_bkgx_params *px, double *d_bkg_raw, double *d_rms_raw,
+                         double *d_median, double *d_mean, int32_t *d_n_kept, int32_t *d_n_valid, void *d_ws,
+                         size_t ws_bytes, void *cuda_stream);
+
+/* a1 + fill (B3) + a2.  Outputs as bkg_estimate plus d_valid_mesh (uint8 [B,ny,nx], 1 = the mesh was valid; may be NULL).
+ * d_ws / ws_bytes: at least bd_bkg_workspace_bytes(). */
+int bkg_estimate_masked(bd_ctx *ctx, const float *d_img, const uint8_t *d_bad, int B, int H, int W,
+                        const bd_bkg_params *p, const bd_bkgx_params *px, float *d_bkg_mesh, float *d_rms_mesh,
+                        double *d_bkg_coef, double *d_rms_coef, uint8_t *d_valid_mesh, void *d_ws, size_t ws_bytes,
+                        void *cuda_stream);
+
+/* B4.  d_bad0 may be NULL.  d_bad_out: uint8 [B,H,W], required: the exclusion mask the last estimate used (0/1).
+ * n_iter >= 0 (0 = bkg_estimate_masked with d_bad0; d_bad_out is then d_bad0 != 0, or zeros).
+ * d_ws / ws_bytes: at least bd_bkg_iterate_workspace_bytes(). */
+int bd_bkg_iterate_workspace_bytes(const bd_ctx *ctx, int B, int H, int W, const bd_bkg_params *p, size_t *bytes);
+int bkg_iterate(bd_ctx *ctx, const float *d_img, const uint8_t *d_bad0, int B, int H, int W, const bd_bkg_params *p,
+                const bd_bkgx_params *px, double detect_k, int n_iter, float *d_bkg_mesh, float *d_rms_mesh,
+                double *d_bkg_coef, double *d_rms_coef, uint8_t *d_valid_mesh, uint8_t *d_bad_out, void *d_ws,
+                size_t ws_bytes, void *cuda_stream);
+
 /* ---- whole chain from HOST buffers (pinned or pageable), synchronous. ----------------------------------
  * Copies h_img to the device, runs bkg_estimate -> bkg_subtract_detect, copies the
  * catalogue and the per-frame counts back, and waits.  Device buffers are cached in ctx between calls.

@@ -21,7 +21,8 @@ __all__ = ["BkgParams", "Context", "SOURCE_DTYPE", "bkg_estimate", "bkg_subtract
 EXPORTS = ["bd_create", "bd_destroy", "bd_last_error", "bd_default_bkg_params", "bd_grid_shape",
            "bd_bkg_workspace_bytes", "bd_detect_workspace_bytes", "bd_mesh_stats", "bd_grid_filter_spline",
            "bkg_estimate", "bkg_subtract", "detect_sources", "bkg_subtract_detect", "bd_default_phot_params", "bd_phot_workspace_bytes", "photometry",
-           "bd_run_host"]
+           "bd_run_host", "bd_default_bkgx_params", "bd_mesh_stats_masked", "bkg_estimate_masked",
+           "bd_bkg_iterate_workspace_bytes", "bkg_iterate"]
 DEBUG_EXPORTS = ["bd_debug_k1_slow_meshes", "bd_debug_k1_reasons", "bd_debug_k1_force_slow", "bd_debug_tile_kernel_events"]
 
 
@@ -54,6 +55,22 @@ class BkgParams:
     def c(self) -> _CParams:
         return _CParams(self.mesh_h, self.mesh_w, self.filt_h, self.filt_w, self.clip_sigma, self.clip_iters,
                         self.skew_guard, self.median_factor, self.mean_factor)
+
+
+class _CBkgXParams(C.Structure):
+    _fields_ = [("min_valid_px", C.c_int32), ("grow", C.c_int32), ("max_masked_frac", C.c_double), ("max_reject_frac", C.c_double)]
+
+
+@dataclass
+class BkgXParams:
+    """bd_bkgx_params: the background variants (readings B1-B6)."""
+    min_valid_px: int = 100
+    grow: int = 1
+    max_masked_frac: float = 1.0
+    max_reject_frac: float = 1.0
+
+    def c(self) -> _CBkgXParams:
+        return _CBkgXParams(self.min_valid_px, self.grow, self.max_masked_frac, self.max_reject_frac)
 
 
 _lib = None
@@ -205,6 +222,62 @@ def mesh_stats(ctx: Context, img: torch.Tensor, p: BkgParams):
                                     _ptr(out["median"]), _ptr(out["mean"]), _ptr(out["n_kept"]), _ptr(ws),
                                     C.c_size_t(ws.numel()), _stream(ctx)))
     return out
+
+
+def mesh_stats_masked(ctx: Context, img: torch.Tensor, bad: torch.Tensor | None, p: BkgParams, px: BkgXParams):
+    """a1 with a bad-pixel mask / validity rules (NEXT-3).  -> dict as mesh_stats plus n_valid; invalid meshes hold NaN."""
+    _chk(ctx, img, torch.float32, "img"); _chk(ctx, bad, torch.uint8, "bad", img.shape, optional=True)
+    B, H, W = img.shape
+    ny, nx = grid_shape(H, W, p.mesh_h, p.mesh_w)
+    dev = _dev(ctx)
+    out = {k: torch.empty((B, ny, nx), dtype=torch.float64, device=dev) for k in ("bkg", "rms", "median", "mean")}
+    out["n_kept"] = torch.empty((B, ny, nx), dtype=torch.int32, device=dev)
+    out["n_valid"] = torch.empty((B, ny, nx), dtype=torch.int32, device=dev)
+    cp, cx = p.c(), px.c()
+    ws = torch.empty(ctx.bkg_workspace_bytes(B, H, W, p), dtype=torch.uint8, device=dev)
+    ctx.check(ctx.lib.bd_mesh_stats_masked(ctx.h, _ptr(img), _ptr(bad), B, H, W, C.byref(cp), C.byref(cx), _ptr(out["bkg"]),
+                                           _ptr(out["rms"]), _ptr(out["median"]), _ptr(out["mean"]), _ptr(out["n_kept"]),
+                                           _ptr(out["n_valid"]), _ptr(ws), C.c_size_t(ws.numel()), _stream(ctx)))
+    return out
+
+
+def _grids(ctx, B, ny, nx):
+    dev = _dev(ctx)
+    bm = torch.empty((B, ny, nx), dtype=torch.float32, device=dev); rm = torch.empty_like(bm)
+    cb = torch.empty((B, ny, nx), dtype=torch.float64, device=dev); cr = torch.empty_like(cb)
+    return bm, rm, cb, cr, torch.empty((B, ny, nx), dtype=torch.uint8, device=dev)
+
+
+def bkg_estimate_masked(ctx: Context, img: torch.Tensor, bad: torch.Tensor | None, p: BkgParams, px: BkgXParams,
+                        ws: torch.Tensor | None = None):
+    """a1 + fill + a2 with the variants (NEXT-3).  -> (bkg_mesh, rms_mesh, bkg_coef, rms_coef, valid_mesh u8)."""
+    _chk(ctx, img, torch.float32, "img"); _chk(ctx, bad, torch.uint8, "bad", img.shape, optional=True)
+    B, H, W = img.shape
+    bm, rm, cb, cr, valid = _grids(ctx, B, *grid_shape(H, W, p.mesh_h, p.mesh_w))
+    if ws is None:
+        ws = torch.empty(ctx.bkg_workspace_bytes(B, H, W, p), dtype=torch.uint8, device=_dev(ctx))
+    cp, cx = p.c(), px.c()
+    ctx.check(ctx.lib.bkg_estimate_masked(ctx.h, _ptr(img), _ptr(bad), B, H, W, C.byref(cp), C.byref(cx), _ptr(bm), _ptr(rm),
+                                          _ptr(cb), _ptr(cr), _ptr(valid), _ptr(ws), C.c_size_t(ws.numel()), _stream(ctx)))
+    return bm, rm, cb, cr, valid
+
+
+def bkg_iterate(ctx: Context, img: torch.Tensor, bad0: torch.Tensor | None, p: BkgParams, px: BkgXParams, detect_k: float,
+                n_iter: int, ws: torch.Tensor | None = None):
+    """Iterated background estimation (NEXT-3, B4).  -> (bkg_mesh, rms_mesh, bkg_coef, rms_coef, valid_mesh, bad_out u8 [B,H,W])."""
+    _chk(ctx, img, torch.float32, "img"); _chk(ctx, bad0, torch.uint8, "bad0", img.shape, optional=True)
+    B, H, W = img.shape
+    bm, rm, cb, cr, valid = _grids(ctx, B, *grid_shape(H, W, p.mesh_h, p.mesh_w))
+    bad_out = torch.empty((B, H, W), dtype=torch.uint8, device=_dev(ctx))
+    cp, cx = p.c(), px.c()
+    if ws is None:
+        n = C.c_size_t()
+        ctx.check(ctx.lib.bd_bkg_iterate_workspace_bytes(ctx.h, B, H, W, C.byref(cp), C.byref(n)))
+        ws = torch.empty(n.value, dtype=torch.uint8, device=_dev(ctx))
+    ctx.check(ctx.lib.bkg_iterate(ctx.h, _ptr(img), _ptr(bad0), B, H, W, C.byref(cp), C.byref(cx), C.c_double(detect_k),
+                                  C.c_int(n_iter), _ptr(bm), _ptr(rm), _ptr(cb), _ptr(cr), _ptr(valid), _ptr(bad_out), _ptr(ws),
+                                  C.c_size_t(ws.numel()), _stream(ctx)))
+    return bm, rm, cb, cr, valid, bad_out
 
 
 def grid_filter_spline(ctx: Context, bkg_raw: torch.Tensor, rms_raw: torch.Tensor, filt_h: int, filt_w: int):

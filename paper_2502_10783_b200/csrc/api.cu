@@ -95,8 +95,8 @@ int bd_bkg_workspace_bytes(const bd_ctx *ctx, int B, int H, int W, const bd_bkg_
     if (!ctx || !p || !bytes || B <= 0 || H <= 0 || W <= 0 || p->mesh_h <= 0 || p->mesh_w <= 0) return BD_EINVAL;
     const int ny = (H + p->mesh_h - 1) / p->mesh_h, nx = (W + p->mesh_w - 1) / p->mesh_w;
     size_t cells = (size_t)B * ny * nx;
-    // raw bkg, raw rms, K2's scratch, K1's worklist
-    *bytes = 2 * bd_align_up(cells * sizeof(double), 256) + bd_align_up(2 * (size_t)B * k2_scratch_per_grid(ny, nx) * sizeof(double), 256) +
+    // raw bkg, raw rms, the two filled grids of the variants, K2's scratch, K1's worklist
+    *bytes = 4 * bd_align_up(cells * sizeof(double), 256) + bd_align_up(2 * (size_t)B * k2_scratch_per_grid(ny, nx) * sizeof(double), 256) +
              k1_workspace_bytes(B, ny, nx) + 512;
     return BD_OK;
 }
@@ -137,6 +137,29 @@ int bd_grid_filter_spline(bd_ctx *ctx, const double *d_bkg_raw, const double *d_
                      (double *)d_ws, (cudaStream_t)cuda_stream);
 }
 
+// a1 (+ fill of invalid cells when the variants are on) + a2, shared by bkg_estimate, bkg_estimate_masked, bkg_iterate
+static int estimate_impl(bd_ctx *ctx, const float *d_img, const uint8_t *d_bad, int B, int H, int W, const bd_bkg_params *p,
+                         const bd_bkgx_params *px, float *d_bkg_mesh, float *d_rms_mesh, double *d_bkg_coef, double *d_rms_coef,
+                         uint8_t *d_valid_mesh, void *d_ws, size_t ws_bytes, cudaStream_t st) {
+    size_t need = 0;
+    bd_bkg_workspace_bytes(ctx, B, H, W, p, &need);
+    if (ws_bytes < need) return bd_set_error(ctx, BD_EWORKSPACE, "bkg workspace: need %zu bytes, got %zu", need, ws_bytes);
+    const int ny = (H + p->mesh_h - 1) / p->mesh_h, nx = (W + p->mesh_w - 1) / p->mesh_w;
+    const size_t cells = (size_t)B * ny * nx, stride = bd_align_up(cells * sizeof(double), 256);
+    char *base = (char *)bd_align_up((size_t)d_ws, 256);
+    double *raw_b = (double *)base, *raw_r = (double *)(base + stride);
+    double *fill_b = (double *)(base + 2 * stride), *fill_r = (double *)(base + 3 * stride), *scratch = (double *)(base + 4 * stride);
+    void *k1_ws = base + 4 * stride + bd_align_up(2 * (size_t)B * k2_scratch_per_grid(ny, nx) * sizeof(double), 256);
+    int rc = k1_launch(ctx, d_img, B, H, W, p, raw_b, raw_r, nullptr, nullptr, nullptr, k1_ws, st, d_bad, px, nullptr);
+    if (rc) return rc;
+    if (d_bad || px) {
+        if ((rc = k2f_launch(ctx, raw_b, raw_r, B, ny, nx, fill_b, fill_r, d_valid_mesh, st))) return rc;
+        raw_b = fill_b; raw_r = fill_r;
+    }
+    return k2_launch(ctx, raw_b, raw_r, B, ny, nx, p->filt_h, p->filt_w, d_bkg_mesh, d_rms_mesh, d_bkg_coef, d_rms_coef,
+                     scratch, st);
+}
+
 int bkg_estimate(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg_params *p, float *d_bkg_mesh,
                  float *d_rms_mesh, double *d_bkg_coef, double *d_rms_coef, void *d_ws, size_t ws_bytes,
                  void *cuda_stream) {
@@ -146,19 +169,90 @@ int bkg_estimate(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_
     if ((rc = check_params(ctx, p))) return rc;
     if (!d_img || !aligned16(d_img)) return bd_set_error(ctx, BD_EINVAL, "d_img null or misaligned");
     if (!d_bkg_coef || !d_rms_coef || !d_ws) return bd_set_error(ctx, BD_EINVAL, "null coefficient or workspace pointer");
-    size_t need = 0;
-    bd_bkg_workspace_bytes(ctx, B, H, W, p, &need);
-    if (ws_bytes < need) return bd_set_error(ctx, BD_EWORKSPACE, "bkg workspace: need %zu bytes, got %zu", need, ws_bytes);
-    const int ny = (H + p->mesh_h - 1) / p->mesh_h, nx = (W + p->mesh_w - 1) / p->mesh_w;
-    const size_t cells = (size_t)B * ny * nx, stride = bd_align_up(cells * sizeof(double), 256);
-    char *base = (char *)bd_align_up((size_t)d_ws, 256);
-    double *raw_b = (double *)base, *raw_r = (double *)(base + stride), *scratch = (double *)(base + 2 * stride);
-    void *k1_ws = base + 2 * stride + bd_align_up(2 * (size_t)B * k2_scratch_per_grid(ny, nx) * sizeof(double), 256);
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    rc = k1_launch(ctx, d_img, B, H, W, p, raw_b, raw_r, nullptr, nullptr, nullptr, k1_ws, st);
+    return estimate_impl(ctx, d_img, nullptr, B, H, W, p, nullptr, d_bkg_mesh, d_rms_mesh, d_bkg_coef, d_rms_coef, nullptr, d_ws,
+                         ws_bytes, (cudaStream_t)cuda_stream);
+}
+
+// ---- background variants (NEXT-3) ------------------------------------------------------------------------------------------
+void bd_default_bkgx_params(bd_bkgx_params *px) {
+    if (!px) return;
+    px->min_valid_px = 100; px->grow = 1; px->max_masked_frac = 1.0; px->max_reject_frac = 1.0;
+}
+
+static int check_bkgx(bd_ctx *ctx, const bd_bkgx_params *px) {
+    if (!px) return bd_set_error(ctx, BD_EINVAL, "null variant params");
+    if (px->min_valid_px < 0 || px->grow < 0 || px->grow > 3 || !(px->max_masked_frac >= 0.0) || !(px->max_reject_frac >= 0.0))
+        return bd_set_error(ctx, BD_EINVAL, "variant params: min_valid_px >= 0, grow in 0..3, fractions >= 0 required");
+    return BD_OK;
+}
+
+int bd_mesh_stats_masked(bd_ctx *ctx, const float *d_img, const uint8_t *d_bad, int B, int H, int W, const bd_bkg_params *p,
+                         const bd_bkgx_params *px, double *d_bkg_raw, double *d_rms_raw, double *d_median, double *d_mean,
+                         int32_t *d_n_kept, int32_t *d_n_valid, void *d_ws, size_t ws_bytes, void *cuda_stream) {
+    int rc = check_frame(ctx, B, H, W);
     if (rc) return rc;
-    return k2_launch(ctx, raw_b, raw_r, B, ny, nx, p->filt_h, p->filt_w, d_bkg_mesh, d_rms_mesh, d_bkg_coef, d_rms_coef,
-                     scratch, st);
+    BD_BIND_DEVICE(ctx);
+    if ((rc = check_params(ctx, p))) return rc;
+    if ((rc = check_bkgx(ctx, px))) return rc;
+    if (!d_img || !aligned16(d_img) || !aligned16(d_bad)) return bd_set_error(ctx, BD_EINVAL, "d_img null, or d_img / d_bad misaligned");
+    const int ny = (H + p->mesh_h - 1) / p->mesh_h, nx = (W + p->mesh_w - 1) / p->mesh_w;
+    const size_t need = k1_workspace_bytes(B, ny, nx) + 256;
+    if (!d_ws || ws_bytes < need) return bd_set_error(ctx, BD_EWORKSPACE, "mesh statistics workspace: need %zu bytes, got %zu", need, ws_bytes);
+    return k1_launch(ctx, d_img, B, H, W, p, d_bkg_raw, d_rms_raw, d_median, d_mean, d_n_kept, (void *)bd_align_up((size_t)d_ws, 256),
+                     (cudaStream_t)cuda_stream, d_bad, px, d_n_valid);
+}
+
+int bkg_estimate_masked(bd_ctx *ctx, const float *d_img, const uint8_t *d_bad, int B, int H, int W, const bd_bkg_params *p,
+                        const bd_bkgx_params *px, float *d_bkg_mesh, float *d_rms_mesh, double *d_bkg_coef, double *d_rms_coef,
+                        uint8_t *d_valid_mesh, void *d_ws, size_t ws_bytes, void *cuda_stream) {
+    int rc = check_frame(ctx, B, H, W);
+    if (rc) return rc;
+    BD_BIND_DEVICE(ctx);
+    if ((rc = check_params(ctx, p))) return rc;
+    if ((rc = check_bkgx(ctx, px))) return rc;
+    if (!d_img || !aligned16(d_img) || !aligned16(d_bad)) return bd_set_error(ctx, BD_EINVAL, "d_img null, or d_img / d_bad misaligned");
+    if (!d_bkg_coef || !d_rms_coef || !d_ws) return bd_set_error(ctx, BD_EINVAL, "null coefficient or workspace pointer");
+    return estimate_impl(ctx, d_img, d_bad, B, H, W, p, px, d_bkg_mesh, d_rms_mesh, d_bkg_coef, d_rms_coef, d_valid_mesh, d_ws,
+                         ws_bytes, (cudaStream_t)cuda_stream);
+}
+
+int bd_bkg_iterate_workspace_bytes(const bd_ctx *ctx, int B, int H, int W, const bd_bkg_params *p, size_t *bytes) {
+    size_t b = 0;
+    int rc = bd_bkg_workspace_bytes(ctx, B, H, W, p, &b);
+    if (rc) return rc;
+    *bytes = bd_align_up(b, 256) + (size_t)B * H * W + 512;   // + the detection mask of one iteration
+    return BD_OK;
+}
+
+int bkg_iterate(bd_ctx *ctx, const float *d_img, const uint8_t *d_bad0, int B, int H, int W, const bd_bkg_params *p,
+                const bd_bkgx_params *px, double detect_k, int n_iter, float *d_bkg_mesh, float *d_rms_mesh, double *d_bkg_coef,
+                double *d_rms_coef, uint8_t *d_valid_mesh, uint8_t *d_bad_out, void *d_ws, size_t ws_bytes, void *cuda_stream) {
+    int rc = check_frame(ctx, B, H, W);
+    if (rc) return rc;
+    BD_BIND_DEVICE(ctx);
+    if ((rc = check_params(ctx, p))) return rc;
+    if ((rc = check_bkgx(ctx, px))) return rc;
+    if (!d_img || !aligned16(d_img) || !aligned16(d_bad0) || !d_bad_out || !aligned16(d_bad_out))
+        return bd_set_error(ctx, BD_EINVAL, "d_img / d_bad_out null, or a pointer misaligned");
+    if (!d_bkg_coef || !d_rms_coef || !d_ws) return bd_set_error(ctx, BD_EINVAL, "null coefficient or workspace pointer");
+    if (n_iter < 0 || (n_iter > 0 && !(detect_k > 0.0))) return bd_set_error(ctx, BD_EINVAL, "n_iter >= 0 and detect_k > 0 required");
+    size_t need = 0, ws_b = 0;
+    bd_bkg_iterate_workspace_bytes(ctx, B, H, W, p, &need);
+    bd_bkg_workspace_bytes(ctx, B, H, W, p, &ws_b);
+    if (ws_bytes < need) return bd_set_error(ctx, BD_EWORKSPACE, "iterate workspace: need %zu bytes, got %zu", need, ws_bytes);
+    char *base = (char *)bd_align_up((size_t)d_ws, 256);
+    uint8_t *det = (uint8_t *)(base + bd_align_up(ws_b, 256));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if ((rc = k7_dilate_or(ctx, nullptr, d_bad0, B, H, W, 0, d_bad_out, st))) return rc;   // bad_out = (bad0 != 0)
+    rc = estimate_impl(ctx, d_img, d_bad0 ? d_bad_out : nullptr, B, H, W, p, px, d_bkg_mesh, d_rms_mesh, d_bkg_coef, d_rms_coef,
+                       d_valid_mesh, base, ws_b, st);
+    for (int it = 0; it < n_iter && !rc; ++it) {
+        rc = k3_launch(ctx, d_img, B, H, W, p->mesh_h, p->mesh_w, d_bkg_coef, d_rms_coef, detect_k, nullptr, nullptr, nullptr, det, st);
+        if (!rc) rc = k7_dilate_or(ctx, det, d_bad0, B, H, W, px->grow, d_bad_out, st);
+        if (!rc) rc = estimate_impl(ctx, d_img, d_bad_out, B, H, W, p, px, d_bkg_mesh, d_rms_mesh, d_bkg_coef, d_rms_coef,
+                                    d_valid_mesh, base, ws_b, st);
+    }
+    return rc;
 }
 
 int bkg_subtract(bd_ctx *ctx, const float *d_img, int B, int H, int W, int mesh_h, int mesh_w, const double *d_bkg_coef,

@@ -70,8 +70,10 @@ struct K1Plan {
 int k1_plan(const bd_ctx *ctx, int mesh_h, int mesh_w, K1Plan *plan);
 // d_ws: k1_workspace_bytes() of device memory (the worklist of meshes the warp-per-mesh kernel hands to the general path)
 size_t k1_workspace_bytes(int B, int ny, int nx);
+// d_bad / px / d_n_valid: the background variants (bad-pixel mask, validity rules, valid-pixel counts); all may be null
 int k1_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg_params *p, double *d_bkg_raw,
-              double *d_rms_raw, double *d_median, double *d_mean, int32_t *d_n_kept, void *d_ws, cudaStream_t st);
+              double *d_rms_raw, double *d_median, double *d_mean, int32_t *d_n_kept, void *d_ws, cudaStream_t st,
+              const uint8_t *d_bad = nullptr, const bd_bkgx_params *px = nullptr, int32_t *d_n_valid = nullptr);
 
 // doubles of scratch K2 needs per (frame, grid): the Thomas factors of both directions
 static inline __host__ __device__ size_t k2_scratch_per_grid(int ny, int nx) { return 2 * ((size_t)ny + (size_t)nx); }
@@ -79,6 +81,15 @@ int k2_launch(bd_ctx *ctx, const double *d_bkg_raw, const double *d_rms_raw, int
               float *d_bkg_mesh, float *d_rms_mesh, double *d_bkg_coef, double *d_rms_coef, double *d_scratch,
               cudaStream_t st);
 
+// B3: invalid (NaN) cells filled from their valid neighbours; d_valid may be null
+int k2f_launch(bd_ctx *ctx, const double *d_bkg_raw, const double *d_rms_raw, int B, int ny, int nx, double *d_bkg_filled,
+               double *d_rms_filled, uint8_t *d_valid, cudaStream_t st);
+
+// B5: out = (bad0 != 0) | dilate(det, grow); det and bad0 may be null (zeros)
+int k7_dilate_or(bd_ctx *ctx, const uint8_t *d_det, const uint8_t *d_bad0, int B, int H, int W, int grow, uint8_t *d_out,
+                 cudaStream_t st);
+
+// d_sub may be null here (bkg_iterate wants the mask only)
 int k3_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, int mh, int mw, const double *d_bkg_coef,
               const double *d_rms_coef, double detect_k, float *d_sub, float *d_bkg, float *d_rms, uint8_t *d_mask,
               cudaStream_t st);

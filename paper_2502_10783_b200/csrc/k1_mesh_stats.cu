@@ -68,6 +68,11 @@ struct K1Args {
     double *bkg_raw, *rms_raw, *median, *mean;
     int32_t *n_kept;
     const uint32_t *list_count, *list;   // list mode (C == 1): the meshes to do are list[0 .. *list_count), grid-stride
+    // background variants (readings B1, B2, B6): bad-pixel mask [B,H,W] (non-zero = excluded) and the validity rules
+    const uint8_t *bad;
+    int min_valid;
+    double max_masked_frac, max_reject_frac;
+    int32_t *n_valid;
 };
 
 struct Xch {   // one CTA's contribution to the team-wide totals (peers read it through DSMEM)
@@ -433,6 +438,7 @@ struct MeshSrc {
     const float *g;      // else: top-left pixel of the mesh in global memory, row pitch W
     int W, vh, vw;
     bool vec4;           // rows of g are 16-byte aligned and vw % 4 == 0
+    const uint8_t *bad;  // non-null (then slab is null): mask of the mesh, same geometry as g; masked pixels are skipped
 };
 
 // Apply f(float) to every pixel of the mesh.  The assignment of pixels to threads is the same on every call
@@ -454,22 +460,35 @@ __device__ __forceinline__ void for_each_px(const MeshSrc &m, F f) {
             const int dr = nt / f4_row, dc = nt - dr * f4_row;
             for (int i0 = tid; i0 < n_f4; i0 += nt * 4) {
                 float4 v[4];
+                const float4 *pv[4];
                 int r = i0 / f4_row, c = i0 - r * f4_row;
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
-                    if (i0 + k * nt < n_f4) v[k] = __ldg(reinterpret_cast<const float4 *>(m.g + (size_t)r * m.W) + c);
+                    pv[k] = reinterpret_cast<const float4 *>(m.g + (size_t)r * m.W) + c;
+                    if (i0 + k * nt < n_f4) v[k] = __ldg(pv[k]);
                     r += dr; c += dc;
                     if (c >= f4_row) { c -= f4_row; ++r; }
                 }
 #pragma unroll
                 for (int k = 0; k < 4; ++k)
-                    if (i0 + k * nt < n_f4) { f(v[k].x); f(v[k].y); f(v[k].z); f(v[k].w); }
+                    if (i0 + k * nt < n_f4) {
+                        if (m.bad) {   // 4 mask bytes of the same 4 pixels (the mask has the frame's geometry)
+                            const size_t off = reinterpret_cast<const float *>(pv[k]) - m.g;
+                            const uint32_t mb = __ldg(reinterpret_cast<const uint32_t *>(m.bad + off));
+                            if (!(mb & 0x000000FFu)) f(v[k].x);
+                            if (!(mb & 0x0000FF00u)) f(v[k].y);
+                            if (!(mb & 0x00FF0000u)) f(v[k].z);
+                            if (!(mb & 0xFF000000u)) f(v[k].w);
+                        } else { f(v[k].x); f(v[k].y); f(v[k].z); f(v[k].w); }
+                    }
             }
         } else {
             const int lane = tid & 31, warp = tid >> 5, nw = nt >> 5;
             for (int r = warp; r < m.vh; r += nw) {
                 const float *row = m.g + (size_t)r * m.W;
-                for (int c = lane; c < m.vw; c += 32) f(__ldg(row + c));
+                const uint8_t *brow = m.bad ? m.bad + (size_t)r * m.W : nullptr;
+                for (int c = lane; c < m.vw; c += 32)
+                    if (!brow || !__ldg(brow + c)) f(__ldg(row + c));
             }
         }
     }
@@ -478,7 +497,7 @@ __device__ __forceinline__ void for_each_px(const MeshSrc &m, F f) {
 // ---- slow path: one CTA, general -------------------------------------------------------------------------
 // Leaves the final statistics of the survivors in med/mu/sd/n.
 __device__ __noinline__ void k1_slow_path(const MeshSrc &src, Smem &s, int &ph, uint8_t *hist8, int n_tot, double k_c, int iters,
-                                          double &med, double &mu, double &sd, int &n_out) {
+                                          double &med, double &mu, double &sd, int &n_out, int &n_valid_out) {
     const int tid = threadIdx.x, nt = blockDim.x;
     const SortArea srt = make_sort_area(hist8);
     const uint32_t listcap = k1_listcap();
@@ -490,8 +509,11 @@ __device__ __noinline__ void k1_slow_path(const MeshSrc &src, Smem &s, int &ph, 
         double z2 = 0;
         for_each_px(src, [&](float e) { t1 += (double)e; ++c; });
         block_reduce_stats(s, ph, t1, z2, c, z);
+        n_tot = c;   // with a bad-pixel mask: the pixels that are left (B1)
+        if (n_tot == 0) { n_out = 0; n_valid_out = 0; return; }
         pivot = t1 / (double)n_tot;
     }
+    n_valid_out = n_tot;
     double s1, s2;
     {
         double t1 = 0, t2 = 0;
@@ -688,7 +710,7 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
 #endif
 
     // ---- stage the slab ---------------------------------------------------------------------------------
-    const bool stream = C == 1 && a.stream;
+    const bool stream = C == 1 && (a.stream || a.bad);   // with a mask every sweep reads global memory (general path)
     const bool tma = a.use_tma && vw == a.mw && !stream;
     if (tma && tid == 0) {
         uint32_t bar = smem_u32(&s.mbar);
@@ -705,7 +727,7 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
     }
 
     // ---- lattice sample of this CTA's slab rows (read from global while the TMA load is in flight), sorted ---
-    bool fast = a.allow_fast && n_tot >= K1_FAST_MIN_PX && vw >= 16;
+    bool fast = a.allow_fast && !a.bad && n_tot >= K1_FAST_MIN_PX && vw >= 16;
     constexpr int M_S = 256, G_S = 8;   // 8 x 8 lattice points x 4 consecutive pixels
     if (fast && my_rows > 0) {
         if constexpr (C == 1) {   // one warp sorts the sample in registers: no block barrier (the CTA-wide bitonic sort
@@ -830,7 +852,7 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
     }
 
     double med = 0, mu = 0, sd = 0;
-    int n_final = n_tot;
+    int n_final = n_tot, n_valid = n_tot;
     bool done_fast = false;
     bool slab_dirty = false;   // the fast path reuses the slab for its sort arrays
 
@@ -1020,9 +1042,10 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
         src.slab = (C == 1 && !slab_dirty && !stream) ? slab : nullptr;
         src.n_slab = n_c;
         src.g = mesh_ptr; src.W = a.W; src.vh = vh; src.vw = vw;
+        src.bad = a.bad ? a.bad + (mesh_ptr - a.img) : nullptr;
         src.vec4 = (vw % 4 == 0) && (a.mw % 4 == 0) && (a.W % 4 == 0);
         __syncthreads();
-        k1_slow_path(src, s, ph, hist8, n_tot, a.k_c, a.iters, med, mu, sd, n_final);
+        k1_slow_path(src, s, ph, hist8, n_tot, a.k_c, a.iters, med, mu, sd, n_final, n_valid);
     }
 
     K1_T(10);
@@ -1032,11 +1055,19 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
             if (sd == 0.0) bkg = mu;
             else if (fabs(mu - med) / sd >= 0.3) bkg = med;
         }
+        // B2, B6: too few valid pixels, too much of the mesh masked, or too much of it rejected -> invalid (NaN)
+        const int n_px = vh * vw;
+        if (n_valid < 1 || n_valid < a.min_valid || (double)(n_px - n_valid) > a.max_masked_frac * (double)n_px ||
+            (double)(n_valid - n_final) > a.max_reject_frac * (double)n_valid) {
+            const double nan = __longlong_as_double(0x7FF8000000000000ll);
+            bkg = nan; sd = nan; med = nan; mu = nan; n_final = 0;
+        }
         if (a.bkg_raw) a.bkg_raw[mesh] = bkg;
         if (a.rms_raw) a.rms_raw[mesh] = sd;
         if (a.median) a.median[mesh] = med;
         if (a.mean) a.mean[mesh] = mu;
         if (a.n_kept) a.n_kept[mesh] = n_final;
+        if (a.n_valid) a.n_valid[mesh] = n_valid;
     }
     if constexpr (LIST) { __syncthreads(); it += gridDim.x; }   // the next mesh reuses the shared memory
     else break;
@@ -1155,7 +1186,8 @@ static cudaError_t k1_launch_c(const CUtensorMap &tmap, const K1Args &a, const K
 size_t k1_workspace_bytes(int B, int ny, int nx) { return 256 + (size_t)B * ny * nx * sizeof(uint32_t); }
 
 int k1_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg_params *p, double *d_bkg_raw,
-              double *d_rms_raw, double *d_median, double *d_mean, int32_t *d_n_kept, void *d_ws, cudaStream_t st) {
+              double *d_rms_raw, double *d_median, double *d_mean, int32_t *d_n_kept, void *d_ws, cudaStream_t st,
+              const uint8_t *d_bad, const bd_bkgx_params *px, int32_t *d_n_valid) {
     K1Plan plan;
     int rc = k1_plan(ctx, p->mesh_h, p->mesh_w, &plan);
     if (rc != BD_OK) return bd_set_error(ctx, rc, "mesh %dx%d is too large for the statistics kernel", p->mesh_h, p->mesh_w);
@@ -1169,11 +1201,17 @@ int k1_launch(bd_ctx *ctx, const float *d_img, int B, int H, int W, const bd_bkg
     a.median_factor = p->median_factor; a.mean_factor = p->mean_factor;
     a.bkg_raw = d_bkg_raw; a.rms_raw = d_rms_raw; a.median = d_median; a.mean = d_mean; a.n_kept = d_n_kept;
     a.list_count = nullptr; a.list = nullptr;
+    const bool variants = d_bad || px;   // mask or validity rules: every mesh takes the general path
+    a.bad = d_bad; a.n_valid = d_n_valid;
+    a.min_valid = px ? px->min_valid_px : 0;
+    a.max_masked_frac = px ? px->max_masked_frac : 1.0;
+    a.max_reject_frac = px ? px->max_reject_frac : 1.0;
+    if (d_bad) { a.allow_fast = 0; a.use_tma = 0; plan.use_tma = 0; }
     const int n_mesh = B * a.ny * a.nx;
 
     // Small meshes (the paper's default 64x64 and anything else up to 4096 pixels with mesh_w % 4 == 0): one warp per mesh
     // (k1w_warp_mesh.cuh); the meshes it cannot finish go through the general path of k1_mesh_stats<1> in list mode.
-    const bool warp_mode = a.allow_fast && p->mesh_w % 4 == 0 && (long long)p->mesh_h * p->mesh_w <= 4096 &&
+    const bool warp_mode = !variants && a.allow_fast && p->mesh_w % 4 == 0 && (long long)p->mesh_h * p->mesh_w <= 4096 &&
                            (long long)p->mesh_h * p->mesh_w >= KW_MIN_PX && p->mesh_w >= 16 && plan.cluster == 1 && d_ws;
     if (warp_mode) {
         K1WArgs w;

@@ -62,6 +62,61 @@ __global__ void __launch_bounds__(K2_NT) k2a_window_median(const double *bkg_raw
     }
 }
 
+// ---- K2f: invalid cells (NaN: background variants, reading B3) take the median of the VALID cells of the smallest square
+// window (2r+1)^2, r = 1, 2, ..., truncated at the grid border, that holds one; both grids, read from the unfilled grids.
+// One thread per cell: an invalid cell is rare and its window is a handful of cells (rank counting, as in K2a).
+__device__ double k2f_window_median(const double *g, const double *gv, int nx, int j0, int j1, int i0, int i1, int n) {
+    const int ww = i1 - i0 + 1, tot = (j1 - j0 + 1) * ww;
+    const int k_lo = (n - 1) / 2, k_hi = n / 2;
+    double lo = 0.0, hi = 0.0;
+    for (int a = 0; a < tot; ++a) {
+        const size_t ia = (size_t)(j0 + a / ww) * nx + i0 + a % ww;
+        if (isnan(gv[ia])) continue;
+        const double va = g[ia];
+        int rank = 0;
+        for (int b = 0; b < tot; ++b) {
+            const size_t ib = (size_t)(j0 + b / ww) * nx + i0 + b % ww;
+            if (isnan(gv[ib])) continue;
+            const double vb = g[ib];
+            rank += (vb < va || (vb == va && b < a)) ? 1 : 0;
+        }
+        if (rank == k_lo) lo = va;
+        if (rank == k_hi) hi = va;
+    }
+    return (n & 1) ? lo : 0.5 * (lo + hi);
+}
+__global__ void __launch_bounds__(K2_NT) k2f_fill_invalid(const double *bkg_raw, const double *rms_raw, int B, int ny, int nx,
+                                                          double *bkg_out, double *rms_out, uint8_t *valid) {
+    const long long idx = (long long)blockIdx.x * K2_NT + threadIdx.x;
+    const int cells = ny * nx;
+    if (idx >= (long long)B * cells) return;
+    const int c = (int)(idx % cells);
+    const size_t goff = (size_t)(idx / cells) * cells;
+    const double *gb = bkg_raw + goff, *gr = rms_raw + goff;
+    const double vb = gb[c];
+    if (!isnan(vb)) {
+        bkg_out[idx] = vb; rms_out[idx] = gr[c];
+        if (valid) valid[idx] = 1;
+        return;
+    }
+    if (valid) valid[idx] = 0;
+    const int j = c / nx, i = c - j * nx;
+    double fb = 0.0, fr = 0.0;
+    const int rmax = max(ny, nx);
+    for (int r = 1; r <= rmax; ++r) {
+        const int j0 = max(j - r, 0), j1 = min(j + r, ny - 1), i0 = max(i - r, 0), i1 = min(i + r, nx - 1);
+        int n = 0;
+        for (int jj = j0; jj <= j1; ++jj)
+            for (int ii = i0; ii <= i1; ++ii) n += isnan(gb[(size_t)jj * nx + ii]) ? 0 : 1;
+        if (n > 0) {
+            fb = k2f_window_median(gb, gb, nx, j0, j1, i0, i1, n);
+            fr = k2f_window_median(gr, gb, nx, j0, j1, i0, i1, n);
+            break;
+        }
+    }
+    bkg_out[idx] = fb; rms_out[idx] = fr;
+}
+
 // ---- K2b: cubic-B-spline prefilter ------------------------------------------------------------------------
 // Solve (c[k-1] + 4 c[k] + c[k+1]) / 6 = f[k], c[-1]=c[0], c[n]=c[n-1], along a strided line, in place
 // (Thomas algorithm; the matrix is strictly diagonally dominant).  cp[k], im[k] are the forward-sweep
@@ -131,6 +186,15 @@ __global__ void __launch_bounds__(K2_NT) k2b_spline_prefilter(int ny, int nx, do
 }
 
 }  // namespace
+
+int k2f_launch(bd_ctx *ctx, const double *d_bkg_raw, const double *d_rms_raw, int B, int ny, int nx, double *d_bkg_filled,
+               double *d_rms_filled, uint8_t *d_valid, cudaStream_t st) {
+    const long long n = (long long)B * ny * nx;
+    k2f_fill_invalid<<<(unsigned)((n + K2_NT - 1) / K2_NT), K2_NT, 0, st>>>(d_bkg_raw, d_rms_raw, B, ny, nx, d_bkg_filled,
+                                                                          d_rms_filled, d_valid);
+    BD_CUDA_CHECK(ctx, cudaGetLastError());
+    return BD_OK;
+}
 
 int k2_launch(bd_ctx *ctx, const double *d_bkg_raw, const double *d_rms_raw, int B, int ny, int nx, int fh, int fw,
               float *d_bkg_mesh, float *d_rms_mesh, double *d_bkg_coef, double *d_rms_coef, double *d_scratch,

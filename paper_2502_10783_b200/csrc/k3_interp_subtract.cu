@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(K3_NT, K3_MIN_CTAS) k3_interp_subtract(K3Args 
                 mbits |= (fg ? 1u : 0u) << (8 * q);
             }
             const size_t off = frame_off + (size_t)y * a.W + x0;
-            __stcs(reinterpret_cast<float4 *>(a.sub + off), make_float4(o_sub[0], o_sub[1], o_sub[2], o_sub[3]));
+            if (a.sub) __stcs(reinterpret_cast<float4 *>(a.sub + off), make_float4(o_sub[0], o_sub[1], o_sub[2], o_sub[3]));
             if (a.bkg) __stcs(reinterpret_cast<float4 *>(a.bkg + off), make_float4(o_bkg[0], o_bkg[1], o_bkg[2], o_bkg[3]));
             if (a.rms) __stcs(reinterpret_cast<float4 *>(a.rms + off), make_float4(o_rms[0], o_rms[1], o_rms[2], o_rms[3]));
             if (a.mask) __stcs(reinterpret_cast<uint32_t *>(a.mask + off), mbits);

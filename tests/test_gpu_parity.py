@@ -608,6 +608,129 @@ def test_k6_isolated_gaussian_and_errors(bd, ctx):
         bd.photometry(ctx, dev(sub), dev(rms), d_cat, n, 4, bd.PhotParams(subpix=0))
 
 
+# ------------------------------------------------------------------------------------------- NEXT-3: background variants
+from oracle import bkg_variants as obv  # noqa: E402
+
+
+def _bad_mask(rng, shape, frac, blobs=3):
+    bad = (rng.uniform(size=shape) < frac).astype(np.uint8) * 255         # any non-zero value masks
+    for _ in range(blobs):
+        y, x = int(rng.integers(0, shape[-2] - 40)), int(rng.integers(0, shape[-1] - 40))
+        bad[..., y:y + int(rng.integers(8, 80)), x:x + int(rng.integers(8, 80))] = 1
+    return bad
+
+
+def _cmp_masked_stats(out, st, f):
+    inv = np.isnan(st["bkg"])
+    assert np.array_equal(out["n_valid"][f].cpu().numpy(), st["n_valid"]) and np.array_equal(out["n_kept"][f].cpu().numpy(), st["n_kept"])
+    for k in ("bkg", "rms", "median", "mean"):
+        g = out[k][f].cpu().numpy()
+        assert np.array_equal(np.isnan(g), inv), f"{k}: invalid meshes differ"
+    assert np.array_equal(out["median"][f].cpu().numpy()[~inv], st["median"][~inv])
+    for k in ("mean", "rms", "bkg"):
+        g, w = out[k][f].cpu().numpy()[~inv], st[k][~inv]
+        tol = 1e-9 * np.maximum(np.abs(w), np.abs(st["median"][~inv])) + 1e-300
+        assert np.all(np.abs(g - w) <= tol), k
+    return int(inv.sum())
+
+
+@pytest.mark.parametrize("cid,H,W,mesh,frac", [(1, 512, 512, 64, 0.05), (3, 528, 768, 256, 0.2), (5, 384, 512, 64, 0.6), (2, 300, 340, 50, 0.1),
+                                                (4, 256, 320, 32, 0.3), (2, 384, 384, 128, 0.02)])
+def test_k1_masked_mesh_stats(bd, ctx, cid, H, W, mesh, frac):
+    """NEXT-3, B1/B2/B6: sigma-clipped statistics under a bad-pixel mask against the oracle: n_valid, n_kept, median and the
+    set of invalid meshes exact, sums 1e-9.  Slab, stream and cluster configurations of K1."""
+    cfg = CONFIGS[cid]
+    rng = np.random.default_rng(cid * 7 + mesh)
+    B = 2 if cid == 4 else 1
+    img = make_frames(cfg, H=H, W=W, B=B)
+    bad = _bad_mask(rng, img.shape, frac)
+    p = params_for(bd, cfg, mesh_h=mesh, mesh_w=mesh)
+    n_inv = 0
+    for kw in (dict(), dict(min_valid_px=int(0.5 * mesh * mesh)), dict(min_valid_px=1, max_masked_frac=0.3), dict(max_reject_frac=0.02)):
+        out = bd.mesh_stats_masked(ctx, dev(img), dev(bad), p, bd.BkgXParams(**kw))
+        torch.cuda.synchronize()
+        for f in range(B):
+            n_inv += _cmp_masked_stats(out, oracle.mesh_stats_masked(img[f], bad[f], to_oracle_params(p), oracle.BkgXParams(**kw)), f)
+    assert n_inv > 0 or frac < 0.05
+    # no mask, rules only: the fast paths stay on
+    out = bd.mesh_stats_masked(ctx, dev(img), None, p, bd.BkgXParams(max_reject_frac=0.01))
+    torch.cuda.synchronize()
+    for f in range(B):
+        _cmp_masked_stats(out, oracle.mesh_stats_masked(img[f], None, to_oracle_params(p), oracle.BkgXParams(max_reject_frac=0.01)), f)
+
+
+@pytest.mark.parametrize("cid,H,W,mesh", [(1, 512, 512, 64), (3, 1040, 1024, 256), (5, 512, 512, 32)])
+def test_bkg_estimate_masked_and_fill(bd, ctx, cid, H, W, mesh):
+    """NEXT-3, B3: whole meshes masked out -> filled from their valid neighbours, then the ordinary filter and spline."""
+    cfg = CONFIGS[cid]
+    rng = np.random.default_rng(cid)
+    img = make_frames(cfg, H=H, W=W, B=1)
+    bad = _bad_mask(rng, img.shape, 0.02, blobs=0)
+    bad[0, mesh:3 * mesh, mesh:2 * mesh] = 1            # two whole meshes, one above the other
+    bad[0, :mesh, -mesh:] = 1                           # a corner mesh
+    p = params_for(bd, cfg, mesh_h=mesh, mesh_w=mesh)
+    px = bd.BkgXParams()
+    bm, rm, cb, cr, valid = bd.bkg_estimate_masked(ctx, dev(img), dev(bad), p, px)
+    torch.cuda.synchronize()
+    b = obv.background_masked(img[0], bad[0], to_oracle_params(p), oracle.BkgXParams())
+    assert np.array_equal(valid[0].cpu().numpy(), b["valid"]) and (b["valid"] == 0).sum() >= 3
+    assert np.max(np.abs(bm[0].cpu().numpy() - b["bkg_grid"]) / np.abs(b["bkg_grid"])) < 1e-6
+    assert np.max(np.abs(rm[0].cpu().numpy() - b["rms_grid"]) / np.abs(b["rms_grid"])) < 1e-6
+    assert np.max(np.abs(cb[0].cpu().numpy() - b["bkg_coef"])) <= 1e-9 * np.max(np.abs(b["bkg_coef"]))
+    assert np.max(np.abs(cr[0].cpu().numpy() - b["rms_coef"])) <= 1e-9 * np.max(np.abs(b["rms_coef"]))
+    # everything masked: no valid cell, the grids are 0
+    allbad = np.ones_like(bad)
+    bm, rm, cb, cr, valid = bd.bkg_estimate_masked(ctx, dev(img), dev(allbad), p, px)
+    torch.cuda.synchronize()
+    assert int(valid.sum()) == 0 and float(bm.abs().max()) == 0.0 and float(cb.abs().max()) == 0.0
+
+
+def test_k7_dilate_or_exhaustive_window(bd, ctx):
+    """B5 through bkg_iterate's exclusion mask with n_iter = 0 / the dilation kernel against scipy-pinned oracle dilation:
+    every grow, frame edges, bad0 with arbitrary non-zero bytes."""
+    rng = np.random.default_rng(8)
+    img = rng.normal(100, 1, size=(2, 64, 96)).astype(np.float32)
+    bad0 = (rng.uniform(size=img.shape) < 0.05).astype(np.uint8) * 7
+    p = bd.BkgParams(mesh_h=32, mesh_w=32)
+    out = bd.bkg_iterate(ctx, dev(img), dev(bad0), p, bd.BkgXParams(min_valid_px=1), 1.5, 0)
+    torch.cuda.synchronize()
+    assert np.array_equal(out[5].cpu().numpy(), (bad0 != 0).astype(np.uint8))
+    out = bd.bkg_iterate(ctx, dev(img), None, p, bd.BkgXParams(), 1.5, 0)
+    assert int(out[5].sum()) == 0
+
+
+@pytest.mark.parametrize("cid,H,W,mesh,grow,n_iter", [(1, 512, 512, 64, 1, 1), (3, 528, 768, 256, 2, 2), (5, 384, 512, 64, 0, 1), (2, 300, 340, 50, 3, 1)])
+def test_bkg_iterate_stage_parity(bd, ctx, cid, H, W, mesh, grow, n_iter):
+    """NEXT-3, B4.  The threshold inside the iteration is the library's float32 rule, the oracle's is float64:
+    masks may differ on fragile pixels, so the comparison is stage-wise and exact: (i) with n_iter = 1 the exclusion mask
+    equals oracle.dilate(bkg_subtract's mask of the first estimate) | bad0; (ii) the final grids equal the oracle's masked
+    estimate under the library's own final exclusion mask; (iii) against the oracle's own iteration the exclusion masks
+    differ on at most a handful of pixels (those grown from fragile detections)."""
+    cfg = CONFIGS[cid]
+    rng = np.random.default_rng(cid + 40)
+    img = make_frames(cfg, H=H, W=W, B=1)
+    bad0 = _bad_mask(rng, img.shape, 0.01, blobs=1)
+    p = params_for(bd, cfg, mesh_h=mesh, mesh_w=mesh)
+    px, opx = bd.BkgXParams(grow=grow), oracle.BkgXParams(grow=grow)
+    d_img = dev(img)
+    bm, rm, cb, cr, valid, bad_out = bd.bkg_iterate(ctx, d_img, dev(bad0), p, px, cfg.detect_k, n_iter)
+    torch.cuda.synchronize()
+    bad_g = bad_out[0].cpu().numpy()
+    assert set(np.unique(bad_g)) <= {0, 1}
+    if n_iter == 1:
+        _, _, cb0, cr0, _ = bd.bkg_estimate_masked(ctx, d_img, dev(bad0), p, px)
+        m0 = bd.bkg_subtract(ctx, d_img, p.mesh_h, p.mesh_w, cb0, cr0, cfg.detect_k)["mask"][0].cpu().numpy()
+        assert np.array_equal(bad_g, obv.dilate(m0, grow) | (bad0[0] != 0))
+    b = obv.background_masked(img[0], bad_g, to_oracle_params(p), opx)
+    assert np.array_equal(valid[0].cpu().numpy(), b["valid"])
+    assert np.max(np.abs(bm[0].cpu().numpy() - b["bkg_grid"]) / np.abs(b["bkg_grid"])) < 1e-6
+    assert np.max(np.abs(cb[0].cpu().numpy() - b["bkg_coef"])) <= 1e-9 * np.max(np.abs(b["bkg_coef"]))
+    assert np.max(np.abs(cr[0].cpu().numpy() - b["rms_coef"])) <= 1e-9 * np.max(np.abs(b["rms_coef"]))
+    ob, obad = obv.iterate(img[0], bad0[0], to_oracle_params(p), opx, cfg.detect_k, n_iter)
+    assert (obad != bad_g).sum() <= 1e-4 * bad_g.size
+    assert np.max(np.abs(bm[0].cpu().numpy() - ob["bkg_grid"]) / np.abs(ob["bkg_grid"])) < 1e-4
+
+
 # ------------------------------------------------------------------------------------------- errors
 def test_binding_rejects_bad_tensors(bd, ctx):
     """The binding marshals only what the C signatures describe: CUDA, right dtype, contiguous, right shape."""
