@@ -238,6 +238,35 @@ int bkg_iterate(bd_ctx *ctx, const float *d_img, const uint8_t *d_bad0, int B, i
                 double *d_bkg_coef, double *d_rms_coef, uint8_t *d_valid_mesh, uint8_t *d_bad_out, void *d_ws,
                 size_t ws_bytes, void *cuda_stream);
 
+/* ---- stamp-wise spatially varying convolution of the template + image subtraction (kernel K8).
+ * eq. 8 K(u,v) = sum_n a_n(x,y) K_n(u,v); eq. 9 K_n = exp(-(u^2+v^2)/(2 sigma_k^2)) u^i v^j, i + j <= degree;
+ * eq. 10 R (x) K = I + B; one stamp of the kernel size (21 x 21 by default) per thread block with a preloaded kernel.
+ * The kernel FIT is out of scope: the coefficients are inputs.  Readings C1-C7:
+ *   C1  basis order: Gaussian g = 0.., inside it (i, j) with i = 0..degree[g], j = 0..degree[g] - i;
+ *   C2  a_n(x,y) = sum_t kcoef[n][t] xh^p yh^q, t over p = 0..spatial_order, q = 0..spatial_order - p,
+ *       xh = (2x - (W-1))/W, yh = (2y - (H-1))/H;  B(x,y) likewise from bgcoef with bg_order;
+ *   C3  stamps of S x S pixels (S = 2 half_width + 1) from the top-left corner; a stamp's kernel is K at its nominal
+ *       centre (sx S + half_width, sy S + half_width), the same for all its pixels;
+ *   C4  conv(x,y) = sum_{u,v} K(u,v) R(x-u, y-v), R = 0 outside the frame;   C5  diff = I + B - conv, B at the pixel.
+ * d_ref, d_img: float32 [B,H,W]; d_kcoef: float64 [B][n_basis][n_sp]; d_bgcoef: float64 [B][n_bg]
+ * (n_sp = (so+1)(so+2)/2, n_bg likewise); d_diff: float32 [B,H,W]; d_conv: float32 [B,H,W] or NULL.
+ * Arithmetic: the kernels are built in float64 and rounded to float32; the 441-term sums are float32 FMAs.
+ * d_ws / ws_bytes: at least bd_subtract_workspace_bytes(). */
+typedef struct {
+    int32_t half_width;       /* 1..15; default 10 (21 x 21; the register-blocked kernel; others use a generic one) */
+    int32_t n_gauss;          /* 1..4; default 3 */
+    double sigma[4];          /* default 0.7, 1.5, 3.0 */
+    int32_t degree[4];        /* 0..8 each; default 6, 4, 2  -> 49 basis kernels */
+    int32_t spatial_order;    /* 0..4; default 2 */
+    int32_t bg_order;         /* 0..4; default 1 */
+} bd_conv_params;
+void bd_default_conv_params(bd_conv_params *p);
+int bd_conv_num_basis(const bd_conv_params *p);      /* n_basis, or a negative code */
+int bd_subtract_workspace_bytes(const bd_ctx *ctx, int B, const bd_conv_params *p, size_t *bytes);
+int image_subtract(bd_ctx *ctx, const float *d_ref, const float *d_img, int B, int H, int W, const bd_conv_params *p,
+                   const double *d_kcoef, const double *d_bgcoef, float *d_diff, float *d_conv, void *d_ws,
+                   size_t ws_bytes, void *cuda_stream);
+
 /* ---- whole chain from HOST buffers (pinned or pageable), synchronous. ----------------------------------
  * Copies h_img to the device, runs bkg_estimate -> bkg_subtract_detect, copies the
  * catalogue and the per-frame counts back, and waits.  Device buffers are cached in ctx between calls.

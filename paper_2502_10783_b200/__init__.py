@@ -22,7 +22,8 @@ EXPORTS = ["bd_create", "bd_destroy", "bd_last_error", "bd_default_bkg_params", 
            "bd_bkg_workspace_bytes", "bd_detect_workspace_bytes", "bd_mesh_stats", "bd_grid_filter_spline",
            "bkg_estimate", "bkg_subtract", "detect_sources", "bkg_subtract_detect", "bd_default_phot_params", "bd_phot_workspace_bytes", "photometry",
            "bd_run_host", "bd_default_bkgx_params", "bd_mesh_stats_masked", "bkg_estimate_masked",
-           "bd_bkg_iterate_workspace_bytes", "bkg_iterate"]
+           "bd_bkg_iterate_workspace_bytes", "bkg_iterate", "bd_default_conv_params", "bd_conv_num_basis",
+           "bd_subtract_workspace_bytes", "image_subtract"]
 DEBUG_EXPORTS = ["bd_debug_k1_slow_meshes", "bd_debug_k1_reasons", "bd_debug_k1_force_slow", "bd_debug_tile_kernel_events"]
 
 
@@ -374,6 +375,55 @@ def bkg_subtract_detect(ctx: Context, img: torch.Tensor, mesh_h: int, mesh_w: in
                                           _ptr(mask), _ptr(labels), _ptr(cat), C.c_int64(cat_capacity), _ptr(nsrc),
                                           _ptr(ws), C.c_size_t(ws.numel()), _stream(ctx)))
     return dict(sub=sub, bkg=bkg, rms=rms, mask=mask, labels=labels, cat=cat, n_sources=nsrc)
+
+
+class _CConvParams(C.Structure):
+    _fields_ = [("half_width", C.c_int32), ("n_gauss", C.c_int32), ("sigma", C.c_double * 4), ("degree", C.c_int32 * 4),
+                ("spatial_order", C.c_int32), ("bg_order", C.c_int32)]
+
+
+class ConvParams:
+    """bd_conv_params (NEXT-4): kernel half-width, Gaussian widths and polynomial degrees, spatial and background orders."""
+
+    def __init__(self, half_width=10, sigma=(0.7, 1.5, 3.0), degree=(6, 4, 2), spatial_order=2, bg_order=1):
+        assert len(sigma) == len(degree) <= 4
+        c = _CConvParams()
+        c.half_width, c.n_gauss, c.spatial_order, c.bg_order = half_width, len(sigma), spatial_order, bg_order
+        for g in range(4):
+            c.sigma[g] = sigma[g] if g < len(sigma) else 1.0
+            c.degree[g] = degree[g] if g < len(degree) else 0
+        self._c = c
+        self.half_width, self.sigma, self.degree, self.spatial_order, self.bg_order = half_width, tuple(sigma), tuple(degree), spatial_order, bg_order
+
+    @property
+    def n_basis(self):
+        return int(load_library().bd_conv_num_basis(C.byref(self._c)))
+
+    @property
+    def n_sp(self):
+        return (self.spatial_order + 1) * (self.spatial_order + 2) // 2
+
+    @property
+    def n_bg(self):
+        return (self.bg_order + 1) * (self.bg_order + 2) // 2
+
+
+def image_subtract(ctx: Context, ref: torch.Tensor, img: torch.Tensor, p: ConvParams, kcoef: torch.Tensor, bgcoef: torch.Tensor,
+                   want_conv: bool = False, out: dict | None = None):
+    """NEXT-4 (K8): diff = img + B - ref (x) K with one kernel per 21x21 stamp.  kcoef float64 [B, n_basis, n_sp], bgcoef
+    float64 [B, n_bg].  -> dict(diff, conv or None)."""
+    _chk(ctx, ref, torch.float32, "ref"); _chk(ctx, img, torch.float32, "img", ref.shape)
+    B, H, W = ref.shape
+    _chk(ctx, kcoef, torch.float64, "kcoef", (B, p.n_basis, p.n_sp)); _chk(ctx, bgcoef, torch.float64, "bgcoef", (B, p.n_bg))
+    o = out or {}
+    diff = o.get("diff") if o.get("diff") is not None else torch.empty_like(ref)
+    conv = (o.get("conv") if o.get("conv") is not None else torch.empty_like(ref)) if want_conv else None
+    n = C.c_size_t()
+    ctx.check(ctx.lib.bd_subtract_workspace_bytes(ctx.h, B, C.byref(p._c), C.byref(n)))
+    ws = o.get("ws") if o.get("ws") is not None else torch.empty(n.value, dtype=torch.uint8, device=_dev(ctx))
+    ctx.check(ctx.lib.image_subtract(ctx.h, _ptr(ref), _ptr(img), B, H, W, C.byref(p._c), _ptr(kcoef), _ptr(bgcoef), _ptr(diff),
+                                     _ptr(conv), _ptr(ws), C.c_size_t(ws.numel()), _stream(ctx)))
+    return dict(diff=diff, conv=conv)
 
 
 PHOT_DTYPE = np.dtype([("flux_aper", np.float64), ("fluxerr_aper", np.float64), ("area_aper", np.float64),

@@ -345,6 +345,40 @@ int photometry(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H
     return k6_launch(ctx, d_sub, d_rms, B, H, W, d_cat, d_n_sources, cat_capacity, p, d_phot, d_ws, ws_bytes, (cudaStream_t)cuda_stream);
 }
 
+// ---- stamp convolution + subtraction (NEXT-4) -----------------------------------------------------------------------------
+void bd_default_conv_params(bd_conv_params *p) {
+    if (!p) return;
+    memset(p, 0, sizeof(*p));
+    p->half_width = 10; p->n_gauss = 3;
+    p->sigma[0] = 0.7; p->sigma[1] = 1.5; p->sigma[2] = 3.0; p->sigma[3] = 1.0;
+    p->degree[0] = 6; p->degree[1] = 4; p->degree[2] = 2; p->degree[3] = 0;
+    p->spatial_order = 2; p->bg_order = 1;
+}
+
+int bd_conv_num_basis(const bd_conv_params *p) {
+    const int n = k8_num_basis(p);
+    return n < 0 ? BD_EINVAL : n;
+}
+
+int bd_subtract_workspace_bytes(const bd_ctx *ctx, int B, const bd_conv_params *p, size_t *bytes) {
+    if (!ctx || !bytes || B <= 0 || k8_num_basis(p) < 0) return BD_EINVAL;
+    *bytes = k8_workspace_bytes(B, p) + 256;
+    return BD_OK;
+}
+
+int image_subtract(bd_ctx *ctx, const float *d_ref, const float *d_img, int B, int H, int W, const bd_conv_params *p,
+                   const double *d_kcoef, const double *d_bgcoef, float *d_diff, float *d_conv, void *d_ws, size_t ws_bytes,
+                   void *cuda_stream) {
+    int rc = check_frame(ctx, B, H, W);
+    if (rc) return rc;
+    BD_BIND_DEVICE(ctx);
+    if (!d_ref || !d_img || !d_kcoef || !d_bgcoef || !d_diff || !d_ws) return bd_set_error(ctx, BD_EINVAL, "null pointer");
+    if (k8_num_basis(p) < 0) return bd_set_error(ctx, BD_EINVAL, "bad convolution parameters");
+    const size_t need = k8_workspace_bytes(B, p) + 256;
+    if (ws_bytes < need) return bd_set_error(ctx, BD_EWORKSPACE, "subtract workspace: need %zu bytes, got %zu", need, ws_bytes);
+    return k8_launch(ctx, d_ref, d_img, B, H, W, p, d_kcoef, d_bgcoef, d_diff, d_conv, d_ws, (cudaStream_t)cuda_stream);
+}
+
 int bd_run_host(bd_ctx *ctx, const float *h_img, int B, int H, int W, const bd_bkg_params *p, double detect_k,
                 int32_t min_area, bd_source *h_cat, int64_t cat_capacity, int64_t *h_n_sources) {
     int rc = check_frame(ctx, B, H, W);

@@ -114,6 +114,11 @@ int k6_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H,
               size_t ws_bytes, cudaStream_t st);
 size_t k6_workspace_bytes(int64_t cat_capacity);
 
+int k8_num_basis(const bd_conv_params *p);
+size_t k8_workspace_bytes(int B, const bd_conv_params *p);
+int k8_launch(bd_ctx *ctx, const float *d_ref, const float *d_img, int B, int H, int W, const bd_conv_params *p,
+              const double *d_kcoef, const double *d_bgcoef, float *d_diff, float *d_conv, void *d_ws, cudaStream_t st);
+
 // ---- small device helpers ------------------------------------------------------------------------------
 #ifdef __CUDACC__
 __device__ __forceinline__ uint32_t f32_to_key(float f) {   // order-preserving map float32 -> uint32

@@ -731,6 +731,88 @@ def test_bkg_iterate_stage_parity(bd, ctx, cid, H, W, mesh, grow, n_iter):
     assert np.max(np.abs(bm[0].cpu().numpy() - ob["bkg_grid"]) / np.abs(ob["bkg_grid"])) < 1e-4
 
 
+# ------------------------------------------------------------------------------------------- NEXT-4: stamp convolution (K8)
+from oracle import subtract as osub  # noqa: E402
+
+
+def _conv_case(rng, B, H, W, p):
+    """Template / science frames shaped like a survey frame (sky + noise + a few stars) and kernel coefficients of the size a
+    fit returns: a_0 ~ 1 on the narrow Gaussian, small higher-order and spatially varying terms."""
+    ref = rng.normal(500, 12, size=(B, H, W)).astype(np.float32)
+    for _ in range(max(4, H * W // 4000)):
+        f, y, x = int(rng.integers(0, B)), int(rng.integers(0, H)), int(rng.integers(0, W))
+        yy, xx = np.mgrid[max(0, y - 6):min(H, y + 7), max(0, x - 6):min(W, x + 7)]
+        ref[f, yy, xx] += (rng.uniform(200, 5000) * np.exp(-0.5 * ((yy - y) ** 2 + (xx - x) ** 2) / 1.5 ** 2)).astype(np.float32)
+    img = (ref * 1.03 + rng.normal(20, 12, size=ref.shape)).astype(np.float32)
+    kc = rng.normal(0, 0.02, size=(B, p.n_basis, p.n_sp))
+    kc[:, 0, 0] += 0.6
+    bc = rng.normal(0, 5, size=(B, p.n_bg))
+    return ref, img, kc, bc
+
+
+@pytest.mark.parametrize("H,W,B,kw", [(100, 132, 2, {}), (42, 128, 1, {}), (64, 64, 1, dict(spatial_order=0, bg_order=0)),
+                                      (75, 88, 2, dict(half_width=3, sigma=(0.8, 1.7), degree=(2, 1), spatial_order=1, bg_order=2)),
+                                      (40, 52, 1, dict(half_width=15, sigma=(2.0,), degree=(3,), spatial_order=3, bg_order=0))])
+def test_k8_stamp_convolution_against_oracle(bd, ctx, H, W, B, kw):
+    """NEXT-4: conv and diff of every pixel against the float64 oracle.  Tolerance: the taps are float32
+    roundings of float64 values and the 441-term sum is float32 FMA, so |d conv| <= eps32 * S^2/2 * sum|K| * max|R| in the
+    worst case; 3e-6 * sum|K| * max|R| is asserted (observed: a few 1e-7).  Partial stamps, frame edges (zero fill),
+    several frames with their own coefficients, the generic kernel for other half-widths."""
+    p = bd.ConvParams(**kw)
+    op = osub.ConvParams(half_width=p.half_width, sigma=p.sigma, degree=p.degree, spatial_order=p.spatial_order, bg_order=p.bg_order)
+    assert p.n_basis == osub.n_basis(op)
+    rng = np.random.default_rng(H * W + B)
+    ref, img, kc, bc = _conv_case(rng, B, H, W, p)
+    out = bd.image_subtract(ctx, dev(ref), dev(img), p, dev(kc), dev(bc), want_conv=True)
+    torch.cuda.synchronize()
+    S = 2 * p.half_width + 1
+    for f in range(B):
+        diff, conv = osub.subtract(ref[f], img[f], op, kc[f], bc[f])
+        tol = np.empty((H, W))
+        for sy in range((H + S - 1) // S):
+            for sx in range((W + S - 1) // S):
+                tol[sy * S:(sy + 1) * S, sx * S:(sx + 1) * S] = 3e-6 * np.abs(osub.stamp_kernel(op, kc[f], H, W, sx, sy)).sum() * np.abs(ref[f]).max()
+        e1 = np.abs(out["conv"][f].cpu().numpy() - conv)
+        e2 = np.abs(out["diff"][f].cpu().numpy() - diff)
+        assert np.all(e1 <= tol), f"conv: worst {np.max(e1 / tol):.2f} x tol"
+        assert np.all(e2 <= tol + 1e-6 * np.abs(diff) + 1e-4), f"diff: worst {np.max(e2 / (tol + 1e-4)):.2f} x tol"
+    o2 = bd.image_subtract(ctx, dev(ref), dev(img), p, dev(kc), dev(bc))
+    torch.cuda.synchronize()
+    assert o2["conv"] is None and torch.equal(o2["diff"], out["diff"])
+
+
+def test_k8_impulse_and_identity(bd, ctx):
+    """Properties through the GPU path alone: a delta template returns the stamp's kernel (orientation: convolution, not
+    correlation); a delta KERNEL (a_0 = 1 on a very narrow Gaussian) returns the template, so diff = I + B - R exactly."""
+    p = bd.ConvParams(sigma=(0.05,), degree=(1,), spatial_order=0, bg_order=0)          # exp(-1/(2*0.0025)) = 0: a delta
+    H = W = 64
+    rng = np.random.default_rng(3)
+    ref = rng.normal(100, 5, size=(1, H, W)).astype(np.float32); img = rng.normal(100, 5, size=(1, H, W)).astype(np.float32)
+    kc = np.zeros((1, 3, 1)); kc[0, 0, 0] = 1.0
+    out = bd.image_subtract(ctx, dev(ref), dev(img), p, dev(kc), dev(np.array([[2.0]])), want_conv=True)
+    torch.cuda.synchronize()
+    assert np.array_equal(out["conv"][0].cpu().numpy(), ref[0])
+    assert np.array_equal(out["diff"][0].cpu().numpy(), ((img[0].astype(np.float64) + 2.0) - ref[0].astype(np.float64)).astype(np.float32))
+    p = bd.ConvParams(sigma=(2.0,), degree=(1,), spatial_order=0, bg_order=0)
+    ref = np.zeros((1, H, W), np.float32); ref[0, 31, 31] = 1.0                               # centre of the middle stamp
+    for n, (i, j) in enumerate(osub.poly_terms(1)):
+        kc = np.zeros((1, 3, 1)); kc[0, n, 0] = 1.0
+        conv = bd.image_subtract(ctx, dev(ref), dev(ref), p, dev(kc), dev(np.zeros((1, 1))), want_conv=True)["conv"][0].cpu().numpy()
+        yy, xx = np.mgrid[21:42, 21:42] - 31
+        want = np.exp(-(xx ** 2 + yy ** 2) / 8.0) * xx ** i * yy ** j
+        assert np.allclose(conv[21:42, 21:42], want, rtol=2e-7, atol=1e-12), (i, j)
+
+
+def test_k8_errors(bd, ctx):
+    p = bd.ConvParams()
+    ref = torch.zeros((1, 64, 64), dtype=torch.float32, device="cuda")
+    with pytest.raises(bd.BkgdetError):
+        bd.image_subtract(ctx, ref, ref, p, torch.zeros((1, 48, 6), dtype=torch.float64, device="cuda"), torch.zeros((1, 3), dtype=torch.float64, device="cuda"))
+    with pytest.raises((bd.BkgdetError, AssertionError)):
+        bd.image_subtract(ctx, ref, ref, bd.ConvParams(half_width=20), torch.zeros((1, 49, 6), dtype=torch.float64, device="cuda"),
+                          torch.zeros((1, 3), dtype=torch.float64, device="cuda"))
+
+
 # ------------------------------------------------------------------------------------------- errors
 def test_binding_rejects_bad_tensors(bd, ctx):
     """The binding marshals only what the C signatures describe: CUDA, right dtype, contiguous, right shape."""
