@@ -193,6 +193,53 @@ int photometry(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H
                const int64_t *d_n_sources, int64_t cat_capacity, const bd_phot_params *p, bd_phot *d_phot,
                void *d_ws, size_t ws_bytes, void *cuda_stream);
 
+/* ---- multi-threshold deblending (kernel K9) and cleaning (kernel K10).
+ * PAPER.md:155 ("calculate multi-level deblending thresholds.  At each threshold level, the algorithm re-evaluates objects
+ * and splits them as necessary, constructing a binary tree structure rooted in the original source candidate ... traversed
+ * from bottom to top ... pruning"), :157 ("determine if the current object can be merged with any adjacent objects ...
+ * flagged as a false detection ... a parallel operation to remove the marked pixels").  The paper gives no constants and no
+ * formulas; readings D1-D12 restate the method it adapts:
+ *   D1  candidates = the records of detect_sources;  D2  levels t_i = t_0 q^i, t_0 = (float)detect_k * rms[peak pixel],
+ *       q = (peak / t_0)^(1/n_thresh) by repeated float64 square roots (n_thresh a power of two, 2..64);
+ *   D3  node of level i = an 8-connected component of {sub > t_i} inside the candidate with >= min_area pixels;
+ *   D4  significant = flux > min_cont * candidate flux;  D5  bottom-to-top pruning: a node splits when at least two of its
+ *       children are split or significant;  D6  one object: candidate unchanged;
+ *   D7  the other pixels join the object of their brightest assigned 8-neighbour, in synchronous rounds;
+ *   D8  label of an object = 1 + minimum raster index of its pixels; records as in detect_sources;
+ *   D9-D11  cleaning: object i is a false detection when a brighter object j (Moffat-like profile of index clean_param
+ *       fitted to j's flux, second moments, area and threshold) within clean_zone isophotal radii of j leaves
+ *       flux_i / npix_i - I_j(i) <= t_i;  D12  its pixels become 0 in the label map, its record leaves the catalogue.
+ * deblend_sources: d_labels (in/out) int32 [B,H,W] and d_cat_in / d_n_in from detect_sources (the first
+ * min(sum n_in, cap_in) records are the candidates; records cut off by cap_in are dropped).  d_cat_out: ascending
+ * (frame, label), the first min(n, cap_out) records; d_n_out int64 [B] true counts.  cap_out also bounds the number of NEW
+ * objects whose records can be formed: a candidate that cannot reserve its records still gets its new labels and is counted
+ * in d_n_out, so sum(d_n_out) > cap_out or missing records tell the caller to retry with more room.  d_cat_out must not
+ * alias d_cat_in.  Label maps are bit-reproducible; flux sums are float64 atomics (tree decisions within 1e-9 relative of
+ * the contrast limit may differ from the float64 definition).
+ * clean_sources: d_cat_in / d_n_in are a catalogue of d_labels (normally deblend_sources' output); d_flags (uint8
+ * [cap_in], may be NULL) receives 1 for every false detection.  Decisions use float64 pow(): pairs within 1e-9 relative of
+ * the limit may differ from the definition.
+ * d_ws / ws_bytes: at least bd_deblend_workspace_bytes() (about 42 bytes per pixel: the frame-sized arrays of the
+ * candidates too large for shared memory) / bd_clean_workspace_bytes(). */
+typedef struct {
+    int32_t n_thresh;         /* number of levels, a power of two in 2..64; default 32                      D2 */
+    int32_t pad;
+    double min_cont;          /* minimum contrast; default 0.005                                            D4 */
+    double clean_param;       /* index beta of the neighbour profile; default 1.0                          D10 */
+    double clean_zone;        /* reach of a neighbour in isophotal radii; default 4.0                      D11 */
+} bd_deblend_params;
+void bd_default_deblend_params(bd_deblend_params *p);
+int bd_deblend_workspace_bytes(const bd_ctx *ctx, int B, int H, int W, int64_t cap_in, int64_t cap_out, size_t *bytes);
+int deblend_sources(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H, int W, double detect_k,
+                    int32_t min_area, const bd_deblend_params *p, int32_t *d_labels, const bd_source *d_cat_in,
+                    const int64_t *d_n_in, int64_t cap_in, bd_source *d_cat_out, int64_t cap_out, int64_t *d_n_out,
+                    void *d_ws, size_t ws_bytes, void *cuda_stream);
+int bd_clean_workspace_bytes(const bd_ctx *ctx, int B, int H, int W, int64_t cap_in, size_t *bytes);
+int clean_sources(bd_ctx *ctx, const float *d_rms, int B, int H, int W, double detect_k, const bd_deblend_params *p,
+                  int32_t *d_labels, const bd_source *d_cat_in, const int64_t *d_n_in, int64_t cap_in,
+                  bd_source *d_cat_out, int64_t cap_out, int64_t *d_n_out, uint8_t *d_flags, void *d_ws,
+                  size_t ws_bytes, void *cuda_stream);
+
 /* ---- background variants.  PAPER.md:67 ("This division can be based on either predefined masks
  * generated by the Image Quality Assessment function or rectangular regions ... each sub-region containing at least 100
  * pixels"), :181 ("We will iterate to remove background noises with the background estimation and removal function").

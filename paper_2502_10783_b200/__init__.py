@@ -16,14 +16,15 @@ import torch
 from . import _build
 
 __all__ = ["BkgParams", "Context", "SOURCE_DTYPE", "bkg_estimate", "bkg_subtract", "detect_sources", "mesh_stats",
-           "grid_filter_spline", "bkg_subtract_detect", "photometry", "PhotParams", "PHOT_DTYPE", "run_host", "grid_shape", "load_library", "EXPORTS"]
+           "grid_filter_spline", "bkg_subtract_detect", "photometry", "PhotParams", "PHOT_DTYPE", "deblend_sources", "clean_sources", "DeblendParams", "run_host", "grid_shape", "load_library", "EXPORTS"]
 
 EXPORTS = ["bd_create", "bd_destroy", "bd_last_error", "bd_default_bkg_params", "bd_grid_shape",
            "bd_bkg_workspace_bytes", "bd_detect_workspace_bytes", "bd_mesh_stats", "bd_grid_filter_spline",
            "bkg_estimate", "bkg_subtract", "detect_sources", "bkg_subtract_detect", "bd_default_phot_params", "bd_phot_workspace_bytes", "photometry",
            "bd_run_host", "bd_default_bkgx_params", "bd_mesh_stats_masked", "bkg_estimate_masked",
            "bd_bkg_iterate_workspace_bytes", "bkg_iterate", "bd_default_conv_params", "bd_conv_num_basis",
-           "bd_subtract_workspace_bytes", "image_subtract"]
+           "bd_subtract_workspace_bytes", "image_subtract", "bd_default_deblend_params", "bd_deblend_workspace_bytes",
+           "deblend_sources", "bd_clean_workspace_bytes", "clean_sources"]
 DEBUG_EXPORTS = ["bd_debug_k1_slow_meshes", "bd_debug_k1_reasons", "bd_debug_k1_force_slow", "bd_debug_tile_kernel_events"]
 
 
@@ -470,6 +471,75 @@ def photometry(ctx: Context, sub: torch.Tensor, rms: torch.Tensor, cat: torch.Te
     ctx.check(ctx.lib.photometry(ctx.h, _ptr(sub), _ptr(rms), B, H, W, _ptr(cat), _ptr(n_sources), C.c_int64(cat_capacity),
                                  C.byref(p._c), _ptr(out), _ptr(ws), C.c_size_t(ws.numel()), _stream(ctx)))
     return out
+
+
+class _CDeblendParams(C.Structure):
+    _fields_ = [("n_thresh", C.c_int32), ("pad", C.c_int32), ("min_cont", C.c_double), ("clean_param", C.c_double),
+                ("clean_zone", C.c_double)]
+
+
+class DeblendParams:
+    """bd_deblend_params (defaults from bd_default_deblend_params)."""
+
+    def __init__(self, **kw):
+        c = _CDeblendParams()
+        load_library().bd_default_deblend_params(C.byref(c))
+        for k, v in kw.items():
+            if not hasattr(c, k):
+                raise TypeError(f"unknown deblending parameter {k}")
+            setattr(c, k, v)
+        self._c = c
+
+    def __getattr__(self, k):
+        return getattr(self._c, k)
+
+
+def deblend_sources(ctx: Context, sub: torch.Tensor, rms: torch.Tensor, labels: torch.Tensor, cat: torch.Tensor,
+                    n_sources: torch.Tensor, cat_capacity: int, detect_k: float, min_area: int,
+                    p: "DeblendParams | None" = None, out_capacity: int | None = None, ws: torch.Tensor | None = None):
+    """NEXT-1 (K9): multi-threshold deblending of the candidates.  `labels` is updated IN PLACE.
+    -> dict(labels, cat uint8 [out_capacity*88] (device), n_sources int64 [B])."""
+    _chk(ctx, sub, torch.float32, "sub")
+    B, H, W = sub.shape
+    _chk(ctx, rms, torch.float32, "rms", (B, H, W)); _chk(ctx, labels, torch.int32, "labels", (B, H, W))
+    _chk(ctx, cat, torch.uint8, "cat"); _chk(ctx, n_sources, torch.int64, "n_sources", (B,)); _chk(ctx, ws, torch.uint8, "ws", optional=True)
+    p = p or DeblendParams()
+    cap_out = cat_capacity if out_capacity is None else out_capacity
+    dev = _dev(ctx)
+    cat_out = torch.empty(max(cap_out, 1) * SOURCE_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+    n_out = torch.empty(B, dtype=torch.int64, device=dev)
+    if ws is None:
+        nb = C.c_size_t()
+        ctx.check(ctx.lib.bd_deblend_workspace_bytes(ctx.h, B, H, W, C.c_int64(cat_capacity), C.c_int64(cap_out), C.byref(nb)))
+        ws = torch.empty(nb.value, dtype=torch.uint8, device=dev)
+    ctx.check(ctx.lib.deblend_sources(ctx.h, _ptr(sub), _ptr(rms), B, H, W, C.c_double(detect_k), C.c_int32(min_area),
+                                      C.byref(p._c), _ptr(labels), _ptr(cat), _ptr(n_sources), C.c_int64(cat_capacity),
+                                      _ptr(cat_out), C.c_int64(cap_out), _ptr(n_out), _ptr(ws), C.c_size_t(ws.numel()),
+                                      _stream(ctx)))
+    return dict(labels=labels, cat=cat_out, n_sources=n_out)
+
+
+def clean_sources(ctx: Context, rms: torch.Tensor, labels: torch.Tensor, cat: torch.Tensor, n_sources: torch.Tensor,
+                  cat_capacity: int, detect_k: float, p: "DeblendParams | None" = None, ws: torch.Tensor | None = None):
+    """NEXT-1 (K10): cleaning.  `labels` is updated IN PLACE.
+    -> dict(labels, cat uint8 [cap*88] (device), n_sources int64 [B], flags uint8 [cap])."""
+    _chk(ctx, rms, torch.float32, "rms")
+    B, H, W = rms.shape
+    _chk(ctx, labels, torch.int32, "labels", (B, H, W)); _chk(ctx, cat, torch.uint8, "cat")
+    _chk(ctx, n_sources, torch.int64, "n_sources", (B,)); _chk(ctx, ws, torch.uint8, "ws", optional=True)
+    p = p or DeblendParams()
+    dev = _dev(ctx)
+    cat_out = torch.empty(max(cat_capacity, 1) * SOURCE_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+    n_out = torch.empty(B, dtype=torch.int64, device=dev)
+    flags = torch.zeros(max(cat_capacity, 1), dtype=torch.uint8, device=dev)
+    if ws is None:
+        nb = C.c_size_t()
+        ctx.check(ctx.lib.bd_clean_workspace_bytes(ctx.h, B, H, W, C.c_int64(cat_capacity), C.byref(nb)))
+        ws = torch.empty(nb.value, dtype=torch.uint8, device=dev)
+    ctx.check(ctx.lib.clean_sources(ctx.h, _ptr(rms), B, H, W, C.c_double(detect_k), C.byref(p._c), _ptr(labels), _ptr(cat),
+                                    _ptr(n_sources), C.c_int64(cat_capacity), _ptr(cat_out), C.c_int64(cat_capacity), _ptr(n_out),
+                                    _ptr(flags), _ptr(ws), C.c_size_t(ws.numel()), _stream(ctx)))
+    return dict(labels=labels, cat=cat_out, n_sources=n_out, flags=flags)
 
 
 def phot_to_numpy(phot: torch.Tensor, n_sources: torch.Tensor, cat_capacity: int) -> np.ndarray:

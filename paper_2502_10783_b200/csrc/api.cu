@@ -317,6 +317,66 @@ int bkg_subtract_detect(bd_ctx *ctx, const float *d_img, int B, int H, int W, in
                       ws_bytes, st, &fz);
 }
 
+// ---- NEXT-1: deblending and cleaning -------------------------------------------------------------------------
+void bd_default_deblend_params(bd_deblend_params *p) {
+    if (!p) return;
+    p->n_thresh = 32; p->pad = 0; p->min_cont = 0.005; p->clean_param = 1.0; p->clean_zone = 4.0;
+}
+
+static int check_deblend_params(bd_ctx *ctx, const bd_deblend_params *p) {
+    if (!p) return bd_set_error(ctx, BD_EINVAL, "null pointer");
+    if (p->n_thresh < 2 || p->n_thresh > 64 || (p->n_thresh & (p->n_thresh - 1)))
+        return bd_set_error(ctx, BD_EINVAL, "n_thresh must be a power of two in 2..64");
+    if (!(p->min_cont >= 0.0) || !(p->min_cont <= 1.0)) return bd_set_error(ctx, BD_EINVAL, "min_cont must be in [0, 1]");
+    if (!(p->clean_param > 0.0) || !(p->clean_param <= 64.0) || !(p->clean_zone > 0.0) || !(p->clean_zone <= 1024.0))
+        return bd_set_error(ctx, BD_EINVAL, "clean_param must be in (0, 64], clean_zone in (0, 1024]");
+    return BD_OK;
+}
+
+int bd_deblend_workspace_bytes(const bd_ctx *ctx, int B, int H, int W, int64_t cap_in, int64_t cap_out, size_t *bytes) {
+    if (!ctx || !bytes || B <= 0 || H <= 0 || W <= 0 || cap_in < 0 || cap_out < 0) return BD_EINVAL;
+    *bytes = k9_workspace_bytes(B, H, W, cap_in, cap_out);
+    return BD_OK;
+}
+
+int deblend_sources(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H, int W, double detect_k,
+                    int32_t min_area, const bd_deblend_params *p, int32_t *d_labels, const bd_source *d_cat_in,
+                    const int64_t *d_n_in, int64_t cap_in, bd_source *d_cat_out, int64_t cap_out, int64_t *d_n_out,
+                    void *d_ws, size_t ws_bytes, void *cuda_stream) {
+    int rc = check_frame(ctx, B, H, W);
+    if (rc) return rc;
+    BD_BIND_DEVICE(ctx);
+    if (!d_sub || !d_rms || !d_labels || !d_cat_in || !d_n_in || !d_n_out || !d_ws) return bd_set_error(ctx, BD_EINVAL, "null pointer");
+    if ((rc = check_deblend_params(ctx, p))) return rc;
+    if (cap_in < 0 || cap_out < 0 || (cap_out > 0 && !d_cat_out)) return bd_set_error(ctx, BD_EINVAL, "bad catalogue capacity");
+    if (!(detect_k > 0.0) || min_area < 1) return bd_set_error(ctx, BD_EINVAL, "detect_k must be positive, min_area >= 1");
+    if (d_cat_out == d_cat_in) return bd_set_error(ctx, BD_EINVAL, "d_cat_out must not alias d_cat_in");
+    return k9_launch(ctx, d_sub, d_rms, B, H, W, detect_k, min_area, p, d_labels, d_cat_in, d_n_in, cap_in, d_cat_out, cap_out,
+                     d_n_out, d_ws, ws_bytes, (cudaStream_t)cuda_stream);
+}
+
+int bd_clean_workspace_bytes(const bd_ctx *ctx, int B, int H, int W, int64_t cap_in, size_t *bytes) {
+    if (!ctx || !bytes || B <= 0 || H <= 0 || W <= 0 || cap_in < 0) return BD_EINVAL;
+    *bytes = k10_workspace_bytes(B, H, W, cap_in);
+    return BD_OK;
+}
+
+int clean_sources(bd_ctx *ctx, const float *d_rms, int B, int H, int W, double detect_k, const bd_deblend_params *p,
+                  int32_t *d_labels, const bd_source *d_cat_in, const int64_t *d_n_in, int64_t cap_in,
+                  bd_source *d_cat_out, int64_t cap_out, int64_t *d_n_out, uint8_t *d_flags, void *d_ws,
+                  size_t ws_bytes, void *cuda_stream) {
+    int rc = check_frame(ctx, B, H, W);
+    if (rc) return rc;
+    BD_BIND_DEVICE(ctx);
+    if (!d_rms || !d_labels || !d_cat_in || !d_n_in || !d_n_out || !d_ws) return bd_set_error(ctx, BD_EINVAL, "null pointer");
+    if ((rc = check_deblend_params(ctx, p))) return rc;
+    if (cap_in < 0 || cap_out < 0 || (cap_out > 0 && !d_cat_out)) return bd_set_error(ctx, BD_EINVAL, "bad catalogue capacity");
+    if (!(detect_k > 0.0)) return bd_set_error(ctx, BD_EINVAL, "detect_k must be positive");
+    if (d_cat_out == d_cat_in) return bd_set_error(ctx, BD_EINVAL, "d_cat_out must not alias d_cat_in");
+    return k10_launch(ctx, d_rms, B, H, W, detect_k, p, d_labels, d_cat_in, d_n_in, cap_in, d_cat_out, cap_out, d_n_out, d_flags,
+                      d_ws, ws_bytes, (cudaStream_t)cuda_stream);
+}
+
 int bd_phot_workspace_bytes(const bd_ctx *ctx, int64_t cat_capacity, size_t *bytes) {
     if (!ctx || !bytes || cat_capacity < 0) return BD_EINVAL;
     *bytes = k6_workspace_bytes(cat_capacity);

@@ -114,6 +114,15 @@ int k6_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H,
               size_t ws_bytes, cudaStream_t st);
 size_t k6_workspace_bytes(int64_t cat_capacity);
 
+size_t k9_workspace_bytes(int B, int H, int W, int64_t cap_in, int64_t cap_out);
+int k9_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H, int W, double detect_k, int min_area,
+              const bd_deblend_params *p, int32_t *d_labels, const bd_source *d_cat_in, const int64_t *d_n_in, int64_t cap_in,
+              bd_source *d_cat_out, int64_t cap_out, int64_t *d_n_out, void *d_ws, size_t ws_bytes, cudaStream_t st);
+size_t k10_workspace_bytes(int B, int H, int W, int64_t cap_in);
+int k10_launch(bd_ctx *ctx, const float *d_rms, int B, int H, int W, double detect_k, const bd_deblend_params *p, int32_t *d_labels,
+               const bd_source *d_cat_in, const int64_t *d_n_in, int64_t cap_in, bd_source *d_cat_out, int64_t cap_out,
+               int64_t *d_n_out, uint8_t *d_flags, void *d_ws, size_t ws_bytes, cudaStream_t st);
+
 int k8_num_basis(const bd_conv_params *p);
 size_t k8_workspace_bytes(int B, const bd_conv_params *p);
 int k8_launch(bd_ctx *ctx, const float *d_ref, const float *d_img, int B, int H, int W, const bd_conv_params *p,
