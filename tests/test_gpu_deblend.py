@@ -263,3 +263,80 @@ def test_k9_batch_and_capacity(bd, ctx):
     torch.cuda.synchronize()
     assert np.array_equal(tiny["labels"].cpu().numpy(), lab_g)
     assert np.array_equal(tiny["n_sources"].cpu().numpy(), n_out)
+
+
+# ------------------------------------------------------------------------------------------- full-size frames, sampled
+def _reach_bound(c, zone):
+    """A generous upper bound of the distance at which record j can satisfy the zone test of D11 (test-side selection
+    only: r_j^2 >= |d|^2 / (x2 + y2), so |d|^2 <= zone^2 rho^2 (x2 + y2) with rho^2 = npix / (pi sqrt(D)))."""
+    x2, y2 = c["x2"] + 1.0 / 12.0, c["y2"] + 1.0 / 12.0
+    D = np.maximum(c["x2"] * c["y2"] - c["xy"] ** 2, 1e-3)
+    return 1.05 * zone * np.sqrt(c["npix"] / (np.pi * np.sqrt(D)) * (x2 + y2)) + 2.0
+
+
+@pytest.mark.parametrize("cfgn", [3, 5])
+def test_k9_k10_full_size_sampled(bd, ctx, cfgn):
+    """BASELINE.json's full configs 3 and 5 in the launch configuration the bench uses: K9 on the whole frame; O10 on a
+    sample of the candidates (the 12 largest, which take the workspace tier, and 400 seeded random ones): their pixels and
+    records must agree.  K10 on the whole catalogue; O11 on the objects of a 768 x 768 window plus every object that can
+    reach into it."""
+    cfg = CONFIGS[cfgn]
+    img = make_frames(cfg)
+    B, H, W = img.shape
+    p = bd.BkgParams(mesh_h=cfg.mesh, mesh_w=cfg.mesh, filt_h=cfg.filt, filt_w=cfg.filt)
+    cap = 1 << 20
+    d_img = dev(img)
+    _, _, cb, cr = bd.bkg_estimate(ctx, d_img, p)
+    fz = bd.bkg_subtract_detect(ctx, d_img, p.mesh_h, p.mesh_w, cb, cr, cfg.detect_k, cfg.min_area, cap)
+    torch.cuda.synchronize()
+    sub, rms, labels = fz["sub"][0].cpu().numpy(), fz["rms"][0].cpu().numpy(), fz["labels"][0].cpu().numpy()
+    cat = bd.catalogue_to_numpy(fz["cat"], fz["n_sources"], cap)
+    assert len(cat) < cap
+    lab_d = fz["labels"].clone()
+    out = bd.deblend_sources(ctx, fz["sub"], fz["rms"], lab_d, fz["cat"], fz["n_sources"], cap, cfg.detect_k, cfg.min_area)
+    torch.cuda.synchronize()
+    lab_g = lab_d[0].cpu().numpy()
+    cat_g = bd.catalogue_to_numpy(out["cat"], out["n_sources"], cap)
+    assert len(cat_g) < cap and np.all(np.diff(cat_g["label"].astype(np.int64)) > 0)
+    assert np.array_equal(lab_g > 0, labels > 0)
+    rng = np.random.default_rng(cfgn)
+    big = np.argsort(cat["npix"])[-12:]
+    pick = np.unique(np.concatenate([big, rng.choice(len(cat), 400, replace=False)]))
+    only = cat["label"][pick]
+    lab_o, nobj, frag = odb.deblend(sub, rms, labels, as_oracle(cat), cfg.detect_k, cfg.min_area, odb.DeblendParams(), only=only)
+    solid = np.setdiff1d(only, frag)
+    sel = np.isin(labels, solid)
+    assert np.array_equal(lab_g[sel], lab_o[sel]), f"{(lab_g[sel] != lab_o[sel]).sum()} label mismatches"
+    assert sum(v > 1 for v in nobj.values()) >= 5
+    new_labels = np.unique(lab_o[sel])
+    cat_o = oracle.reduce_sources(lab_o, sub, cfg.min_area)
+    want = cat_o[np.isin(cat_o["label"], new_labels)]
+    got = cat_g[np.isin(cat_g["label"], new_labels)]
+    assert_catalogue_equal(got, want)
+    # untouched by K9: everything that is not a candidate's pixel
+    small_px = ~np.isin(labels, cat["label"])
+    assert np.array_equal(lab_g[small_px], labels[small_px])
+
+    # ---- K10 on the whole deblended catalogue; O11 on a window
+    lab_c = lab_d.clone()
+    cl = bd.clean_sources(ctx, fz["rms"], lab_c, out["cat"], out["n_sources"], cap, cfg.detect_k)
+    torch.cuda.synchronize()
+    flags_g = cl["flags"].cpu().numpy()[: len(cat_g)]
+    x0, y0, S = W // 2 - 384, H // 2 - 384, 768
+    inner = (cat_g["x"] >= x0) & (cat_g["x"] < x0 + S) & (cat_g["y"] >= y0) & (cat_g["y"] < y0 + S)
+    reach = _reach_bound(cat_g, 4.0)
+    dx = np.maximum(np.maximum(x0 - cat_g["x"], cat_g["x"] - (x0 + S)), 0.0)
+    dy = np.maximum(np.maximum(y0 - cat_g["y"], cat_g["y"] - (y0 + S)), 0.0)
+    near = np.hypot(dx, dy) <= reach
+    idx = np.flatnonzero(inner | near)
+    sub_cat = as_oracle(cat_g[idx])
+    flag_o, frag_o = odb.clean_flags(sub_cat, rms, cfg.detect_k, odb.DeblendParams())
+    chk = inner[idx] & (frag_o == 0)
+    assert np.array_equal(flags_g[idx][chk], flag_o[chk]), f"{(flags_g[idx][chk] != flag_o[chk]).sum()} clean flags differ"
+    assert flag_o[chk].sum() > 0
+    # survivors: order kept, records copied; erased pixels are exactly those of the flagged records
+    cat_c = bd.catalogue_to_numpy(cl["cat"], cl["n_sources"], cap)
+    assert np.array_equal(cat_c["label"], cat_g["label"][flags_g == 0])
+    lab_cg = lab_c[0].cpu().numpy()
+    gone = np.isin(lab_g, cat_g["label"][flags_g != 0])
+    assert not lab_cg[gone].any() and np.array_equal(lab_cg[~gone], lab_g[~gone])
