@@ -16,10 +16,14 @@ the "fused interpolate/subtract/threshold pass" BASELINE.json's 70 % target name
 With N > 1 (torchrun) every rank processes its own frame (frames are independent units: no data-path
 collective); value = all ranks' pixels / max-over-ranks time.
 `--impl reference` times the CPU oracle, as it stands, on a bounded crop of the same workload.
+The default run (config 3, N = 1) also reports, outside the timed region: `configs` -- the same step on configs 1, 2, 4, 5
+(inputs of configs 1-2 rotated through > 256 MB of distinct copies so that L2 cannot serve them), each with its own clock
+sample -- and `next_stages_ms` -- deblend_sources, clean_sources, photometry and image_subtract on config 3.
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import subprocess
@@ -41,9 +45,7 @@ CHAIN_BYTES_PER_PX = 30.0       # K1 4 + K3 17 + K4 5 + K5 4
 LAUNCHES_PER_STEP = 10          # K1, K2a, K2b, then bkg_subtract_detect: k_spline_tabs, k4a (fused), k4b, k5m, k5k, k5s, k5f
                                 # (+2 memsets, not counted)
 LAUNCHES_PER_STEP_UNFUSED = 10  # ... K3, then detect_sources: k4a, k4b, k5m, k5k, k5s, k5f
-TILE_TRAFFIC_NCU = 1.8018e9     # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused tile kernel on config 3
-                                # (351.2 MB + 1450.6 MB, profiles/r1_c_fused.md; algorithmic 22 B/px = 1.872 GB)
-K3_TRAFFIC_NCU = 1.3888e9       # same for k3_interp_subtract (340.4 MB + 1048.4 MB; algorithmic 17 B/px = 1.446 GB)
+TRAFFIC_FILE = os.path.join("profiles", "traffic.json")   # ncu DRAM bytes per launch + the hash of the sources they were measured on
 FALLBACK_HBM_GBS = 6650.0       # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 
 
@@ -117,7 +119,36 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.rows), "source": self.source}
 
 
-def run_reference(args, cfg):
+def source_hash(files):
+    h = hashlib.sha256()
+    for f in files:
+        with open(os.path.join(ROOT, "paper_2502_10783_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(kernel):
+    """DRAM bytes per launch from the committed ncu capture (profiles/traffic.json), or None when the kernel's sources have
+    changed since that capture."""
+    try:
+        with open(os.path.join(ROOT, TRAFFIC_FILE)) as f:
+            t = json.load(f)[kernel]
+        return float(t["dram_bytes_per_launch"]) if source_hash(t["sources"]) == t["source_sha256_16"] else None
+    except Exception:
+        return None
+
+
+def omp_threads(n):
+    """Thread count of the oracle's OpenMP loops (a libgomp call; the oracle itself is not touched)."""
+    import ctypes
+    try:
+        ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+        return True
+    except Exception:
+        return False
+
+
+def run_reference(args, cfg, threads=None):
     """CPU oracle, as it stands, on a bounded crop of the workload (host cores of this box)."""
     import oracle
     crop = min(cfg.H, args.ref_crop), min(cfg.W, args.ref_crop)
@@ -125,6 +156,9 @@ def run_reference(args, cfg):
     p = oracle.BkgParams(mesh_h=cfg.mesh, mesh_w=cfg.mesh, filt_h=cfg.filt, filt_w=cfg.filt, clip_sigma=cfg.clip_sigma,
                          clip_iters=cfg.clip_iters)
     oracle.build()
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    if threads is not None and omp_threads(threads):
+        cores = threads
     for _ in range(args.warmup_ref):
         oracle.chain(img, p, cfg.detect_k, cfg.min_area)
     t0 = time.perf_counter()
@@ -132,10 +166,138 @@ def run_reference(args, cfg):
     for _ in range(args.steps_ref):
         nsrc = len(oracle.chain(img, p, cfg.detect_k, cfg.min_area)["cat"])
     dt = (time.perf_counter() - t0) / args.steps_ref
-    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
     mpix = crop[0] * crop[1] / dt / 1e6
     return dict(value=mpix, unit="Mpix/s", cores=cores, kind="oracle", ms_per_step=dt * 1e3,
                 sample=f"top-left {crop[0]}x{crop[1]} crop of {cfg.name}, whole chain O1-O6, float64, {nsrc} sources")
+
+
+class Workload:
+    """One config resident on the device: buffers, the step functions, the timing of K steps."""
+
+    def __init__(self, bd, torch, ctx, cfg, img_h, cap, dev, rotate_bytes=0):
+        self.bd, self.torch, self.ctx, self.cfg, self.cap = bd, torch, ctx, cfg, cap
+        B, H, W = img_h.shape
+        self.B, self.H, self.W, self.npx = B, H, W, B * H * W
+        self.p = bd.BkgParams(mesh_h=cfg.mesh, mesh_w=cfg.mesh, filt_h=cfg.filt, filt_w=cfg.filt, clip_sigma=cfg.clip_sigma,
+                              clip_iters=cfg.clip_iters)
+        img = torch.from_numpy(img_h).to(dev)
+        # L2 honesty: inputs smaller than L2 are rotated through enough distinct copies that L2 cannot serve them
+        n_copies = 1 if self.npx * 4 >= rotate_bytes else int(-(-rotate_bytes // (self.npx * 4)))
+        self.imgs = [img] + [img.clone() for _ in range(n_copies - 1)]
+        self.k = 0
+        self.ws_b = torch.empty(ctx.bkg_workspace_bytes(B, H, W, self.p), dtype=torch.uint8, device=dev)
+        self.ws_d = torch.empty(ctx.detect_workspace_bytes(B, H, W, cap), dtype=torch.uint8, device=dev)
+        f32 = lambda: torch.empty((B, H, W), dtype=torch.float32, device=dev)  # noqa: E731
+        self.o3 = dict(sub=f32(), bkg=f32(), rms=f32(), mask=torch.empty((B, H, W), dtype=torch.uint8, device=dev))
+        self.o5 = dict(labels=torch.empty((B, H, W), dtype=torch.int32, device=dev),
+                       cat=torch.empty(cap * bd.SOURCE_DTYPE.itemsize, dtype=torch.uint8, device=dev),
+                       n_sources=torch.empty(B, dtype=torch.int64, device=dev))
+
+    def l2_note(self):
+        mb = self.npx * 4 / 1e6
+        if len(self.imgs) > 1:
+            return (f"input {mb:.0f} MB per step: rotated through {len(self.imgs)} distinct copies ({mb * len(self.imgs):.0f} MB > 2 x 126 MB L2), "
+                    "so no step finds its input in L2")
+        return f"input {mb:.0f} MB per step > 126 MB L2 (no flush needed)"
+
+    def next_img(self):
+        self.k = (self.k + 1) % len(self.imgs)
+        return self.imgs[self.k]
+
+    def step_unfused(self, ev=None):
+        bd, cfg, p, img = self.bd, self.cfg, self.p, self.next_img()
+        if ev: ev[0].record()
+        bm, rm, cb, cr = bd.bkg_estimate(self.ctx, img, p, ws=self.ws_b)
+        if ev: ev[1].record()
+        bd.bkg_subtract(self.ctx, img, p.mesh_h, p.mesh_w, cb, cr, cfg.detect_k, out=self.o3)
+        if ev: ev[2].record()
+        bd.detect_sources(self.ctx, self.o3["sub"], self.o3["rms"], self.o3["mask"], cfg.detect_k, cfg.min_area, self.cap, ws=self.ws_d,
+                          out=self.o5)
+        if ev: ev[3].record()
+
+    def step_fused(self, ev=None):
+        bd, cfg, p, img = self.bd, self.cfg, self.p, self.next_img()
+        if ev: ev[0].record()
+        bm, rm, cb, cr = bd.bkg_estimate(self.ctx, img, p, ws=self.ws_b)
+        if ev: ev[1].record()
+        o35 = dict(self.o3); o35.update(self.o5)
+        bd.bkg_subtract_detect(self.ctx, img, p.mesh_h, p.mesh_w, cb, cr, cfg.detect_k, cfg.min_area, self.cap, ws=self.ws_d, out=o35)
+        if ev: ev[2].record()
+        if ev: ev[3].record()
+
+    def timed(self, step, steps, warmup, barrier, local_rank):
+        """warmup untimed steps, then exactly `steps` steps between two events; clocks sampled during the timed region."""
+        torch = self.torch
+        for _ in range(max(warmup, 3)):
+            step()
+        barrier()
+        sampler = ClockSampler(local_rank); sampler.start()
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(steps)]
+        t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        t_start.record()
+        for k in range(steps):
+            step(evs[k])
+        t_end.record()
+        barrier()
+        sampler.stop_flag = True
+        sampler.join(timeout=2.0)
+        total_ms = t_start.elapsed_time(t_end)
+        stage_ms = [float(np.mean([e[i].elapsed_time(e[i + 1]) for e in evs])) for i in range(3)]
+        return total_ms, stage_ms, sampler.summary()
+
+    def tile_kernel_ms(self, step, ev_tile, n=5):
+        self.bd.tile_kernel_events(self.ctx, ev_tile[0], ev_tile[1])
+        out = []
+        for _ in range(n):
+            step(); self.torch.cuda.synchronize()
+            out.append(ev_tile[0].elapsed_time(ev_tile[1]))
+        self.bd.tile_kernel_events(self.ctx, None, None)
+        return float(np.mean(out))
+
+    def free(self):
+        for k in ("imgs", "ws_b", "ws_d", "o3", "o5"):
+            setattr(self, k, None)
+        self.torch.cuda.empty_cache()
+
+
+def time_next_stages(bd, torch, ctx, wl, reps=3):
+    """deblend_sources, clean_sources, photometry and image_subtract on the maps of the last step (outside the timed region)."""
+    cfg, cap = wl.cfg, wl.cap
+    sub, rms = wl.o3["sub"], wl.o3["rms"]
+    ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
+    lab0 = wl.o5["labels"].clone()
+    nb = bd.C.c_size_t()
+    ctx.check(ctx.lib.bd_deblend_workspace_bytes(ctx.h, wl.B, wl.H, wl.W, bd.C.c_int64(cap), bd.C.c_int64(cap), bd.C.byref(nb)))
+    ws = torch.empty(nb.value, dtype=torch.uint8, device=sub.device)
+    t = {"deblend_sources": [], "clean_sources": [], "photometry": [], "image_subtract": []}
+    counts = {}
+    cp = bd.ConvParams()
+    gen = torch.Generator(device=sub.device); gen.manual_seed(7)
+    kcoef = 1e-3 * torch.randn((wl.B, cp.n_basis, cp.n_sp), dtype=torch.float64, device=sub.device, generator=gen)
+    kcoef[:, 0, 0] = 1.0
+    bgcoef = torch.zeros((wl.B, cp.n_bg), dtype=torch.float64, device=sub.device)
+    diff = torch.empty_like(sub)
+    for _ in range(reps + 1):
+        lab = lab0.clone()
+        e = [ev() for _ in range(5)]
+        e[0].record()
+        d = bd.deblend_sources(ctx, sub, rms, lab, wl.o5["cat"], wl.o5["n_sources"], cap, cfg.detect_k, cfg.min_area, ws=ws)
+        e[1].record()
+        c = bd.clean_sources(ctx, rms, lab, d["cat"], d["n_sources"], cap, cfg.detect_k)
+        e[2].record()
+        bd.photometry(ctx, sub, rms, c["cat"], c["n_sources"], cap)
+        e[3].record()
+        bd.image_subtract(ctx, wl.imgs[0], wl.imgs[0], cp, kcoef, bgcoef, out=dict(diff=diff))
+        e[4].record()
+        torch.cuda.synchronize()
+        for i, k in enumerate(t):
+            t[k].append(e[i].elapsed_time(e[i + 1]))
+        counts = {"candidates": int(wl.o5["n_sources"].sum()), "deblended": int(d["n_sources"].sum()), "cleaned": int(c["n_sources"].sum())}
+    out = {k: float(np.mean(v[1:])) for k, v in t.items()}
+    out["objects"] = counts
+    out["image_subtract_gflops"] = 2.0 * 441 * wl.npx / (out["image_subtract"] * 1e-3) / 1e9
+    return out
 
 
 def main():
@@ -150,6 +312,7 @@ def main():
     ap.add_argument("--warmup-ref", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the other configs and the NEXT stages (default run only)")
     ap.add_argument("--unfused", action="store_true", help="time bkg_subtract + detect_sources instead of bkg_subtract_detect")
     ap.add_argument("--cat-capacity", type=int, default=1 << 20)
     args = ap.parse_args()
@@ -185,85 +348,37 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
-    # ---- workload: each rank its own frame batch (seed offset by rank) -------------------------------
-    from dataclasses import replace
-    my_cfg = replace(cfg, seed=shard.rank_seed(cfg.seed, rank)) if rank else cfg
-    img_h = make_frames(my_cfg)
-    B, H, W = img_h.shape
-    npx = B * H * W
-    p = bd.BkgParams(mesh_h=cfg.mesh, mesh_w=cfg.mesh, filt_h=cfg.filt, filt_w=cfg.filt, clip_sigma=cfg.clip_sigma,
-                     clip_iters=cfg.clip_iters)
-    ctx = bd.Context(local_rank)
-    dev = torch.device("cuda", local_rank)
-    img = torch.from_numpy(img_h).to(dev)
-    cap = args.cat_capacity
-    ws_b = torch.empty(ctx.bkg_workspace_bytes(B, H, W, p), dtype=torch.uint8, device=dev)
-    ws_d = torch.empty(ctx.detect_workspace_bytes(B, H, W, cap), dtype=torch.uint8, device=dev)
-    o3 = dict(sub=torch.empty((B, H, W), dtype=torch.float32, device=dev), bkg=torch.empty((B, H, W), dtype=torch.float32, device=dev),
-              rms=torch.empty((B, H, W), dtype=torch.float32, device=dev), mask=torch.empty((B, H, W), dtype=torch.uint8, device=dev))
-    o5 = dict(labels=torch.empty((B, H, W), dtype=torch.int32, device=dev),
-              cat=torch.empty(cap * bd.SOURCE_DTYPE.itemsize, dtype=torch.uint8, device=dev),
-              n_sources=torch.empty(B, dtype=torch.int64, device=dev))
-
-    ev_tile = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-    for e in ev_tile:
-        e.record()          # creates the handles
-
-    def step_unfused(ev=None):
-        if ev: ev[0].record()
-        bm, rm, cb, cr = bd.bkg_estimate(ctx, img, p, ws=ws_b)
-        if ev: ev[1].record()
-        bd.bkg_subtract(ctx, img, p.mesh_h, p.mesh_w, cb, cr, cfg.detect_k, out=o3)
-        if ev: ev[2].record()
-        bd.detect_sources(ctx, o3["sub"], o3["rms"], o3["mask"], cfg.detect_k, cfg.min_area, cap, ws=ws_d, out=o5)
-        if ev: ev[3].record()
-
-    def step_fused(ev=None):
-        if ev: ev[0].record()
-        bm, rm, cb, cr = bd.bkg_estimate(ctx, img, p, ws=ws_b)
-        if ev: ev[1].record()
-        o35 = dict(o3); o35.update(o5)
-        bd.bkg_subtract_detect(ctx, img, p.mesh_h, p.mesh_w, cb, cr, cfg.detect_k, cfg.min_area, cap, ws=ws_d, out=o35)
-        if ev: ev[2].record()
-        if ev: ev[3].record()
-
-    step = step_unfused if args.unfused else step_fused
-
     def barrier():
         if dist: dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
-        step()
-    barrier()
-    sampler = ClockSampler(local_rank); sampler.start()
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
-    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    t_start.record()
-    for k in range(args.steps):
-        step(evs[k])
-    t_end.record()
-    barrier()
-    sampler.stop_flag = True
-    total_ms = t_start.elapsed_time(t_end)
-    stage_ms = [float(np.mean([e[i].elapsed_time(e[i + 1]) for e in evs])) for i in range(3)]
+    # ---- workload: each rank its own frame batch (seed offset by rank) -------------------------------
+    from dataclasses import replace
+    my_cfg = replace(cfg, seed=shard.rank_seed(cfg.seed, rank)) if rank else cfg
+    img_h = make_frames(my_cfg)
+    ctx = bd.Context(local_rank)
+    dev = torch.device("cuda", local_rank)
+    cap = args.cat_capacity
+    ROTATE = 256 << 20
+    wl = Workload(bd, torch, ctx, cfg, img_h, cap, dev, rotate_bytes=ROTATE)
+    B, H, W, npx = wl.B, wl.H, wl.W, wl.npx
+    ev_tile = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    for e in ev_tile:
+        e.record()          # creates the handles
+    step = wl.step_unfused if args.unfused else wl.step_fused
+
+    total_ms, stage_ms, clocks = wl.timed(step, args.steps, args.warmup, barrier, local_rank)
     # outside the timed region: (i) the tile kernel alone (events recorded by the library around its launch),
     # (ii) the three calls one by one (bkg_subtract = the K3 pass alone, for the 17 B/px figure)
-    tile_ms = []
-    bd.tile_kernel_events(ctx, ev_tile[0], ev_tile[1])
-    for _ in range(5):
-        step(); torch.cuda.synchronize()
-        tile_ms.append(ev_tile[0].elapsed_time(ev_tile[1]))
-    bd.tile_kernel_events(ctx, None, None)
-    tile_ms = float(np.mean(tile_ms))
+    tile_ms = wl.tile_kernel_ms(step, ev_tile)
     ev_u = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(5)]
-    step_unfused(); torch.cuda.synchronize()
+    wl.step_unfused(); torch.cuda.synchronize()
     for k in range(5):
-        step_unfused(ev_u[k])
+        wl.step_unfused(ev_u[k])
     torch.cuda.synchronize()
     unfused_ms = [float(np.mean([e[i].elapsed_time(e[i + 1]) for e in ev_u])) for i in range(3)]
-    n_src = int(o5["n_sources"].sum().item())
+    step(); torch.cuda.synchronize()
+    n_src = int(wl.o5["n_sources"].sum().item())
     total_ms = shard.max_over_ranks(total_ms, dist, dev)
     ms_per_step = total_ms / args.steps
     value = shard.whole_job_value(shard.sum_over_ranks(npx, dist, dev), ms_per_step * 1e-3) / 1e6
@@ -275,26 +390,33 @@ def main():
         cat_h = np.empty(cap, dtype=bd.SOURCE_DTYPE)
         host_img = pinned.numpy()
         for _ in range(2):
-            bd.run_host(ctx, host_img, p, cfg.detect_k, cfg.min_area, cap, cat=cat_h)
+            bd.run_host(ctx, host_img, wl.p, cfg.detect_k, cfg.min_area, cap, cat=cat_h)
         barrier()
         n_e2e = max(3, min(args.steps, 10))
         t0 = time.perf_counter()
         for _ in range(n_e2e):
-            recs, nn = bd.run_host(ctx, host_img, p, cfg.detect_k, cfg.min_area, cap, cat=cat_h)
+            recs, nn = bd.run_host(ctx, host_img, wl.p, cfg.detect_k, cfg.min_area, cap, cat=cat_h)
         torch.cuda.synchronize()
         dt = (time.perf_counter() - t0) / n_e2e
         dt = shard.max_over_ranks(dt, dist, dev)
         e2e = {"value": world * npx / dt / 1e6, "unit": "Mpix/s", "h2d_bytes_per_step": int(npx * 4),
                "d2h_bytes_per_step": int(len(recs) * bd.SOURCE_DTYPE.itemsize + B * 8), "ms_per_step": dt * 1e3,
                "api": "bd_run_host (pinned host frame -> catalogue on host)"}
+        del pinned, host_img
 
     if rank != 0:
         if dist: dist.destroy_process_group()
         return
     peak, peak_src = measured_peak()
+
+    def chain_roofline(n_px, ms):
+        gbs = CHAIN_BYTES_PER_PX * n_px / (ms * 1e-3) / 1e9
+        return {"bytes_per_px": CHAIN_BYTES_PER_PX, "achieved_gbs": gbs, "frac_of_measured": gbs / peak, "frac_of_8000": gbs / 8000.0}
+
     k3_gbs = K3_BYTES_PER_PX * npx / (unfused_ms[1] * 1e-3) / 1e9
     tile_bpp = 5.0 if args.unfused else TILE_BYTES_PER_PX
     tile_gbs = tile_bpp * npx / (tile_ms * 1e-3) / 1e9
+    tile_traffic = ncu_traffic("k4a_tile_label<fused>") if not args.unfused and args.config == 3 else None
     line = {
         "metric": METRIC, "value": value, "unit": "Mpix/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32/f64",
@@ -302,29 +424,48 @@ def main():
         "config": {"workload": cfg.name, "B": B, "H": H, "W": W, "mesh": cfg.mesh, "filter": cfg.filt, "detect_k": cfg.detect_k,
                    "min_area": cfg.min_area, "sources_found": n_src, "parallelism": f"frames x{world} (no collective)",
                    "calls": "bkg_estimate + bkg_subtract + detect_sources" if args.unfused else "bkg_estimate + bkg_subtract_detect",
-                   "l2": "input 340 MB per step > 126 MB L2 (no flush needed)" if npx * 4 > 200e6 else "inputs smaller than L2: L2-warm"},
+                   "l2": wl.l2_note()},
         "stages_ms": ({"bkg_estimate": stage_ms[0], "bkg_subtract": stage_ms[1], "detect_sources": stage_ms[2]} if args.unfused else
                       {"bkg_estimate": stage_ms[0], "bkg_subtract_detect": stage_ms[1]}),
         "stages_ms_separate_calls": {"bkg_estimate": unfused_ms[0], "bkg_subtract": unfused_ms[1], "detect_sources": unfused_ms[2]},
-        "chain_roofline": {"bytes_per_px": CHAIN_BYTES_PER_PX, "achieved_gbs": CHAIN_BYTES_PER_PX * npx / (ms_per_step * 1e-3) / 1e9,
-                           "frac_of_measured": CHAIN_BYTES_PER_PX * npx / (ms_per_step * 1e-3) / 1e9 / peak,
-                           "frac_of_8000": CHAIN_BYTES_PER_PX * npx / (ms_per_step * 1e-3) / 1e9 / 8000.0},
+        "chain_roofline": chain_roofline(npx, ms_per_step),
         "roofline": {"kernel": "k4a_tile_label" + ("" if args.unfused else "<fused: a3 + a4 + partial sums of a5>"), "bound": "hbm",
                      "achieved": tile_gbs, "peak": peak, "unit": "GB/s", "frac": tile_gbs / peak, "frac_of_8000": tile_gbs / 8000.0,
-                     "traffic": TILE_TRAFFIC_NCU if not args.unfused and args.config == 3 else None, "peak_source": peak_src,
+                     "traffic": tile_traffic, "traffic_source": TRAFFIC_FILE if tile_traffic else None, "peak_source": peak_src,
                      "bytes_per_px": tile_bpp, "ms": tile_ms},
         "roofline_k3_pass": {"kernel": "k3_interp_subtract (bkg_subtract called alone)", "bound": "hbm", "achieved": k3_gbs, "peak": peak,
-                             "unit": "GB/s", "frac": k3_gbs / peak, "frac_of_8000": k3_gbs / 8000.0, "traffic": K3_TRAFFIC_NCU if args.config == 3 else None,
+                             "unit": "GB/s", "frac": k3_gbs / peak, "frac_of_8000": k3_gbs / 8000.0,
+                             "traffic": ncu_traffic("k3_interp_subtract") if args.config == 3 else None,
                              "bytes_per_px": K3_BYTES_PER_PX, "ms": unfused_ms[1]},
         "gpu_launches": (LAUNCHES_PER_STEP_UNFUSED if args.unfused else LAUNCHES_PER_STEP) * args.steps,
-        "clocks": sampler.summary(),
+        "clocks": clocks,
         "host": {"nproc": os.cpu_count()},
     }
     if e2e:
         line["e2e"] = e2e
+    extras = not args.no_extras and world == 1 and args.config == 3 and not args.unfused
+    if extras:
+        # SURVEY 8(f) stages on this config, then the other configs (parity-test cases; reported, not the headline)
+        line["next_stages_ms"] = time_next_stages(bd, torch, ctx, wl)
+        wl.free()
+        others = []
+        for c in (1, 2, 4, 5):
+            ocfg = CONFIGS[c]
+            owl = Workload(bd, torch, ctx, ocfg, make_frames(ocfg), cap, dev, rotate_bytes=ROTATE)
+            o_total, o_stage, o_clocks = owl.timed(owl.step_fused, 10, 3, barrier, local_rank)
+            o_tile = owl.tile_kernel_ms(owl.step_fused, ev_tile, n=3)
+            o_ms = o_total / 10
+            others.append({"workload": ocfg.name, "B": owl.B, "H": owl.H, "W": owl.W, "ms_per_step": o_ms, "value": owl.npx / (o_ms * 1e-3) / 1e6,
+                           "unit": "Mpix/s", "stages_ms": {"bkg_estimate": o_stage[0], "bkg_subtract_detect": o_stage[1]},
+                           "tile_kernel_ms": o_tile, "chain_roofline": chain_roofline(owl.npx, o_ms), "l2": owl.l2_note(),
+                           "sources_found": int(owl.o5["n_sources"].sum().item()), "clocks": o_clocks})
+            owl.free()
+        line["configs"] = others
     if not args.no_cpu_baseline and world == 1:
         r = run_reference(args, cfg)
         line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        r1 = run_reference(args, cfg, threads=1)
+        line["cpu_baseline"]["one_core"] = {"value": r1["value"], "unit": "Mpix/s", "cores": r1["cores"]}
     print(json.dumps(line))
     if dist: dist.destroy_process_group()
 
