@@ -13,7 +13,10 @@
 
 namespace {
 
-constexpr int K6_LARGE_PX = 4096;   // search boxes larger than this go to the CTA-per-object kernel
+constexpr int K6_LARGE_PX = 4096;     // search boxes larger than this go to the CTA-per-object kernel,
+constexpr int K6_HUGE_PX = 1 << 18;   // larger than this to the grid-wide kernels (k6h_*): chunks of the box over all CTAs
+constexpr int K6H_CHUNK = 1 << 14;    // pixels of a box one CTA sums at a time (grows when the units would exceed K6H_MAX_UNITS)
+constexpr int K6H_MAX_UNITS = 1 << 16;
 
 struct K6Args {
     const float *sub, *rms;
@@ -23,8 +26,12 @@ struct K6Args {
     int B, H, W;
     bd_phot_params p;
     bd_phot *out;
-    uint32_t *large_count;   // workspace: number of queued large objects, then their indices
+    uint32_t *large_count;   // workspace: [0] number of queued large objects, [1] of huge ones, [2] units, [3] chunk size
     uint32_t *large_list;
+    uint32_t *huge_list;     // [cap]
+    uint32_t *huge_first;    // [cap + 1] first unit of every huge object (exclusive prefix of its chunk count)
+    double *huge_kron;       // [cap] Kron radius after the first pass
+    double *huge_part;       // [K6H_MAX_UNITS][4] per-unit partial sums
 };
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -65,23 +72,37 @@ __device__ __forceinline__ bool ellipse_box(const Ellipse &e, double R, int H, i
     return b.x_hi >= b.x_lo && b.y_hi >= b.y_lo;
 }
 __device__ __forceinline__ long long box_area(const Box &b) { return (long long)(b.x_hi - b.x_lo + 1) * (b.y_hi - b.y_lo + 1); }
-// this thread's share (pixels t, t + nt, ... of the box) of  S0 = sum I, S1 = sum r I, V = sum rms^2, N = count  over r <= R
+// rad <= R with rad = sqrt(max(r2, 0)) rounded to nearest  <=>  r2 <= r2_limit(R): the largest double whose rounded square
+// root does not exceed R (sqrt is monotone, so the limit is R*R up to a couple of ulps, found by stepping).  The per-pixel
+// test is then one comparison, with the SAME membership as the definition's; the root is taken for members only.
+__device__ __forceinline__ double r2_limit(double R) {
+    double t = __dmul_rn(R, R);
+    for (int k = 0; k < 4 && sqrt(t) > R; ++k) t = __longlong_as_double(__double_as_longlong(t) - 1);
+    for (int k = 0; k < 4; ++k) {
+        const double u = __longlong_as_double(__double_as_longlong(t) + 1);
+        if (sqrt(u) <= R) t = u; else break;
+    }
+    return t;
+}
+// this thread's share (pixels k0 + t, k0 + t + nt, ... < k1 of the box) of  S0 = sum I, S1 = sum r I, V = sum rms^2,
+// N = count  over r <= R (T = r2_limit(R)).  NEED_R: S1 is wanted (the first pass).
 // (32-bit pixel indices: the box lies inside the frame and H*W < 2^31 is enforced at the boundary)
-__device__ __forceinline__ void ellipse_partial(const Ellipse &e, const Box &b, double R, const float *sub, const float *rms, int W,
-                                                int t, int nt, double &S0, double &S1, double &V, int &N) {
+template <bool NEED_R>
+__device__ __forceinline__ void ellipse_partial(const Ellipse &e, const Box &b, double T, const float *sub, const float *rms, int W,
+                                                int k0, int k1, int t, int nt, double &S0, double &S1, double &V, int &N) {
     S0 = 0.0; S1 = 0.0; V = 0.0; N = 0;
     const int bw = b.x_hi - b.x_lo + 1;
-    const int n = (int)box_area(b);
-    for (int k = t; k < n; k += nt) {
+    for (int k = k0 + t; k < k1; k += nt) {
         const int row = k / bw;
         const int yy = b.y_lo + (int)row, xx = b.x_lo + (int)(k - row * bw);
         const double dx = (double)xx - e.xc, dy = (double)yy - e.yc;
         const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(__dmul_rn(e.cxx, dx), dx), __dmul_rn(__dmul_rn(e.cyy, dy), dy)),
                                     __dmul_rn(__dmul_rn(e.cxy, dx), dy));
-        const double rad = sqrt(fmax(r2, 0.0));
-        if (rad <= R) {
-            const double I = (double)__ldg(sub + (size_t)yy * W + xx), q = (double)__ldg(rms + (size_t)yy * W + xx);
-            S0 += I; S1 += rad * I; V += q * q; ++N;
+        if (r2 <= T) {
+            const double I = (double)__ldg(sub + (size_t)yy * W + xx);
+            S0 += I; ++N;
+            if (NEED_R) S1 += sqrt(fmax(r2, 0.0)) * I;
+            else { const double q = (double)__ldg(rms + (size_t)yy * W + xx); V += q * q; }
         }
     }
 }
@@ -108,6 +129,7 @@ __global__ void __launch_bounds__(256) k6_photometry(K6Args a) {
     const int H = a.H, W = a.W;
     const size_t HW = (size_t)H * W;
     const long long warps = (long long)gridDim.x * (blockDim.x >> 5);
+    const double T_search = r2_limit(a.p.kron_search);
     for (long long i = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); i < total; i += warps) {
         const bd_source s = a.cat[i];
         const float *sub = a.sub + (size_t)s.frame * HW, *rms = a.rms + (size_t)s.frame * HW;
@@ -165,22 +187,42 @@ __global__ void __launch_bounds__(256) k6_photometry(K6Args a) {
         double S0 = 0.0, S1 = 0.0, V = 0.0, kron = a.p.kron_min_radius;
         int N = 0;
         bool ok = ellipse_box(e, a.p.kron_search, H, W, b, cut);
-        const bool large = ok && box_area(b) > K6_LARGE_PX;
-        if (large) {   // measured by k6_photometry_large; the aperture part is final
-            if (lane == 0) a.large_list[atomicAdd(a.large_count, 1u)] = (uint32_t)i;
+        // objects with more than K6_LARGE_PX pixels in either box are measured by k6_photometry_large / the k6h_* kernels
+        // (which redo both passes); the aperture part is final
+        auto defer = [&](long long area) {
+            if (lane != 0) return;
+            // (at most K6H_MAX_UNITS / 2 huge objects, so that their chunks fit the partial-sum table; the rest, if a frame
+            //  ever has that many, are measured by one CTA each like the large ones)
+            bool huge = area > K6_HUGE_PX;
+            if (huge) {
+                const uint32_t k = atomicAdd(a.large_count + 1, 1u);
+                if (k < (uint32_t)(K6H_MAX_UNITS / 2)) a.huge_list[k] = (uint32_t)i;
+                else huge = false;
+            }
+            if (!huge) a.large_list[atomicAdd(a.large_count, 1u)] = (uint32_t)i;
+        };
+        if (ok && box_area(b) > K6_LARGE_PX) {
+            defer(box_area(b));
         } else {
-            if (cut) flags |= 2;
             if (ok) {
-                ellipse_partial(e, b, a.p.kron_search, sub, rms, W, lane, 32, S0, S1, V, N);
+                ellipse_partial<true>(e, b, T_search, sub, rms, W, 0, (int)box_area(b), lane, 32, S0, S1, V, N);
                 S0 = warp_sum(S0); S1 = warp_sum(S1);
             }
             kron = kron_radius_of(a.p, S0, S1);
             S0 = 0.0; V = 0.0; N = 0;
-            ok = ellipse_box(e, kron, H, W, b, cut);
-            if (cut) flags |= 2;
-            if (ok) {
-                ellipse_partial(e, b, kron, sub, rms, W, lane, 32, S0, S1, V, N);
-                S0 = warp_sum(S0); V = warp_sum(V); N = warp_sum_i(N);
+            bool cut2;
+            const bool ok2 = ellipse_box(e, kron, H, W, b, cut2);
+            if (ok2 && box_area(b) > K6_LARGE_PX) {
+                // a faint object whose flux sum inside the search ellipse is nearly zero gets an arbitrarily large Kron radius
+                // (A25 has no upper limit): its second box can be the whole frame
+                defer(box_area(b));
+                kron = a.p.kron_min_radius;
+            } else {
+                if (cut || cut2) flags |= 2;
+                if (ok2) {
+                    ellipse_partial<false>(e, b, r2_limit(kron), sub, rms, W, 0, (int)box_area(b), lane, 32, S0, S1, V, N);
+                    S0 = warp_sum(S0); V = warp_sum(V); N = warp_sum_i(N);
+                }
             }
         }
         if (lane == 0) {
@@ -219,12 +261,26 @@ __global__ void __launch_bounds__(256) k6_photometry_large(K6Args a) {
         bool cut;
         int flags = 0, N = 0;
         double S0 = 0.0, S1 = 0.0, V = 0.0;
-        if (ellipse_box(e, a.p.kron_search, H, W, b, cut)) ellipse_partial(e, b, a.p.kron_search, sub, rms, W, threadIdx.x, blockDim.x, S0, S1, V, N);
+        if (ellipse_box(e, a.p.kron_search, H, W, b, cut))
+            ellipse_partial<true>(e, b, r2_limit(a.p.kron_search), sub, rms, W, 0, (int)box_area(b), threadIdx.x, blockDim.x, S0, S1, V, N);
         if (cut) flags |= 2;
         block_sum4(sm, S0, S1, V, N);
         const double kron = kron_radius_of(a.p, S0, S1);
         S0 = 0.0; S1 = 0.0; V = 0.0; N = 0;
-        if (ellipse_box(e, kron, H, W, b, cut)) ellipse_partial(e, b, kron, sub, rms, W, threadIdx.x, blockDim.x, S0, S1, V, N);
+        const bool ok2 = ellipse_box(e, kron, H, W, b, cut);
+        if (ok2 && box_area(b) > K6_HUGE_PX) {   // second box huge: the grid-wide kernels (launched next) take the object over
+            __shared__ uint32_t s_slot;
+            if (threadIdx.x == 0) s_slot = atomicAdd(a.large_count + 1, 1u);
+            __syncthreads();
+            const uint32_t k = s_slot;
+            __syncthreads();
+            if (k < (uint32_t)(K6H_MAX_UNITS / 2)) {
+                if (threadIdx.x == 0) a.huge_list[k] = i;
+                continue;
+            }
+        }
+        if (ok2)
+            ellipse_partial<false>(e, b, r2_limit(kron), sub, rms, W, 0, (int)box_area(b), threadIdx.x, blockDim.x, S0, S1, V, N);
         if (cut) flags |= 2;
         block_sum4(sm, S0, S1, V, N);
         if (threadIdx.x == 0) {
@@ -234,9 +290,113 @@ __global__ void __launch_bounds__(256) k6_photometry_large(K6Args a) {
     }
 }
 
+// ---- huge objects (search box > K6_HUGE_PX pixels: the saturated stars of a crowded field, whose Kron ellipses cover
+// megapixels): the box is cut into chunks of `chunk` consecutive pixels (row-major over the box) that ALL CTAs of the grid
+// share; per-chunk partial sums go to the workspace and are combined per object in chunk order, so the result does not
+// depend on which CTA summed which chunk.  PASS 0: first-moment radius inside kron_search; PASS 1: sums inside kron_radius.
+template <int PASS>
+__device__ __forceinline__ bool k6h_box(const K6Args &a, uint32_t j, const Ellipse &e, Box &b, bool &cut) {
+    const double R = PASS == 0 ? a.p.kron_search : a.huge_kron[j];
+    return ellipse_box(e, R, a.H, a.W, b, cut);
+}
+
+template <int PASS>
+__global__ void __launch_bounds__(256) k6h_plan(K6Args a) {
+    __shared__ unsigned long long s_area;
+    const uint32_t n = min(a.large_count[1], (uint32_t)(K6H_MAX_UNITS / 2));
+    if (threadIdx.x == 0) s_area = 0ull;
+    __syncthreads();
+    unsigned long long mine = 0;
+    for (uint32_t j = threadIdx.x; j < n; j += blockDim.x) {
+        const bd_source s = a.cat[a.huge_list[j]];
+        const Ellipse e = make_ellipse(s);
+        Box b;
+        bool cut;
+        const long long area = k6h_box<PASS>(a, j, e, b, cut) ? box_area(b) : 0;
+        a.huge_first[j] = (uint32_t)area;   // (H*W < 2^31)
+        mine += (unsigned long long)area;
+    }
+    atomicAdd(&s_area, mine);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        // units = sum ceil(area / chunk) <= total / chunk + n <= K6H_MAX_UNITS  (n <= K6H_MAX_UNITS / 2 by construction)
+        unsigned long long chunk = (s_area + K6H_MAX_UNITS / 2 - 1) / (K6H_MAX_UNITS / 2);
+        if (chunk < (unsigned long long)K6H_CHUNK) chunk = K6H_CHUNK;
+        uint32_t run = 0;
+        for (uint32_t j = 0; j < n; ++j) {
+            const uint32_t area = a.huge_first[j];
+            a.huge_first[j] = run;
+            run += (uint32_t)((area + chunk - 1) / chunk);
+        }
+        a.huge_first[n] = run;
+        a.large_count[2] = run;
+        a.large_count[3] = (uint32_t)chunk;
+    }
+}
+
+template <int PASS>
+__global__ void __launch_bounds__(256) k6h_partial(K6Args a) {
+    __shared__ double sm[8 * 4];
+    const uint32_t n = min(a.large_count[1], (uint32_t)(K6H_MAX_UNITS / 2)), units = a.large_count[2], chunk = a.large_count[3];
+    const size_t HW = (size_t)a.H * a.W;
+    for (uint32_t u = blockIdx.x; u < units; u += gridDim.x) {
+        uint32_t lo = 0, hi = n;            // the object whose unit range holds u
+        while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (a.huge_first[mid] <= u) lo = mid; else hi = mid; }
+        const uint32_t j = lo, c = u - a.huge_first[j];
+        const bd_source s = a.cat[a.huge_list[j]];
+        const Ellipse e = make_ellipse(s);
+        Box b;
+        bool cut;
+        double S0 = 0.0, S1 = 0.0, V = 0.0;
+        int N = 0;
+        if (k6h_box<PASS>(a, j, e, b, cut)) {
+            const long long area = box_area(b);
+            const long long k0 = (long long)c * chunk, k1 = k0 + chunk < area ? k0 + chunk : area;
+            const float *sub = a.sub + (size_t)s.frame * HW, *rms = a.rms + (size_t)s.frame * HW;
+            const double T = r2_limit(PASS == 0 ? a.p.kron_search : a.huge_kron[j]);
+            ellipse_partial<PASS == 0>(e, b, T, sub, rms, a.W, (int)k0, (int)k1, threadIdx.x, blockDim.x, S0, S1, V, N);
+        }
+        block_sum4(sm, S0, S1, V, N);
+        if (threadIdx.x == 0) {
+            double *p = a.huge_part + (size_t)u * 4;
+            p[0] = S0; p[1] = S1; p[2] = V; p[3] = (double)N;
+        }
+        __syncthreads();
+    }
+}
+
+template <int PASS>
+__global__ void __launch_bounds__(256) k6h_combine(K6Args a) {
+    const uint32_t n = min(a.large_count[1], (uint32_t)(K6H_MAX_UNITS / 2));
+    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
+        const uint32_t i = a.huge_list[j];
+        double S0 = 0.0, S1 = 0.0, V = 0.0, N = 0.0;
+        for (uint32_t u = a.huge_first[j]; u < a.huge_first[j + 1]; ++u) {
+            const double *p = a.huge_part + (size_t)u * 4;
+            S0 += p[0]; S1 += p[1]; V += p[2]; N += p[3];
+        }
+        const bd_source s = a.cat[i];
+        const Ellipse e = make_ellipse(s);
+        Box b;
+        bool cut;
+        k6h_box<PASS>(a, j, e, b, cut);
+        bd_phot *o = a.out + i;
+        if (cut) o->flags |= 2;
+        if (PASS == 0) {
+            a.huge_kron[j] = kron_radius_of(a.p, S0, S1);
+        } else {
+            o->kron_radius = a.huge_kron[j]; o->flux_auto = S0; o->fluxerr_auto = sqrt(V); o->npix_auto = (int)N;
+        }
+    }
+}
+
 }  // namespace
 
-size_t k6_workspace_bytes(int64_t cat_capacity) { return 256 + (size_t)(cat_capacity > 0 ? cat_capacity : 1) * sizeof(uint32_t); }
+size_t k6_workspace_bytes(int64_t cat_capacity) {
+    const size_t cap = (size_t)(cat_capacity > 0 ? cat_capacity : 1);
+    // counters, large list, huge list, huge first-unit prefix, huge Kron radii, per-unit partial sums
+    return 256 + bd_align_up(cap * 4, 256) * 2 + bd_align_up((cap + 1) * 4, 256) + bd_align_up(cap * 8, 256) + (size_t)K6H_MAX_UNITS * 4 * sizeof(double);
+}
 
 int k6_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H, int W, const bd_source *d_cat,
               const int64_t *d_n_sources, int64_t cat_capacity, const bd_phot_params *p, bd_phot *d_phot, void *d_ws,
@@ -246,15 +406,27 @@ int k6_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H,
     K6Args a;
     a.sub = d_sub; a.rms = d_rms; a.cat = d_cat; a.n_sources = d_n_sources; a.cap = cat_capacity;
     a.B = B; a.H = H; a.W = W; a.p = *p; a.out = d_phot;
-    a.large_count = (uint32_t *)d_ws;
-    a.large_list = (uint32_t *)((char *)d_ws + 256);
-    BD_CUDA_CHECK(ctx, cudaMemsetAsync(a.large_count, 0, sizeof(uint32_t), st));
+    const size_t cap = (size_t)(cat_capacity > 0 ? cat_capacity : 1);
+    char *w = (char *)d_ws;
+    a.large_count = (uint32_t *)w; w += 256;
+    a.large_list = (uint32_t *)w; w += bd_align_up(cap * 4, 256);
+    a.huge_list = (uint32_t *)w; w += bd_align_up(cap * 4, 256);
+    a.huge_first = (uint32_t *)w; w += bd_align_up((cap + 1) * 4, 256);
+    a.huge_kron = (double *)w; w += bd_align_up(cap * 8, 256);
+    a.huge_part = (double *)w;
+    BD_CUDA_CHECK(ctx, cudaMemsetAsync(a.large_count, 0, 4 * sizeof(uint32_t), st));
     long long blocks = (cat_capacity + 7) / 8;
     const long long max_blocks = (long long)ctx->num_sms * 16;
     if (blocks > max_blocks) blocks = max_blocks;
     if (blocks < 1) blocks = 1;
     k6_photometry<<<(unsigned)blocks, 256, 0, st>>>(a);
     k6_photometry_large<<<ctx->num_sms * 4, 256, 0, st>>>(a);
+    k6h_plan<0><<<1, 256, 0, st>>>(a);
+    k6h_partial<0><<<ctx->num_sms * 8, 256, 0, st>>>(a);
+    k6h_combine<0><<<8, 256, 0, st>>>(a);
+    k6h_plan<1><<<1, 256, 0, st>>>(a);
+    k6h_partial<1><<<ctx->num_sms * 8, 256, 0, st>>>(a);
+    k6h_combine<1><<<8, 256, 0, st>>>(a);
     BD_CUDA_CHECK(ctx, cudaGetLastError());
     return BD_OK;
 }

@@ -586,6 +586,64 @@ def test_k6_large_objects_take_the_block_path(bd, ctx):
             assert np.allclose(g[k], want[k], rtol=1e-9, atol=1e-6), k
 
 
+def test_k6_huge_objects_take_the_grid_path(bd, ctx):
+    """Objects whose search box exceeds 2^18 pixels are cut into chunks that all CTAs share (k6h_*): same membership and
+    sums as the oracle; elongated and rotated, cut by the frame edge, in the second frame of a batch, next to small and
+    block-path objects; bit-reproducible run to run."""
+    rng = np.random.default_rng(12)
+    B, H, W = 2, 1100, 1500
+    sub = rng.normal(0, 1, (B, H, W)).astype(np.float32); rms = rng.uniform(0.8, 1.3, (B, H, W)).astype(np.float32)
+    yy, xx = np.mgrid[:H, :W].astype(np.float64)
+    objs = [(0, 700.3, 540.7, 60.0, 42.0, 0.4), (0, 30.2, 25.5, 2.0, 1.5, 0.1), (0, 1300.5, 200.5, 11.0, 10.5, 1.2),
+            (1, 1450.6, 60.2, 70.0, 55.0, 0.0), (1, 600.1, 550.9, 150.0, 16.0, -0.7), (1, 100.0, 250.0, 1.2, 1.2, 0.0)]
+    cat = np.zeros(len(objs), dtype=bd.SOURCE_DTYPE)
+    for i, (f, xc, yc, sx, sy, th) in enumerate(objs):
+        c, s_ = np.cos(th), np.sin(th)
+        u = (xx - xc) * c + (yy - yc) * s_; v = -(xx - xc) * s_ + (yy - yc) * c
+        sub[f] += (5e5 / (2 * np.pi * sx * sy) * np.exp(-0.5 * (u * u / sx**2 + v * v / sy**2))).astype(np.float32)
+        cat[i]["frame"], cat[i]["x"], cat[i]["y"] = f, xc, yc
+        cat[i]["x2"] = sx**2 * c * c + sy**2 * s_ * s_; cat[i]["y2"] = sx**2 * s_ * s_ + sy**2 * c * c
+        cat[i]["xy"] = (sx**2 - sy**2) * s_ * c
+    n = torch.tensor([3, 3], dtype=torch.int64, device="cuda")
+    d_cat = torch.from_numpy(cat.view(np.uint8)).cuda()
+    ph = bd.photometry(ctx, dev(sub), dev(rms), d_cat, n, 16)
+    ph2 = bd.photometry(ctx, dev(sub), dev(rms), d_cat, n, 16)
+    torch.cuda.synchronize()
+    assert torch.equal(ph, ph2)
+    got = bd.phot_to_numpy(ph, n, 16)
+    for f in range(B):
+        sel = cat["frame"] == f
+        want = oph.photometry(sub[f], rms[f], cat[sel], oph.PhotParams())
+        g = got[sel]
+        assert np.array_equal(g["npix_auto"], want["npix_auto"]) and np.array_equal(g["flags"], want["flags"])
+        assert want["npix_auto"].max() > (1 << 16)
+        for k in ("flux_aper", "fluxerr_aper", "area_aper", "kron_radius", "flux_auto", "fluxerr_auto"):
+            assert np.allclose(g[k], want[k], rtol=1e-9, atol=1e-6), k
+
+
+def test_k6_full_size_config5_sampled(bd, ctx):
+    """Config 5 at full size (6144 x 6144, crowded, 200 saturated stars whose Kron ellipses cover megapixels: the grid-wide
+    path at real scale): the 10 records with the largest second moments and 400 seeded random ones against the oracle."""
+    cfg = CONFIGS[5]
+    img = make_frames(cfg)
+    p = params_for(bd, cfg)
+    cap = 1 << 20
+    d_img = dev(img)
+    bm, rm, cb, cr = bd.bkg_estimate(ctx, d_img, p)
+    fz = bd.bkg_subtract_detect(ctx, d_img, p.mesh_h, p.mesh_w, cb, cr, cfg.detect_k, cfg.min_area, cap, want_bkg=False, want_mask=False)
+    ph = bd.photometry(ctx, fz["sub"], fz["rms"], fz["cat"], fz["n_sources"], cap)
+    torch.cuda.synchronize()
+    cat = bd.catalogue_to_numpy(fz["cat"], fz["n_sources"], cap)
+    got = bd.phot_to_numpy(ph, fz["n_sources"], cap)
+    rng = np.random.default_rng(35)
+    idx = np.union1d(rng.choice(len(cat), 400, replace=False), np.argsort(cat["x2"] + cat["y2"])[-10:])
+    # ... and the records with the largest Kron ellipses (A25 has no upper limit: a faint object whose flux sum inside the
+    # search ellipse is nearly zero gets an ellipse that can cover the frame)
+    idx = np.union1d(idx, np.argsort(got["npix_auto"])[-6:])
+    want = _k6_compare(bd, got, cat, fz["sub"][0].cpu().numpy(), fz["rms"][0].cpu().numpy(), idx, oph.PhotParams())
+    assert want["npix_auto"].max() > (1 << 18)
+
+
 def test_k6_isolated_gaussian_and_errors(bd, ctx):
     """An analytic source through the GPU path alone: encircled energy and the Kron radius of a Gaussian."""
     H = W = 128
