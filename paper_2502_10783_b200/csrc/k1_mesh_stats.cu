@@ -868,17 +868,41 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
         uint8_t *col = hist8 + tid;
         K1_T(3);
         const uint32_t col_s = smem_u32(col);
-        K1_SWEEP_ANY({
-            const uint32_t k = f32_to_key(e);
-            k1_hist_inc(col_s, k - ka, span, shift, nt);
-            below += k < ka ? 1u : 0u;
-            const double d = (double)e - pivot;
-            if (e >= A_f && e <= B_f) {
-                t1 += d;
-                t2 = fma(d, d, t2);
-                ++c_core;
-            } else ++c_tail;
-        })
+        // A bracket of non-negative floats (every sky level): key - ka = bits - bits(ka) for the pixels that can fall into
+        // it, a negative pixel's difference exceeds any span (bits >= 2^31 > bits(kb)), and "below the bracket" is a
+        // signed compare of the raw bits -- the order-preserving key (3 instructions per pixel) is not needed.
+        const bool pos = ka >= 0x80000000u;
+        const uint32_t ka_bits = ka ^ 0x80000000u;
+        if (pos) {
+            K1_SWEEP_ANY({
+                const uint32_t bits = __float_as_uint(e);
+                k1_hist_inc(col_s, bits - ka_bits, span, shift, nt);
+                below += (int)bits < (int)ka_bits ? 1u : 0u;
+                const double d = (double)e - pivot;
+                if (e >= A_f && e <= B_f) {
+                    t1 += d;
+                    t2 = fma(d, d, t2);
+                    ++c_core;
+                }
+            })
+        } else {
+            K1_SWEEP_ANY({
+                const uint32_t k = f32_to_key(e);
+                k1_hist_inc(col_s, k - ka, span, shift, nt);
+                below += k < ka ? 1u : 0u;
+                const double d = (double)e - pivot;
+                if (e >= A_f && e <= B_f) {
+                    t1 += d;
+                    t2 = fma(d, d, t2);
+                    ++c_core;
+                }
+            })
+        }
+        {   // pixels this thread swept (the assignment of K1_SWEEP / K1_SWEEP_G): the tail count needs no counter of its own
+            const int my_px = stream ? (tid < n_f4 ? ((n_f4 - tid + nt - 1) / nt) * 4 : 0)
+                                     : (tid < n4 ? ((n4 - tid + nt - 1) / nt) * 4 : 0) + (tid < n_tail4 ? 1 : 0);
+            c_tail = my_px - c_core;
+        }
         __syncthreads();
         reduce_byte_hist(hist8, nt, s.xch.cnt);
         below = block_reduce_u32<false>(s, below);
@@ -938,10 +962,19 @@ __global__ void __launch_bounds__(C == 1 ? 512 : 1024, C == 1 ? K1_MINB : 1) k1_
             uint32_t pos_c = packed & 0xFFFFu, pos_t = packed >> 16;   // (the scan's barriers: histogram is dead)
             K1_T(6);
             uint32_t addr_c = smem_u32(&s.list[pos_c]), addr_t = smem_u32(&tail[pos_t]);
-            K1_SWEEP_ANY({
-                k1_push_u32_if_le(addr_c, f32_to_key(e) - kga, gspan, f32_to_key(e));
-                k1_push_f32_if_outside(addr_t, e, A_f, B_f);
-            })
+            if (pos) {   // (kga >= ka: the window is a bracket of non-negative floats too)
+                const uint32_t kga_bits = kga ^ 0x80000000u;
+                K1_SWEEP_ANY({
+                    const uint32_t bits = __float_as_uint(e);
+                    k1_push_u32_if_le(addr_c, bits - kga_bits, gspan, bits ^ 0x80000000u);
+                    k1_push_f32_if_outside(addr_t, e, A_f, B_f);
+                })
+            } else {
+                K1_SWEEP_ANY({
+                    k1_push_u32_if_le(addr_c, f32_to_key(e) - kga, gspan, f32_to_key(e));
+                    k1_push_f32_if_outside(addr_t, e, A_f, B_f);
+                })
+            }
             if (tid == 0) { s.xch.m_cand = packed_tot & 0xFFFFu; s.xch.m_tail = packed_tot >> 16; }
         }
         K1_T(7);

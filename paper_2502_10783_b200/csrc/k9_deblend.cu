@@ -137,7 +137,13 @@ __global__ void __launch_bounds__(256) k9_classify(DbArgs a) {
         }
         const long long area = (long long)(s.xmax - s.xmin + 1) * (s.ymax - s.ymin + 1);
         const int tier = area <= CAP_WARP ? 0 : area <= CAP_MID ? 1 : area <= CAP_BIG ? 2 : 3;
-        const uint32_t k = atomicAdd(&a.w.counters[C_TIER0 + tier], 1u);
+        // one atomic per (warp, tier) instead of one per candidate on four hot counters
+        const uint32_t peers = __match_any_sync(__activemask(), tier);
+        const int leader = __ffs(peers) - 1;
+        uint32_t base = 0;
+        if ((int)(threadIdx.x & 31) == leader) base = atomicAdd(&a.w.counters[C_TIER0 + tier], (uint32_t)__popc(peers));
+        base = __shfl_sync(peers, base, leader);
+        const uint32_t k = base + (uint32_t)__popc(peers & ((1u << (threadIdx.x & 31)) - 1u));
         a.w.lists[(size_t)tier * a.cap_in + k] = (int32_t)i;
     }
 }
