@@ -223,7 +223,12 @@ def test_k10_clean_synthetic_catalogue(bd, ctx):
     comps = [(5000.0, 128, 128, 6.0, 2.0)]
     for ang in range(0, 360, 20):
         for rad, amp in ((14, 12.0), (30, 25.0), (60, 8.0)):
+            if rad == 14 and 50 < ang % 180 < 130:
+                continue                                   # (room for the faint objects off the short axis)
             comps.append((amp, 128 + rad * np.cos(np.deg2rad(ang)), 128 + rad * np.sin(np.deg2rad(ang)), 1.3, 1.3))
+    # faint objects just off the short axis of the bright one: the Moffat-like wing extrapolated from its isophote
+    # (D10) exceeds what they stand above their own threshold, so they are false detections (D11)
+    comps += [(2.8, 128, 139, 1.3, 1.3), (2.8, 118, 140, 1.3, 1.3), (3.0, 140, 116, 1.3, 1.3), (2.6, 128, 117, 1.3, 1.3)]
     sub = gaussians(H, W, comps)[None]
     sub[0, 10, 10] = 40.0
     sub[0, 10, 11] = 40.0                                # a two-pixel object: degenerate moments
