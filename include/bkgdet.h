@@ -315,8 +315,10 @@ int image_subtract(bd_ctx *ctx, const float *d_ref, const float *d_img, int B, i
                    size_t ws_bytes, void *cuda_stream);
 
 /* ---- whole chain from HOST buffers (pinned or pageable), synchronous. ----------------------------------
- * Copies h_img to the device, runs bkg_estimate -> bkg_subtract_detect, copies the
- * catalogue and the per-frame counts back, and waits.  Device buffers are cached in ctx between calls.
+ * Copies h_img to the device in up to 8 chunks (whole frames of a batch, strips of mesh rows of a single frame) on a
+ * copy stream of its own and runs the statistics kernel of step a1 on every chunk as it arrives, then a2 and
+ * bkg_subtract_detect on the whole frame, copies the catalogue and the per-frame counts back, and waits.  Same results as
+ * the device calls.  Device buffers, the two streams and the events are cached in ctx between calls.
  * h_cat: [cat_capacity] records; h_n_sources: [B].  Returns BD_OK or an error code. */
 int bd_run_host(bd_ctx *ctx, const float *h_img, int B, int H, int W, const bd_bkg_params *p,
                 double detect_k, int32_t min_area, bd_source *h_cat, int64_t cat_capacity,

@@ -51,6 +51,9 @@ void bd_destroy(bd_ctx *ctx) {
         BdDeviceGuard guard(ctx);
         if (ctx->host_dev) cudaFree(ctx->host_dev);
         if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
+        if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+        for (int c = 0; c < BD_HOST_CHUNKS; ++c)
+            if (ctx->host_ev[c]) cudaEventDestroy(ctx->host_ev[c]);
     }
     free(ctx);
 }
@@ -467,10 +470,41 @@ int bd_run_host(bd_ctx *ctx, const float *h_img, int B, int H, int W, const bd_b
         ctx->host_dev_bytes = off;
     }
     char *d = (char *)ctx->host_dev;
-    BD_CUDA_CHECK(ctx, cudaMemcpyAsync(d + o_img, h_img, P * 4, cudaMemcpyHostToDevice, st));
-    rc = bkg_estimate(ctx, (const float *)(d + o_img), B, H, W, p, nullptr, nullptr, (double *)(d + o_cb), (double *)(d + o_cr),
-                      d + o_wsb, ws_b, st);
-    if (rc) return rc;
+    // The frame arrives in chunks on a copy stream (whole frames of a batch, or strips of mesh rows of a single frame) and
+    // K1 runs on every chunk as soon as it is there: the statistics pass hides behind the PCIe transfer.  K2 and the fused
+    // pass need the whole mesh grid and follow the last chunk.
+    if (!ctx->copy_stream) BD_CUDA_CHECK(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+    for (int c = 0; c < BD_HOST_CHUNKS; ++c)
+        if (!ctx->host_ev[c]) BD_CUDA_CHECK(ctx, cudaEventCreateWithFlags(&ctx->host_ev[c], cudaEventDisableTiming));
+    {
+        const size_t stride = bd_align_up(cells * sizeof(double), 256);
+        char *base = (char *)bd_align_up((size_t)(d + o_wsb), 256);
+        double *raw_b = (double *)base, *raw_r = (double *)(base + stride), *scratch = (double *)(base + 4 * stride);
+        void *k1_ws = base + 4 * stride + bd_align_up(2 * (size_t)B * k2_scratch_per_grid(ny, nx) * sizeof(double), 256);
+        // units: frames of a batch, mesh rows of a single frame
+        const int units = B > 1 ? B : ny;
+        const int nch = units < BD_HOST_CHUNKS ? units : BD_HOST_CHUNKS;
+        // (the copy stream must not overwrite the frame while work of the previous call still reads it)
+        BD_CUDA_CHECK(ctx, cudaEventRecord(ctx->host_ev[BD_HOST_CHUNKS - 1], st));
+        BD_CUDA_CHECK(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->host_ev[BD_HOST_CHUNKS - 1], 0));
+        for (int c = 0; c < nch; ++c) {
+            const int u0 = (int)((long long)units * c / nch), u1 = (int)((long long)units * (c + 1) / nch);
+            size_t px0, px1, cell0;
+            int Bc, Hc;
+            if (B > 1) { px0 = (size_t)u0 * H * W; px1 = (size_t)u1 * H * W; cell0 = (size_t)u0 * ny * nx; Bc = u1 - u0; Hc = H; }
+            else {
+                const int r0 = u0 * p->mesh_h, r1 = u1 == ny ? H : u1 * p->mesh_h;
+                px0 = (size_t)r0 * W; px1 = (size_t)r1 * W; cell0 = (size_t)u0 * nx; Bc = 1; Hc = r1 - r0;
+            }
+            BD_CUDA_CHECK(ctx, cudaMemcpyAsync(d + o_img + px0 * 4, h_img + px0, (px1 - px0) * 4, cudaMemcpyHostToDevice, ctx->copy_stream));
+            BD_CUDA_CHECK(ctx, cudaEventRecord(ctx->host_ev[c], ctx->copy_stream));
+            BD_CUDA_CHECK(ctx, cudaStreamWaitEvent(st, ctx->host_ev[c], 0));
+            rc = k1_launch(ctx, (const float *)(d + o_img) + px0, Bc, Hc, W, p, raw_b + cell0, raw_r + cell0, nullptr, nullptr, nullptr, k1_ws, st);
+            if (rc) return rc;
+        }
+        rc = k2_launch(ctx, raw_b, raw_r, B, ny, nx, p->filt_h, p->filt_w, nullptr, nullptr, (double *)(d + o_cb), (double *)(d + o_cr), scratch, st);
+        if (rc) return rc;
+    }
     rc = bkg_subtract_detect(ctx, (const float *)(d + o_img), B, H, W, p->mesh_h, p->mesh_w, (const double *)(d + o_cb),
                              (const double *)(d + o_cr), detect_k, min_area, (float *)(d + o_sub), nullptr, (float *)(d + o_rms),
                              (uint8_t *)(d + o_mask), (int32_t *)(d + o_lab), (bd_source *)(d + o_cat), cat_capacity,

@@ -22,8 +22,10 @@ struct bd_ctx {
     // bd_run_host cache
     void *host_dev;
     size_t host_dev_bytes;
-    cudaStream_t host_stream;
+    cudaStream_t host_stream, copy_stream;
+    cudaEvent_t host_ev[8];   // BD_HOST_CHUNKS: one per chunk of the frame that bd_run_host copies
 };
+#define BD_HOST_CHUNKS 8
 
 int bd_set_error(bd_ctx *ctx, int code, const char *fmt, ...);
 

@@ -432,17 +432,22 @@ def test_chain_config4_batch(bd, ctx):
         assert_catalogue_equal(cat, stage, frame=f)
 
 
-def test_run_host_matches_device_path(bd, ctx):
-    cfg = CONFIGS[1]
-    img = make_frames(cfg)
+@pytest.mark.parametrize("cid,H,W,B", [(1, 512, 512, 1), (3, 1100, 768, 1), (4, 256, 256, 11), (5, 200, 260, 2)])
+def test_run_host_matches_device_path(bd, ctx, cid, H, W, B):
+    """bd_run_host copies the frame in chunks (strips of mesh rows, or frames of a batch) and runs K1 per chunk: the same
+    catalogue as the device calls; a partial last mesh row, more frames than chunks, fewer mesh rows than chunks; called
+    twice (cached buffers)."""
+    cfg = CONFIGS[cid]
+    img = make_frames(cfg, H=H, W=W, B=B)
     p = params_for(bd, cfg)
-    cat_h, n_h = bd.run_host(ctx, img, p, cfg.detect_k, cfg.min_area, 4096)
-    bm, rm, o, det = run_chain(bd, ctx, img, p, cfg.detect_k, cfg.min_area, 4096)
-    cat_d = bd.catalogue_to_numpy(det["cat"], det["n_sources"], 4096)
-    assert np.array_equal(n_h, det["n_sources"].cpu().numpy())
-    for k in ("label", "npix", "xpeak", "ypeak"):
-        assert np.array_equal(cat_h[k], cat_d[k])
-    assert np.allclose(cat_h["flux"], cat_d["flux"], rtol=1e-12)
+    bm, rm, o, det = run_chain(bd, ctx, img, p, cfg.detect_k, cfg.min_area, 1 << 15)
+    cat_d = bd.catalogue_to_numpy(det["cat"], det["n_sources"], 1 << 15)
+    for _ in range(2):
+        cat_h, n_h = bd.run_host(ctx, img, p, cfg.detect_k, cfg.min_area, 1 << 15)
+        assert np.array_equal(n_h, det["n_sources"].cpu().numpy())
+        for k in ("frame", "label", "npix", "xpeak", "ypeak"):
+            assert np.array_equal(cat_h[k], cat_d[k])
+        assert np.allclose(cat_h["flux"], cat_d["flux"], rtol=1e-12)
 
 
 # ------------------------------------------------------------------------------------------- NEXT-2: photometry (K6)
