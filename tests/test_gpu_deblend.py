@@ -345,3 +345,30 @@ def test_k9_k10_full_size_sampled(bd, ctx, cfgn):
     lab_cg = lab_c[0].cpu().numpy()
     gone = np.isin(lab_g, cat_g["label"][flags_g != 0])
     assert not lab_cg[gone].any() and np.array_equal(lab_cg[~gone], lab_g[~gone])
+
+
+def test_k9_workspace_tier_in_a_batch_and_reproducibility(bd, ctx):
+    """Candidates of every tier (the largest take the frame-coordinate workspace arrays) in the SECOND frame of a batch;
+    two runs give bit-identical label maps, counts and record keys (labels never depend on atomic order)."""
+    scale = 9.0
+    s = 1.6 * scale
+    H = W = int(64 * scale) * 2
+    u = 64 * scale
+    big = [(200.0, 0.5 * u, 0.5 * u, s, s), (200.0, 0.5 * u + 3.2 * s, 0.5 * u, s, s),
+           (120.0, 0.6 * u, 1.5 * u, s, s), (90.0, 0.6 * u + 3.4 * s, 1.5 * u, s, s)]
+    small_ = [(60.0, 40 + 30 * k, 60 + 25 * (k % 3), 1.5, 1.5) for k in range(12)] + [(55.0, 44 + 30 * k, 61 + 25 * (k % 3), 1.5, 1.5) for k in range(12)]
+    rng = np.random.default_rng(3)
+    f0 = (gaussians(H, W, small_).astype(np.float64) + rng.normal(0, 0.2, (H, W))).astype(np.float32)
+    f1 = (gaussians(H, W, big + [(c[0], c[1] + 600, c[2] + 700, c[3], c[4]) for c in small_]).astype(np.float64)
+          + rng.normal(0, 0.2, (H, W))).astype(np.float32)
+    sub = np.stack([f0, f1])
+    rms = np.ones_like(sub)
+    labels, cat = labelled(sub, rms, 1.5, 5)
+    areas = (cat["xmax"] - cat["xmin"] + 1) * (cat["ymax"] - cat["ymin"] + 1)
+    assert (areas[cat["frame"] == 1] > 5120).sum() >= 2
+    stats, lab_a, cat_a, n_a = check_deblend(bd, ctx, sub, rms, labels, cat, 1.5, 5)
+    assert stats["n_split"] >= 6
+    _, lab_b, cat_b, n_b = check_deblend(bd, ctx, sub, rms, labels, cat, 1.5, 5)
+    assert np.array_equal(lab_a, lab_b) and np.array_equal(n_a, n_b)
+    for k in ("frame", "label", "npix", "xmin", "xmax", "ymin", "ymax", "xpeak", "ypeak", "peak"):
+        assert np.array_equal(cat_a[k], cat_b[k]), k
