@@ -153,7 +153,7 @@ struct DbCtl {   // per group (warp or block), shared memory
     double t[DB_MAXT];
     int hist[DB_MAXT], start[DB_MAXT], cur[DB_MAXT];
     u64 frzmask;
-    int n_lost, n_touched, n_f[2], nslot, item, pool_base, pool_ok;
+    int n_lost, n_old, n_touched, n_f[2], nslot, item, pool_base, pool_ok;
     long long seg;
 };
 
@@ -222,7 +222,7 @@ __device__ __forceinline__ int db_find(int32_t *par, int x) {
 
 // union by minimum index; a root that is hooked goes into the lost list (exactly once in its life)
 template <bool GL, bool TRACK>
-__device__ __forceinline__ void db_unite(int32_t *par, int a, int b, int32_t *lost, int *n_lost) {
+__device__ __forceinline__ void db_unite(int32_t *par, int a, int b, int32_t *lost, int *n_lost, const int8_t *lvl, int level, int *n_old) {
     while (true) {
         a = db_find<GL>(par, a);
         b = db_find<GL>(par, b);
@@ -230,7 +230,10 @@ __device__ __forceinline__ void db_unite(int32_t *par, int a, int b, int32_t *lo
         if (a < b) { const int t = a; a = b; b = t; }
         const int old = atomicCAS(&par[a], a, b);
         if (old == a) {
-            if (TRACK) lost[atomicAdd(n_lost, 1)] = a;
+            if (TRACK) {
+                lost[atomicAdd(n_lost, 1)] = a;
+                if (lvl[a] > level) atomicAdd(n_old, 1);   // a component of the level above merges: a tree decision is due
+            }
             return;
         }
         a = old;
@@ -250,7 +253,7 @@ __device__ __forceinline__ void db_unite_level(const G &g, const Geo<GL> &geo, c
             for (int dx = -1; dx <= 1; ++dx) {
                 if ((dy == 0 && dx == 0) || lx + dx < 0 || lx + dx >= geo.bw) continue;
                 const int q = p + dy * geo.pitch + dx;
-                if (db_active<GL>(geo, A, q, level)) db_unite<GL, TRACK>(A.par, p, q, A.lost, &C->n_lost);
+                if (db_active<GL>(geo, A, q, level)) db_unite<GL, TRACK>(A.par, p, q, A.lost, &C->n_lost, A.lvl, level, &C->n_old);
             }
         }
     }
@@ -372,12 +375,30 @@ __device__ void db_candidate(const G &g, const DbArgs &a, const DbArr &A0, DbCtl
             A.st[p] = min_area <= 1 ? 1 : 0;
             A.T[p] = 0;
         }
-        if (tid == 0) { C->n_lost = 0; C->n_touched = 0; }
+        if (tid == 0) { C->n_lost = 0; C->n_old = 0; C->n_touched = 0; }
         g.sync();
         db_unite_level<GL, true>(g, geo, A, C, i, beg, end);
         g.sync();
         const int nl = C->n_lost;
         if (nl == 0) {   // nothing merged: the new pixels are isolated at this level and finalised by their initialisation
+            continue;
+        }
+        if (C->n_old == 0) {
+            // Only pixels of this level were hooked: no component of the level above merged, so no node gains a child other
+            // than its own former self and every st[] of a node stays what it was (T = the self contribution: st for a
+            // split node, at most 1 otherwise).  What can change is that a component reaches min_area and becomes a node.
+            for (int k = tid; k < nl; k += nt) {
+                const int c = A.lost[k];
+                const int R = db_find<GL>(A.par, c);
+                atomicAdd(&A.accn[R], A.accn[c]);
+                atomicAdd(&A.accf[R], A.accf[c]);
+            }
+            g.sync();
+            for (int k = tid; k < nl; k += nt) {
+                const int R = db_find<GL>(A.par, A.lost[k]);
+                if (A.st[R] == 0 && ldv<GL>(A.accn + R) >= min_area) A.st[R] = 1;
+            }
+            g.sync();
             continue;
         }
         // children report to the root they ended under
