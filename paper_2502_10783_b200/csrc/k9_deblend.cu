@@ -37,7 +37,7 @@ typedef unsigned long long u64;
 #include "kept_rank.cuh"
 
 constexpr int DB_MAXT = 64;            // n_thresh <= 64
-constexpr int CAP_WARP = 256, CAP_MID = 1536, CAP_BIG = 5120;
+constexpr int CAP_TINY = 112, CAP_WARP = 256, CAP_MID = 1536, CAP_BIG = 5120;   // pixels of the box and its border per tier
 constexpr int WARPS_PER_CTA = 8;
 constexpr int T_QUEUED = 0x40000000, T_SELFSIG = 0x20000000, T_SUM = 0x1FFFFFFF;
 
@@ -54,11 +54,12 @@ struct ORec {   // 96 bytes: one object of a split candidate; sums are about the
 static_assert(sizeof(ORec) == 96, "ORec must be 96 bytes");
 
 // counters[] slots
-enum { C_TIER0 = 0, C_CUR0 = 4, C_POOL = 8, C_SEG = 10 /* u64: [10], [11] */, C_NCOUNT = 64 };
+enum { C_TIER0 = 0 /* 5 tiers */, C_CUR0 = 8, C_POOL = 16, C_SEG = 18 /* u64: [18], [19] */, C_NCOUNT = 64 };
+constexpr int N_TIERS = 5;   // 0 tiny warp, 1 warp, 2 mid block, 3 big block, 4 workspace
 
 struct DbWs {
     uint32_t *counters;
-    int32_t *lists;        // [4][cap_in]
+    int32_t *lists;        // [N_TIERS][cap_in]
     uint8_t *state;        // [cap_in] 1 = the candidate was split (its record is replaced by pool records)
     uint32_t *keptbits, *blkcnt, *blkprefix;
     ORec *pool;            // [cap_out]
@@ -82,7 +83,7 @@ size_t carve(DbWs &w, void *base, int B, int H, int W, int64_t cap_in, int64_t c
     w.blkcnt = (uint32_t *)take((w.NB + 8) * sizeof(uint32_t));
     w.zero_bytes = (size_t)((char *)w.blkcnt - (char *)w.counters) + (w.NB + 1) * sizeof(uint32_t);
     w.blkprefix = (uint32_t *)take((w.NB + 8) * sizeof(uint32_t));
-    w.lists = (int32_t *)take(4 * (size_t)cap_in * sizeof(int32_t));
+    w.lists = (int32_t *)take(5 * (size_t)cap_in * sizeof(int32_t));
     w.state = (uint8_t *)take((size_t)cap_in);
     w.pool = (ORec *)take((size_t)cap_out * sizeof(ORec));
     w.par = (int32_t *)take(P * 4); w.accn = (int32_t *)take(P * 4); w.st = (int32_t *)take(P * 4); w.T = (int32_t *)take(P * 4);
@@ -135,8 +136,8 @@ __global__ void __launch_bounds__(256) k9_classify(DbArgs a) {
             mark_kept(a.w, (size_t)s.frame * HW + (size_t)(s.label - 1));
             continue;
         }
-        const long long area = (long long)(s.xmax - s.xmin + 1) * (s.ymax - s.ymin + 1);
-        const int tier = area <= CAP_WARP ? 0 : area <= CAP_MID ? 1 : area <= CAP_BIG ? 2 : 3;
+        const long long area = (long long)(s.xmax - s.xmin + 3) * (s.ymax - s.ymin + 3);   // the box and its one-pixel border
+        const int tier = area <= CAP_TINY ? 0 : area <= CAP_WARP ? 1 : area <= CAP_MID ? 2 : area <= CAP_BIG ? 3 : 4;
         // one atomic per (warp, tier) instead of one per candidate on four hot counters
         const uint32_t peers = __match_any_sync(__activemask(), tier);
         const int leader = __ffs(peers) - 1;
@@ -240,22 +241,36 @@ __device__ __forceinline__ void db_unite(int32_t *par, int a, int b, int32_t *lo
     }
 }
 
+
+// the 8 neighbours of pixel p = (ly, lx): f(q, dy, dx)
+template <bool GL, class F>
+__device__ __forceinline__ void db_for_neighbours(const Geo<GL> &geo, int p, int ly, int lx, F f) {
+#pragma unroll
+    for (int dy = -1; dy <= 1; ++dy) {
+        if (GL && (ly + dy < 0 || ly + dy >= geo.bh)) continue;
+#pragma unroll
+        for (int dx = -1; dx <= 1; ++dx) {
+            if (dy == 0 && dx == 0) continue;
+            if (GL && (lx + dx < 0 || lx + dx >= geo.bw)) continue;
+            f(p + dy * geo.pitch + dx, dy, dx);
+        }
+    }
+}
+// an entry of the level-sorted list: (row << 16) | column of the box; -> array index
+template <bool GL>
+__device__ __forceinline__ int db_entry(const Geo<GL> &geo, int packed, int &ly, int &lx) {
+    ly = packed >> 16; lx = packed & 0xFFFF;
+    return geo.aidx(ly, lx);
+}
+
 template <bool GL, bool TRACK, class G>
 __device__ __forceinline__ void db_unite_level(const G &g, const Geo<GL> &geo, const DbArr &A, DbCtl *C, int level, int beg, int end) {
     for (int k = beg + g.tid(); k < end; k += g.size()) {
-        const int p = A.order[k];
         int ly, lx;
-        geo.coords(p, ly, lx);
-#pragma unroll
-        for (int dy = -1; dy <= 1; ++dy) {
-            if (ly + dy < 0 || ly + dy >= geo.bh) continue;
-#pragma unroll
-            for (int dx = -1; dx <= 1; ++dx) {
-                if ((dy == 0 && dx == 0) || lx + dx < 0 || lx + dx >= geo.bw) continue;
-                const int q = p + dy * geo.pitch + dx;
-                if (db_active<GL>(geo, A, q, level)) db_unite<GL, TRACK>(A.par, p, q, A.lost, &C->n_lost, A.lvl, level, &C->n_old);
-            }
-        }
+        const int p = db_entry<GL>(geo, A.order[k], ly, lx);
+        db_for_neighbours<GL>(geo, p, ly, lx, [&](int q, int, int) {
+            if (db_active<GL>(geo, A, q, level)) db_unite<GL, TRACK>(A.par, p, q, A.lost, &C->n_lost, A.lvl, level, &C->n_old);
+        });
     }
 }
 
@@ -299,8 +314,10 @@ __device__ void db_candidate(const G &g, const DbArgs &a, const DbArr &A0, DbCtl
     const size_t fo = (size_t)s.frame * HW;
     Geo<GL> geo;
     geo.L = s.label; geo.x0 = s.xmin; geo.y0 = s.ymin; geo.bw = s.xmax - s.xmin + 1; geo.bh = s.ymax - s.ymin + 1; geo.W = W;
-    geo.pitch = GL ? W : geo.bw;
-    geo.base = GL ? s.ymin * W + s.xmin : 0;
+    // shared tiers: the box sits inside a one-pixel border of inactive cells (lvl = -1), so the 8 neighbour tests of a
+    // pixel need no bounds checks; workspace tier: frame coordinates, neighbours are tested against the box
+    geo.pitch = GL ? W : geo.bw + 2;
+    geo.base = GL ? s.ymin * W + s.xmin : geo.pitch + 1;
     geo.sub = a.sub + fo;
     geo.lab = a.labels + fo;
     int32_t *labels = a.labels + fo;
@@ -328,6 +345,10 @@ __device__ void db_candidate(const G &g, const DbArgs &a, const DbArr &A0, DbCtl
     const double min_flux = __dmul_rn(a.min_cont, s.flux);   // D4 (the candidate's flux is the O6 flux of the record)
 
     // ---- levels of the member pixels, counting sort by level (descending) ---------------------------------------
+    if (!GL) {   // the border of inactive cells: rows -1 and bh, columns -1 and bw
+        for (int k = tid; k < geo.pitch; k += nt) { A.lvl[k] = -1; A.lvl[(geo.bh + 1) * geo.pitch + k] = -1; }
+        for (int k = tid; k < geo.bh; k += nt) { A.lvl[(k + 1) * geo.pitch] = -1; A.lvl[(k + 1) * geo.pitch + geo.bw + 1] = -1; }
+    }
     for (int k = tid; k < nbox; k += nt) {
         const int ly = k / geo.bw, lx = k - ly * geo.bw;
         const int f = geo.fidx(ly, lx), p = geo.aidx(ly, lx);
@@ -355,7 +376,7 @@ __device__ void db_candidate(const G &g, const DbArgs &a, const DbArr &A0, DbCtl
         const int ly = k / geo.bw, lx = k - ly * geo.bw;
         const int p = geo.aidx(ly, lx);
         const bool mem = GL ? labels[geo.fidx(ly, lx)] == geo.L : A.lvl[p] >= 0;
-        if (mem) A.order[atomicAdd(&C->cur[A.lvl[p]], 1)] = p;
+        if (mem) A.order[atomicAdd(&C->cur[A.lvl[p]], 1)] = (ly << 16) | lx;
     }
     g.sync();
     const int npix = C->start[0] + C->hist[0];
@@ -366,9 +387,8 @@ __device__ void db_candidate(const G &g, const DbArgs &a, const DbArr &A0, DbCtl
         if (!cnt) continue;
         const int beg = C->start[i], end = beg + cnt;
         for (int k = beg + tid; k < end; k += nt) {
-            const int p = A.order[k];
             int ly, lx;
-            geo.coords(p, ly, lx);
+            const int p = db_entry<GL>(geo, A.order[k], ly, lx);
             A.par[p] = p;
             A.accn[p] = 1;
             A.accf[p] = (double)__ldg(geo.sub + geo.fidx(ly, lx));
@@ -471,14 +491,15 @@ __device__ void db_candidate(const G &g, const DbArgs &a, const DbArr &A0, DbCtl
         const int cnt = C->hist[i];
         const int beg = C->start[i], end = beg + cnt;
         if (cnt) {
-            for (int k = beg + tid; k < end; k += nt) { const int p = A.order[k]; A.par[p] = p; }
+            for (int k = beg + tid; k < end; k += nt) { int ly, lx; const int p = db_entry<GL>(geo, A.order[k], ly, lx); A.par[p] = p; }
             g.sync();
             db_unite_level<GL, false>(g, geo, A, C, i, beg, end);
             g.sync();
         }
         if ((fm >> i) & 1ull) {
             for (int k = tid; k < end; k += nt) {
-                const int p = A.order[k];
+                int ly, lx;
+                const int p = db_entry<GL>(geo, A.order[k], ly, lx);
                 const int r = db_find<GL>(A.par, p);
                 if (A.frz[r] == i) A.obj[p] = r + 1;
             }
@@ -488,7 +509,8 @@ __device__ void db_candidate(const G &g, const DbArgs &a, const DbArr &A0, DbCtl
 
     // ---- object slots, record pool --------------------------------------------------------------------------------
     for (int k = tid; k < npix; k += nt) {
-        const int p = A.order[k];
+        int ly, lx;
+        const int p = db_entry<GL>(geo, A.order[k], ly, lx);
         if (A.frz[p]) A.st[p] = atomicAdd(&C->nslot, 1);
     }
     g.sync();
@@ -505,19 +527,13 @@ __device__ void db_candidate(const G &g, const DbArgs &a, const DbArr &A0, DbCtl
     // ---- D7: synchronous growth from a frontier -------------------------------------------------------------------
     int32_t *qr = A.T, *pend = A.accn, *F[2] = {A.lost, A.touched};
     for (int k = tid; k < npix; k += nt) {
-        const int p = A.order[k];
+        int ly, lx;
+        const int p = db_entry<GL>(geo, A.order[k], ly, lx);
         if (A.obj[p] == 0) {
-            int ly, lx;
-            geo.coords(p, ly, lx);
             bool near = false;
-            for (int dy = -1; dy <= 1; ++dy) {
-                if (ly + dy < 0 || ly + dy >= geo.bh) continue;
-                for (int dx = -1; dx <= 1; ++dx) {
-                    if ((dy == 0 && dx == 0) || lx + dx < 0 || lx + dx >= geo.bw) continue;
-                    const int q = p + dy * geo.pitch + dx;
-                    if (db_member<GL>(geo, A, q) && A.obj[q] != 0) near = true;
-                }
-            }
+            db_for_neighbours<GL>(geo, p, ly, lx, [&](int q, int, int) {
+                if (db_member<GL>(geo, A, q) && A.obj[q] != 0) near = true;
+            });
             qr[p] = near ? 1 : 0;
             if (near) F[0][atomicAdd(&C->n_f[0], 1)] = p;
         } else if (A.frz[p]) {
@@ -551,18 +567,13 @@ __device__ void db_candidate(const G &g, const DbArgs &a, const DbArr &A0, DbCtl
             geo.coords(p, ly, lx);
             float best = 0.f;
             int bo = 0;
-            for (int dy = -1; dy <= 1; ++dy) {
-                if (ly + dy < 0 || ly + dy >= geo.bh) continue;
-                for (int dx = -1; dx <= 1; ++dx) {
-                    if ((dy == 0 && dx == 0) || lx + dx < 0 || lx + dx >= geo.bw) continue;
-                    const int q = p + dy * geo.pitch + dx;
-                    if (!db_member<GL>(geo, A, q)) continue;
-                    const int oq = A.obj[q];
-                    if (oq == 0) continue;
-                    const float vq = __ldg(geo.sub + geo.fidx(ly + dy, lx + dx));
-                    if (bo == 0 || vq > best || (vq == best && oq < bo)) { best = vq; bo = oq; }
-                }
-            }
+            db_for_neighbours<GL>(geo, p, ly, lx, [&](int q, int dy, int dx) {
+                if (!db_member<GL>(geo, A, q)) return;
+                const int oq = A.obj[q];
+                if (oq == 0) return;
+                const float vq = __ldg(geo.sub + geo.fidx(ly + dy, lx + dx));
+                if (bo == 0 || vq > best || (vq == best && oq < bo)) { best = vq; bo = oq; }
+            });
             pend[p] = bo;
         }
         if (tid == 0) C->n_f[cur ^ 1] = 0;
@@ -573,15 +584,10 @@ __device__ void db_candidate(const G &g, const DbArgs &a, const DbArr &A0, DbCtl
             const int p = Fc[k];
             int ly, lx;
             geo.coords(p, ly, lx);
-            for (int dy = -1; dy <= 1; ++dy) {
-                if (ly + dy < 0 || ly + dy >= geo.bh) continue;
-                for (int dx = -1; dx <= 1; ++dx) {
-                    if ((dy == 0 && dx == 0) || lx + dx < 0 || lx + dx >= geo.bw) continue;
-                    const int q = p + dy * geo.pitch + dx;
-                    if (!db_member<GL>(geo, A, q) || A.obj[q] != 0) continue;
-                    if (atomicExch(&qr[q], round + 1) != round + 1) Fn[atomicAdd(&C->n_f[cur ^ 1], 1)] = q;
-                }
-            }
+            db_for_neighbours<GL>(geo, p, ly, lx, [&](int q, int, int) {
+                if (!db_member<GL>(geo, A, q) || A.obj[q] != 0) return;
+                if (atomicExch(&qr[q], round + 1) != round + 1) Fn[atomicAdd(&C->n_f[cur ^ 1], 1)] = q;
+            });
         }
         g.sync();
     }
@@ -589,7 +595,8 @@ __device__ void db_candidate(const G &g, const DbArgs &a, const DbArr &A0, DbCtl
     // ---- D8 + the records of the objects: one raster pass over the box, 32 consecutive pixels per warp step ---------
     int32_t *omin = A.T;   // (qr is done with)
     for (int k = tid; k < npix; k += nt) {
-        const int p = A.order[k];
+        int ly, lx;
+        const int p = db_entry<GL>(geo, A.order[k], ly, lx);
         if (A.frz[p]) omin[p] = INT_MAX;
     }
     g.sync();
@@ -641,9 +648,8 @@ __device__ void db_candidate(const G &g, const DbArgs &a, const DbArr &A0, DbCtl
     }
     g.sync();
     for (int k = tid; k < npix; k += nt) {
-        const int p = A.order[k];
         int ly, lx;
-        geo.coords(p, ly, lx);
+        const int p = db_entry<GL>(geo, A.order[k], ly, lx);
         const int r = A.obj[p] - 1;
         const int m = ldv<GL>(omin + r);
         labels[geo.fidx(ly, lx)] = m + 1;
@@ -676,26 +682,28 @@ __device__ __forceinline__ DbArr db_smem_arrays(char *base, int cap) {
 constexpr size_t db_smem_bytes(int cap) { return (size_t)cap * 42; }
 constexpr size_t DB_CTL_BYTES = (sizeof(DbCtl) + 15) / 16 * 16;
 
-// tier 0: one warp per candidate
-__global__ void __launch_bounds__(WARPS_PER_CTA * 32) k9_deblend_warp(DbArgs a) {
+// tiers 0, 1: one warp per candidate (tier 0: boxes of at most CAP_TINY cells -- half of all candidates -- with half the
+// shared memory per warp, so twice as many warps per SM hide the latency of this short, dependent code)
+template <int TIER, int CAP, int NWARPS>
+__global__ void __launch_bounds__(NWARPS * 32) k9_deblend_warp(DbArgs a) {
     extern __shared__ __align__(16) char smem[];
     const int warp = threadIdx.x >> 5;
     WarpGroup g;
     g.lane = threadIdx.x & 31;
-    char *mine = smem + (size_t)warp * (DB_CTL_BYTES + db_smem_bytes(CAP_WARP));
+    char *mine = smem + (size_t)warp * (DB_CTL_BYTES + db_smem_bytes(CAP));
     DbCtl *C = (DbCtl *)mine;
-    const DbArr A = db_smem_arrays(mine + DB_CTL_BYTES, CAP_WARP);
-    const uint32_t n = a.w.counters[C_TIER0 + 0];
+    const DbArr A = db_smem_arrays(mine + DB_CTL_BYTES, CAP);
+    const uint32_t n = a.w.counters[C_TIER0 + TIER];
     while (true) {
         uint32_t it = 0;
-        if (g.lane == 0) it = atomicAdd(&a.w.counters[C_CUR0 + 0], 1u);
+        if (g.lane == 0) it = atomicAdd(&a.w.counters[C_CUR0 + TIER], 1u);
         it = __shfl_sync(0xffffffffu, it, 0);
         if (it >= n) break;
-        db_candidate<false>(g, a, A, C, a.w.lists[it]);
+        db_candidate<false>(g, a, A, C, a.w.lists[(size_t)TIER * a.cap_in + it]);
     }
 }
 
-// tiers 1, 2: one thread block per candidate, arrays in shared memory
+// tiers 2, 3: one thread block per candidate, arrays in shared memory
 template <int TIER, int CAP, int NT>
 __global__ void __launch_bounds__(NT) k9_deblend_block(DbArgs a) {
     extern __shared__ __align__(16) char smem[];
@@ -713,21 +721,21 @@ __global__ void __launch_bounds__(NT) k9_deblend_block(DbArgs a) {
     }
 }
 
-// tier 3: one thread block per candidate, arrays in the workspace (frame coordinates)
+// tier 4: one thread block per candidate, arrays in the workspace (frame coordinates)
 __global__ void __launch_bounds__(512) k9_deblend_global(DbArgs a) {
     __shared__ DbCtl ctl;
     BlockGroup g;
     DbArr A;
     A.par = a.w.par; A.accn = a.w.accn; A.st = a.w.st; A.T = a.w.T; A.obj = a.w.obj; A.order = a.w.order; A.lost = a.w.lost;
     A.touched = a.w.touched; A.accf = a.w.accf; A.lvl = a.w.lvl; A.frz = a.w.frz;
-    const uint32_t n = a.w.counters[C_TIER0 + 3];
+    const uint32_t n = a.w.counters[C_TIER0 + 4];
     while (true) {
-        if (threadIdx.x == 0) ctl.item = (int)atomicAdd(&a.w.counters[C_CUR0 + 3], 1u);
+        if (threadIdx.x == 0) ctl.item = (int)atomicAdd(&a.w.counters[C_CUR0 + 4], 1u);
         __syncthreads();
         const uint32_t it = (uint32_t)ctl.item;
         __syncthreads();
         if (it >= n) break;
-        db_candidate<true>(g, a, A, &ctl, a.w.lists[(size_t)3 * a.cap_in + it]);
+        db_candidate<true>(g, a, A, &ctl, a.w.lists[(size_t)4 * a.cap_in + it]);
     }
 }
 
@@ -797,14 +805,18 @@ int k9_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H,
     BD_CUDA_CHECK(ctx, cudaMemsetAsync(a.w.counters, 0, a.w.zero_bytes, st));
     const int nsm = ctx->num_sms;
     k9_classify<<<nsm * 8, 256, 0, st>>>(a);
+    constexpr int TINY_WARPS = 16;
+    const size_t sm_tiny = TINY_WARPS * (DB_CTL_BYTES + db_smem_bytes(CAP_TINY));
     const size_t sm_warp = WARPS_PER_CTA * (DB_CTL_BYTES + db_smem_bytes(CAP_WARP));
     const size_t sm_mid = DB_CTL_BYTES + db_smem_bytes(CAP_MID), sm_big = DB_CTL_BYTES + db_smem_bytes(CAP_BIG);
-    BD_CUDA_CHECK(ctx, cudaFuncSetAttribute(k9_deblend_warp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_warp));
-    BD_CUDA_CHECK(ctx, cudaFuncSetAttribute(k9_deblend_block<1, CAP_MID, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_mid));
-    BD_CUDA_CHECK(ctx, cudaFuncSetAttribute(k9_deblend_block<2, CAP_BIG, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_big));
-    k9_deblend_warp<<<nsm * 2, WARPS_PER_CTA * 32, sm_warp, st>>>(a);
-    k9_deblend_block<1, CAP_MID, 128><<<nsm * 3, 128, sm_mid, st>>>(a);
-    k9_deblend_block<2, CAP_BIG, 512><<<nsm, 512, sm_big, st>>>(a);
+    BD_CUDA_CHECK(ctx, cudaFuncSetAttribute(k9_deblend_warp<0, CAP_TINY, TINY_WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_tiny));
+    BD_CUDA_CHECK(ctx, cudaFuncSetAttribute(k9_deblend_warp<1, CAP_WARP, WARPS_PER_CTA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_warp));
+    BD_CUDA_CHECK(ctx, cudaFuncSetAttribute(k9_deblend_block<2, CAP_MID, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_mid));
+    BD_CUDA_CHECK(ctx, cudaFuncSetAttribute(k9_deblend_block<3, CAP_BIG, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_big));
+    k9_deblend_warp<0, CAP_TINY, TINY_WARPS><<<nsm * 2, TINY_WARPS * 32, sm_tiny, st>>>(a);
+    k9_deblend_warp<1, CAP_WARP, WARPS_PER_CTA><<<nsm * 2, WARPS_PER_CTA * 32, sm_warp, st>>>(a);
+    k9_deblend_block<2, CAP_MID, 128><<<nsm * 3, 128, sm_mid, st>>>(a);
+    k9_deblend_block<3, CAP_BIG, 512><<<nsm, 512, sm_big, st>>>(a);
     k9_deblend_global<<<nsm * 2, 512, 0, st>>>(a);
     k5s_scan_blocks<<<1, 1024, 0, st>>>(a.w.blkcnt, a.w.NB, a.w.blkprefix, a.w.counters + 32);
     const int nb = nsm * 8 * 256 >= B ? nsm * 8 : (B + 255) / 256;
