@@ -21,9 +21,10 @@
 // round are looked at); a last raster pass over the box writes the new labels (1 + minimum raster index of the object,
 // D8) and reduces the objects' records (npix, flux, moments, peak, bbox: the quantities of step a5) with a segmented
 // warp reduction and one set of atomics per (warp, object).
-// Four tiers run the same code: a candidate whose bounding box has <= 256 pixels is one WARP's job with every array in
-// shared memory; <= 1536 and <= 5120 pixels: one thread block, arrays in shared memory; larger boxes: one thread block,
-// arrays in the workspace, indexed by frame coordinates (candidates are disjoint, so the frame-sized arrays serve all of
+// Five tiers run the same code, chosen by the cells of the candidate's bounding box plus a one-pixel border: <= 112 and
+// <= 256 cells: one WARP's job with every array in shared memory (32 resp. 16 warps per SM); <= 1536 and <= 5120: one
+// thread block, arrays in shared memory; larger boxes: one thread block, arrays in the workspace, indexed by frame
+// coordinates (candidates are disjoint, so the frame-sized arrays serve all of
 // them at once and cannot overflow).  Label maps are bit-exact by construction; node fluxes are float64 atomics (order
 // dependent in the last bits: decisions within 1e-9 of the contrast limit may differ from the definition).
 #include <limits.h>
