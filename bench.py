@@ -167,7 +167,20 @@ def run_reference(args, cfg, threads=None):
         nsrc = len(oracle.chain(img, p, cfg.detect_k, cfg.min_area)["cat"])
     dt = (time.perf_counter() - t0) / args.steps_ref
     mpix = crop[0] * crop[1] / dt / 1e6
+    # the oracle's steps one by one (same calls chain() makes), once
+    st = {}
+    t = time.perf_counter(); ms = oracle.mesh_stats(img, p); st["O1_mesh_stats"] = time.perf_counter() - t
+    t = time.perf_counter()
+    cb = oracle.spline_coeffs(oracle.grid_median(ms["bkg"], p.filt_h, p.filt_w)); cr = oracle.spline_coeffs(oracle.grid_median(ms["rms"], p.filt_h, p.filt_w))
+    st["O2_grid_filter_prefilter"] = time.perf_counter() - t
+    t = time.perf_counter()
+    bkg = oracle.spline_eval(cb, crop[0], crop[1], p.mesh_h, p.mesh_w); rms = oracle.spline_eval(cr, crop[0], crop[1], p.mesh_h, p.mesh_w)
+    st["O3_spline_eval"] = time.perf_counter() - t
+    t = time.perf_counter(); _, sub32, mask, _ = oracle.subtract_threshold(img, bkg, rms, cfg.detect_k); st["O4_subtract_threshold"] = time.perf_counter() - t
+    t = time.perf_counter(); lab = oracle.label(mask); st["O5_label"] = time.perf_counter() - t
+    t = time.perf_counter(); oracle.reduce_sources(lab, sub32, cfg.min_area); st["O6_reduce"] = time.perf_counter() - t
     return dict(value=mpix, unit="Mpix/s", cores=cores, kind="oracle", ms_per_step=dt * 1e3,
+                stages_ms={k: v * 1e3 for k, v in st.items()},
                 sample=f"top-left {crop[0]}x{crop[1]} crop of {cfg.name}, whole chain O1-O6, float64, {nsrc} sources")
 
 
@@ -331,7 +344,7 @@ def main():
                 "steps": args.steps_ref, "warmup": args.warmup_ref, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": cfg.name, "sample": r["sample"]},
-                "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+                "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample", "stages_ms")},
                 "e2e": {"value": r["value"], "unit": "Mpix/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
         print(json.dumps(line))
         return
@@ -463,9 +476,9 @@ def main():
         line["configs"] = others
     if not args.no_cpu_baseline and world == 1:
         r = run_reference(args, cfg)
-        line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample", "stages_ms")}
         r1 = run_reference(args, cfg, threads=1)
-        line["cpu_baseline"]["one_core"] = {"value": r1["value"], "unit": "Mpix/s", "cores": r1["cores"]}
+        line["cpu_baseline"]["one_core"] = {"value": r1["value"], "unit": "Mpix/s", "cores": r1["cores"], "stages_ms": r1["stages_ms"]}
     print(json.dumps(line))
     if dist: dist.destroy_process_group()
 
