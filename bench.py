@@ -257,6 +257,8 @@ class Workload:
         sampler.join(timeout=2.0)
         total_ms = t_start.elapsed_time(t_end)
         stage_ms = [float(np.mean([e[i].elapsed_time(e[i + 1]) for e in evs])) for i in range(3)]
+        per_step = sorted(e[0].elapsed_time(e[3]) for e in evs)   # device time of each step alone (without the gap to the next)
+        self.step_stats = {"median": float(per_step[len(per_step) // 2]), "best": float(per_step[0]), "worst": float(per_step[-1])}
         return total_ms, stage_ms, sampler.summary()
 
     def tile_kernel_ms(self, step, ev_tile, n=5):
@@ -310,6 +312,12 @@ def time_next_stages(bd, torch, ctx, wl, reps=3):
     out = {k: float(np.mean(v[1:])) for k, v in t.items()}
     out["objects"] = counts
     out["image_subtract_gflops"] = 2.0 * 441 * wl.npx / (out["image_subtract"] * 1e-3) / 1e9
+    # K8 is bound by the float32 FMA pipe (K8): peak = SMs x 128 FMA/clk x 2 flop x the SM clock of the run
+    prop = torch.cuda.get_device_properties(sub.device)
+    peak_tf = prop.multi_processor_count * 128 * 2 * 1.965e9 / 1e12
+    out["roofline_image_subtract"] = {"kernel": "k8_stamp_conv<10>", "bound": "alu", "achieved": out["image_subtract_gflops"] / 1e3, "peak": peak_tf,
+                                      "unit": "TFLOP/s", "frac": out["image_subtract_gflops"] / 1e3 / peak_tf,
+                                      "peak_source": "SMs x 128 FP32 FMA/clk x 2 x 1.965 GHz (B200_PROFILING.md unit counts and clocks)", "traffic": None}
     return out
 
 
@@ -441,6 +449,7 @@ def main():
         "stages_ms": ({"bkg_estimate": stage_ms[0], "bkg_subtract": stage_ms[1], "detect_sources": stage_ms[2]} if args.unfused else
                       {"bkg_estimate": stage_ms[0], "bkg_subtract_detect": stage_ms[1]}),
         "stages_ms_separate_calls": {"bkg_estimate": unfused_ms[0], "bkg_subtract": unfused_ms[1], "detect_sources": unfused_ms[2]},
+        "step_ms_device": wl.step_stats,
         "chain_roofline": chain_roofline(npx, ms_per_step),
         "roofline": {"kernel": "k4a_tile_label" + ("" if args.unfused else "<fused: a3 + a4 + partial sums of a5>"), "bound": "hbm",
                      "achieved": tile_gbs, "peak": peak, "unit": "GB/s", "frac": tile_gbs / peak, "frac_of_8000": tile_gbs / 8000.0,
