@@ -130,6 +130,26 @@ size_t k8_workspace_bytes(int B, const bd_conv_params *p);
 int k8_launch(bd_ctx *ctx, const float *d_ref, const float *d_img, int B, int H, int W, const bd_conv_params *p,
               const double *d_kcoef, const double *d_bgcoef, float *d_diff, float *d_conv, void *d_ws, cudaStream_t st);
 
+// ---- programmatic dependent launch (the small kernels that follow a large one on the same stream) ------------------
+// A kernel launched with bd_launch_pdl may become resident while its predecessor is still draining; it must call
+// bd_pdl_wait() before it touches anything the predecessor wrote (the wait returns when the whole predecessor grid has
+// completed and its memory is visible).  bd_pdl_trigger() in a kernel lets ITS successor start launching early.  Both are
+// no-ops for kernels launched the plain way.
+#ifdef __CUDACC__
+__device__ __forceinline__ void bd_pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void bd_pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+template <typename... KArgs, typename... Args>
+static inline cudaError_t bd_launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args &&...args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+#endif
+
 // ---- small device helpers ------------------------------------------------------------------------------
 #ifdef __CUDACC__
 __device__ __forceinline__ uint32_t f32_to_key(float f) {   // order-preserving map float32 -> uint32

@@ -723,6 +723,8 @@ __device__ __forceinline__ void g_union(int32_t *L, int a, int b) {
 // executes bit l of each (the unions are chains of dependent L2 accesses: one per lane, in parallel).
 __global__ void __launch_bounds__(256) k4b_seams(const uint32_t *edges, int32_t *labels, int H, int W, int TX, int TY,
                                                  size_t n_units) {
+    bd_pdl_wait();
+    bd_pdl_trigger();
     const size_t u = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (u >= n_units) return;
@@ -801,6 +803,8 @@ __device__ __forceinline__ void k5m_merge_into(const Rec *c, Rec *T, int cr, int
 
 __global__ void __launch_bounds__(256) k5m_merge_relabel(const uint32_t *counters, Rec *rec, const uint32_t *recidx,
                                                          int32_t *labels, int H, int W) {
+    bd_pdl_wait();
+    bd_pdl_trigger();
     const uint32_t n = counters[0];
     const int lane = threadIdx.x & 31;
     const size_t HW = (size_t)H * W;
@@ -859,6 +863,8 @@ __global__ void __launch_bounds__(256) k5m_merge_relabel(const uint32_t *counter
 // K5k: final roots with npix >= min_area -> bit in the per-pixel bitmap, count in the 4096-pixel block
 __global__ void __launch_bounds__(256) k5k_mark_kept(const uint32_t *counters, const Rec *rec, int H, int W, int min_area,
                                                      uint32_t *keptbits, uint32_t *blkcnt) {
+    bd_pdl_wait();
+    bd_pdl_trigger();
     const uint32_t n = counters[0];
     const size_t HW = (size_t)H * W;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
@@ -874,6 +880,7 @@ __global__ void __launch_bounds__(256) k5k_mark_kept(const uint32_t *counters, c
 __global__ void __launch_bounds__(256) k5f_finalize(const uint32_t *counters, const Rec *rec, int B, int H, int W,
                                                     int min_area, const uint32_t *keptbits, const uint32_t *blkprefix,
                                                     bd_source *cat, int64_t cap, int64_t *n_sources) {
+    bd_pdl_wait();
     const uint32_t n = counters[0];
     const size_t HW = (size_t)H * W;
     const size_t t0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -1001,15 +1008,17 @@ int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_
     if (ctx->dbg_ev1) cudaEventRecord(ctx->dbg_ev1, st);
     if (TX > 1 || TY > 1) {
         const size_t n_units = w.ntiles * 6;
-        k4b_seams<<<(unsigned)((n_units + 7) / 8), 256, 0, st>>>(w.edges, d_labels, H, W, TX, TY, n_units);
+        BD_CUDA_CHECK(ctx, bd_launch_pdl(k4b_seams, dim3((unsigned)((n_units + 7) / 8)), dim3(256), 0, st, w.edges, d_labels, H, W, TX, TY, n_units));
     }
     const int nb = ctx->num_sms * 32;
-    k5m_merge_relabel<<<nb, 256, 0, st>>>(w.counters, w.rec, w.recidx, d_labels, H, W);
-    k5k_mark_kept<<<nb, 256, 0, st>>>(w.counters, w.rec, H, W, min_area, w.keptbits, w.blkcnt);
-    k5s_scan_blocks<<<1, 1024, 0, st>>>(w.blkcnt, w.NB, w.blkprefix, w.counters + 1);
+    // the five small kernels of the tail are launched programmatically dependent: each becomes resident while its predecessor
+    // drains and waits (griddepcontrol.wait) for it to complete
+    BD_CUDA_CHECK(ctx, bd_launch_pdl(k5m_merge_relabel, dim3(nb), dim3(256), 0, st, w.counters, w.rec, w.recidx, d_labels, H, W));
+    BD_CUDA_CHECK(ctx, bd_launch_pdl(k5k_mark_kept, dim3(nb), dim3(256), 0, st, w.counters, w.rec, H, W, min_area, w.keptbits, w.blkcnt));
+    BD_CUDA_CHECK(ctx, bd_launch_pdl(k5s_scan_blocks, dim3(1), dim3(1024), 0, st, w.blkcnt, w.NB, w.blkprefix, w.counters + 1));
     const int nbf = nb * 256 >= B ? nb : (B + 255) / 256;
-    k5f_finalize<<<nbf, 256, 0, st>>>(w.counters, w.rec, B, H, W, min_area, w.keptbits, w.blkprefix,
-                                      d_cat, cat_capacity, d_n_sources);
+    BD_CUDA_CHECK(ctx, bd_launch_pdl(k5f_finalize, dim3(nbf), dim3(256), 0, st, w.counters, w.rec, B, H, W, min_area, w.keptbits, w.blkprefix,
+                                     d_cat, cat_capacity, d_n_sources));
     BD_CUDA_CHECK(ctx, cudaGetLastError());
     return BD_OK;
 }

@@ -10,6 +10,8 @@ constexpr int RB_SHIFT = 12;   // ranking blocks of 4096 pixels (128 bitmap word
 // the chunk is <= 32 counts), total -> *total_out.  cnt[] is readable up to the next multiple of 4 past n.
 __global__ void __launch_bounds__(1024) k5s_scan_blocks(const uint32_t *cnt, size_t n, uint32_t *prefix, uint32_t *total_out) {
     __shared__ uint32_t red[32];
+    bd_pdl_wait();      // (no-ops unless the kernel was launched programmatically dependent)
+    bd_pdl_trigger();
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const size_t per = (((n + 1023) / 1024) + 3) & ~(size_t)3, i0 = (size_t)tid * per, i1 = i0 + per < n ? i0 + per : n;
     const bool in_regs = per <= 32;
