@@ -34,6 +34,8 @@ __global__ void __launch_bounds__(K2_NT) k2a_window_median(const double *bkg_raw
     const int i0 = max(0, i - fw / 2), i1 = min(nx - 1, i + fw / 2);
     const int ww = i1 - i0 + 1, n = (j1 - j0 + 1) * ww;
     double *w = win[warp];
+    bd_pdl_wait();      // launched programmatically dependent on K1: the raw grids are read from here on
+    bd_pdl_trigger();
     for (int a = lane; a < n; a += 32) w[a] = __ldg(g + (size_t)(j0 + a / ww) * nx + i0 + a % ww);
     __syncwarp();
     const int k_lo = (n - 1) / 2, k_hi = n / 2;
@@ -166,8 +168,9 @@ __global__ void __launch_bounds__(K2_NT) k2b_spline_prefilter(int ny, int nx, do
     double *fac = scratch + ((size_t)frame * 2 + which) * k2_scratch_per_grid(ny, nx);   // global factors otherwise
     double *cp_y = in_smem ? s_cp[0] : fac, *im_y = in_smem ? s_im[0] : fac + ny;
     double *cp_x = in_smem ? s_cp[1] : fac + 2 * ny, *im_x = in_smem ? s_im[1] : fac + 2 * ny + nx;
-    if (threadIdx.x == K2_NT - 32) spline_factors(cp_y, im_y, ny);
+    if (threadIdx.x == K2_NT - 32) spline_factors(cp_y, im_y, ny);   // (depend on the grid shape only: computed while K2a drains)
     if (threadIdx.x == K2_NT - 64) spline_factors(cp_x, im_x, nx);
+    bd_pdl_wait();
     double *work = coef;
     int wp = nx;
     if (in_smem) {
@@ -201,10 +204,10 @@ int k2_launch(bd_ctx *ctx, const double *d_bkg_raw, const double *d_rms_raw, int
               cudaStream_t st) {
     const long long items = 2ll * B * ny * nx;
     const unsigned nblk = (unsigned)((items + K2_NT / 32 - 1) / (K2_NT / 32));
-    k2a_window_median<<<nblk, K2_NT, 0, st>>>(d_bkg_raw, d_rms_raw, B, ny, nx, fh, fw, d_bkg_mesh, d_rms_mesh, d_bkg_coef,
-                                             d_rms_coef);
+    BD_CUDA_CHECK(ctx, bd_launch_pdl(k2a_window_median, dim3(nblk), dim3(K2_NT), 0, st, d_bkg_raw, d_rms_raw, B, ny, nx, fh, fw, d_bkg_mesh,
+                                     d_rms_mesh, d_bkg_coef, d_rms_coef));
     dim3 grid(B, 2);
-    k2b_spline_prefilter<<<grid, K2_NT, 0, st>>>(ny, nx, d_bkg_coef, d_rms_coef, d_scratch);
+    BD_CUDA_CHECK(ctx, bd_launch_pdl(k2b_spline_prefilter, grid, dim3(K2_NT), 0, st, ny, nx, d_bkg_coef, d_rms_coef, d_scratch));
     BD_CUDA_CHECK(ctx, cudaGetLastError());
     return BD_OK;
 }

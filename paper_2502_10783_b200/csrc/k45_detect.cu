@@ -135,18 +135,19 @@ __device__ __forceinline__ uint32_t bytes_to_nibble(uint32_t v) {
 // The x-weights of a column and the y-weights of a row are the same for every tile that contains them: computed once
 // per call (fused mode) with the functions K3 uses, instead of 5 float64 polynomial evaluations per thread per tile.
 __global__ void k_spline_tabs(int H, int W, int mh, int mw, float *wx_tab, double *wy_tab, int32_t *i0_tab, int32_t *j0_tab) {
+    // launched programmatically dependent: the weights are computed while the predecessor on the stream drains, the stores wait
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    int i0 = 0, j0 = 0;
+    float wx[4] = {0.f, 0.f, 0.f, 0.f};
+    double wy[4] = {0.0, 0.0, 0.0, 0.0};
+    if (t < W) { i0 = spl_cell_of(t, mw); spl_x_weights(t, mw, i0, wx); }
+    if (t < H) { j0 = spl_cell_of(t, mh); spl_y_weights(t, mh, j0, wy); }
+    bd_pdl_wait();
     if (t < W) {
-        const int i0 = spl_cell_of(t, mw);
-        float wx[4];
-        spl_x_weights(t, mw, i0, wx);
         reinterpret_cast<float4 *>(wx_tab)[t] = make_float4(wx[0], wx[1], wx[2], wx[3]);
         i0_tab[t] = i0;
     }
     if (t < H) {
-        const int j0 = spl_cell_of(t, mh);
-        double wy[4];
-        spl_y_weights(t, mh, j0, wy);
         wy_tab[4 * t + 0] = wy[0]; wy_tab[4 * t + 1] = wy[1]; wy_tab[4 * t + 2] = wy[2]; wy_tab[4 * t + 3] = wy[3];
         j0_tab[t] = j0;
     }
@@ -951,8 +952,6 @@ int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_
         k_make_mask<<<(unsigned)((n4 + 255) / 256), 256, 0, st>>>(d_sub, d_rms, n4, (float)detect_k, w.maskbuf);
         mask = w.maskbuf;
     }
-    BD_CUDA_CHECK(ctx, cudaMemsetAsync(w.counters, 0, 64 * sizeof(uint32_t), st));
-    BD_CUDA_CHECK(ctx, cudaMemsetAsync(w.keptbits, 0, w.zero_bytes, st));
 
     const int TX = (W + TW - 1) / TW, TY = (H + TH - 1) / TH;
     K4Args a;
@@ -970,8 +969,11 @@ int k45_launch(bd_ctx *ctx, const float *d_sub, const float *d_rms, const uint8_
         a.sub = fz->sub;
         a.wx_tab = w.wx_tab; a.wy_tab = w.wy_tab; a.i0_tab = w.i0_tab; a.j0_tab = w.j0_tab;
         const int nt_tabs = W > H ? W : H;
-        k_spline_tabs<<<(nt_tabs + 255) / 256, 256, 0, st>>>(H, W, fz->mh, fz->mw, w.wx_tab, w.wy_tab, w.i0_tab, w.j0_tab);
+        BD_CUDA_CHECK(ctx, bd_launch_pdl(k_spline_tabs, dim3((nt_tabs + 255) / 256), dim3(256), 0, st, H, W, fz->mh, fz->mw, w.wx_tab, w.wy_tab,
+                                         w.i0_tab, w.j0_tab));
     }
+    BD_CUDA_CHECK(ctx, cudaMemsetAsync(w.counters, 0, 64 * sizeof(uint32_t), st));
+    BD_CUDA_CHECK(ctx, cudaMemsetAsync(w.keptbits, 0, w.zero_bytes, st));
     a.use_tma = (W >= TW && H >= TH && ctx->encode_tiled) ? 1 : 0;
     CUtensorMap tmap;
     memset(&tmap, 0, sizeof(tmap));
