@@ -151,20 +151,24 @@ __device__ void spline_line(double *f, const double *cp, const double *im, int n
 }
 
 // One CTA per (frame, grid), in place on the coefficient array (which K2a filled with the filtered grid).
-// The grid is staged in shared memory when it fits (K2_SMEM_CELLS cells, padded rows so that the x sweep,
-// where thread j walks row j, is free of bank conflicts); otherwise the same code runs on global memory.
-constexpr int K2_SMEM_CELLS = 4096;
+// The grid is staged in (dynamic) shared memory when it fits (up to K2_SMEM_DOUBLES cells incl. the row padding: 144 x 144;
+// padded rows so that the x sweep, where thread j walks row j, is free of bank conflicts); otherwise the same code runs on
+// global memory (126 us instead of ~15 for the 96 x 96 grid of config 5, which the first, 4096-cell limit sent there).
+constexpr int K2_SMEM_DOUBLES = 20736 + 144;
+constexpr int K2_SMEM_LINE = 160;   // longest line whose Thomas factors sit in shared memory
+
+__host__ __device__ inline bool k2b_in_smem(int ny, int nx) { return ny * (nx | 1) <= K2_SMEM_DOUBLES && ny <= K2_SMEM_LINE && nx <= K2_SMEM_LINE; }
 
 __global__ void __launch_bounds__(K2_NT) k2b_spline_prefilter(int ny, int nx, double *bkg_coef, double *rms_coef,
                                                               double *scratch) {
-    __shared__ double s_work[K2_SMEM_CELLS + 128];
-    __shared__ double s_cp[2][128], s_im[2][128];
+    extern __shared__ double s_work[];
+    __shared__ double s_cp[2][K2_SMEM_LINE], s_im[2][K2_SMEM_LINE];
     const int frame = blockIdx.x, which = blockIdx.y;
     const size_t goff = (size_t)frame * ny * nx;
     double *coef = (which ? rms_coef : bkg_coef) + goff;
     const int cells = ny * nx;
     const int pitch = nx | 1;   // odd pitch
-    const bool in_smem = ny * pitch <= K2_SMEM_CELLS + 128 && ny <= 128 && nx <= 128;
+    const bool in_smem = k2b_in_smem(ny, nx);
     double *fac = scratch + ((size_t)frame * 2 + which) * k2_scratch_per_grid(ny, nx);   // global factors otherwise
     double *cp_y = in_smem ? s_cp[0] : fac, *im_y = in_smem ? s_im[0] : fac + ny;
     double *cp_x = in_smem ? s_cp[1] : fac + 2 * ny, *im_x = in_smem ? s_im[1] : fac + 2 * ny + nx;
@@ -207,7 +211,9 @@ int k2_launch(bd_ctx *ctx, const double *d_bkg_raw, const double *d_rms_raw, int
     BD_CUDA_CHECK(ctx, bd_launch_pdl(k2a_window_median, dim3(nblk), dim3(K2_NT), 0, st, d_bkg_raw, d_rms_raw, B, ny, nx, fh, fw, d_bkg_mesh,
                                      d_rms_mesh, d_bkg_coef, d_rms_coef));
     dim3 grid(B, 2);
-    BD_CUDA_CHECK(ctx, bd_launch_pdl(k2b_spline_prefilter, grid, dim3(K2_NT), 0, st, ny, nx, d_bkg_coef, d_rms_coef, d_scratch));
+    const size_t smem_b = k2b_in_smem(ny, nx) ? (size_t)ny * (nx | 1) * sizeof(double) : 0;
+    BD_CUDA_CHECK(ctx, cudaFuncSetAttribute(k2b_spline_prefilter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(K2_SMEM_DOUBLES * sizeof(double))));
+    BD_CUDA_CHECK(ctx, bd_launch_pdl(k2b_spline_prefilter, grid, dim3(K2_NT), smem_b, st, ny, nx, d_bkg_coef, d_rms_coef, d_scratch));
     BD_CUDA_CHECK(ctx, cudaGetLastError());
     return BD_OK;
 }

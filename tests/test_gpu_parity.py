@@ -111,7 +111,7 @@ def test_k1_degenerate_inputs(bd, ctx):
 
 # ------------------------------------------------------------------------------------------- K2
 @pytest.mark.parametrize("ny,nx,fh,fw", [(8, 8, 3, 3), (37, 36, 5, 5), (2, 3, 3, 3), (1, 5, 5, 1), (96, 96, 3, 3),
-                                         (1, 1, 3, 3), (5, 9, 1, 1), (40, 300, 11, 7)])
+                                         (1, 1, 3, 3), (5, 9, 1, 1), (40, 300, 11, 7), (144, 143, 3, 5), (150, 100, 3, 3), (161, 40, 3, 3)])
 def test_k2_filter_and_prefilter(bd, ctx, ny, nx, fh, fw):
     rng = np.random.default_rng(ny * 100 + nx)
     B = 3
