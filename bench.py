@@ -276,7 +276,7 @@ class Workload:
         self.torch.cuda.empty_cache()
 
 
-def time_next_stages(bd, torch, ctx, wl, reps=3):
+def time_next_stages(bd, torch, ctx, wl, reps=5):
     """deblend_sources, clean_sources, photometry and image_subtract on the maps of the last step (outside the timed region)."""
     cfg, cap = wl.cfg, wl.cap
     sub, rms = wl.o3["sub"], wl.o3["rms"]
@@ -285,6 +285,11 @@ def time_next_stages(bd, torch, ctx, wl, reps=3):
     nb = bd.C.c_size_t()
     ctx.check(ctx.lib.bd_deblend_workspace_bytes(ctx.h, wl.B, wl.H, wl.W, bd.C.c_int64(cap), bd.C.c_int64(cap), bd.C.byref(nb)))
     ws = torch.empty(nb.value, dtype=torch.uint8, device=sub.device)
+    ctx.check(ctx.lib.bd_clean_workspace_bytes(ctx.h, wl.B, wl.H, wl.W, bd.C.c_int64(cap), bd.C.byref(nb)))
+    ws_c = torch.empty(nb.value, dtype=torch.uint8, device=sub.device)
+    ctx.check(ctx.lib.bd_phot_workspace_bytes(ctx.h, bd.C.c_int64(cap), bd.C.byref(nb)))
+    ws_p = torch.empty(nb.value, dtype=torch.uint8, device=sub.device)
+    phot = torch.zeros(cap * bd.PHOT_DTYPE.itemsize, dtype=torch.uint8, device=sub.device)
     t = {"deblend_sources": [], "clean_sources": [], "photometry": [], "image_subtract": []}
     counts = {}
     cp = bd.ConvParams()
@@ -299,9 +304,9 @@ def time_next_stages(bd, torch, ctx, wl, reps=3):
         e[0].record()
         d = bd.deblend_sources(ctx, sub, rms, lab, wl.o5["cat"], wl.o5["n_sources"], cap, cfg.detect_k, cfg.min_area, ws=ws)
         e[1].record()
-        c = bd.clean_sources(ctx, rms, lab, d["cat"], d["n_sources"], cap, cfg.detect_k)
+        c = bd.clean_sources(ctx, rms, lab, d["cat"], d["n_sources"], cap, cfg.detect_k, ws=ws_c)
         e[2].record()
-        bd.photometry(ctx, sub, rms, c["cat"], c["n_sources"], cap)
+        bd.photometry(ctx, sub, rms, c["cat"], c["n_sources"], cap, out=phot, ws=ws_p)
         e[3].record()
         bd.image_subtract(ctx, wl.imgs[0], wl.imgs[0], cp, kcoef, bgcoef, out=dict(diff=diff))
         e[4].record()
@@ -309,7 +314,7 @@ def time_next_stages(bd, torch, ctx, wl, reps=3):
         for i, k in enumerate(t):
             t[k].append(e[i].elapsed_time(e[i + 1]))
         counts = {"candidates": int(wl.o5["n_sources"].sum()), "deblended": int(d["n_sources"].sum()), "cleaned": int(c["n_sources"].sum())}
-    out = {k: float(np.mean(v[1:])) for k, v in t.items()}
+    out = {k: float(np.median(v[1:])) for k, v in t.items()}   # (workspaces are allocated once, outside the timed calls)
     out["objects"] = counts
     out["image_subtract_gflops"] = 2.0 * 441 * wl.npx / (out["image_subtract"] * 1e-3) / 1e9
     # K8 is bound by the float32 FMA pipe (K8): peak = SMs x 128 FMA/clk x 2 flop x the SM clock of the run

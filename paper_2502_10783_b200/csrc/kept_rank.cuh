@@ -6,55 +6,46 @@
 
 constexpr int RB_SHIFT = 12;   // ranking blocks of 4096 pixels (128 bitmap words)
 
-// K5s: exclusive scan of the block counts (one CTA; thread t owns a contiguous chunk, held in registers when
-// the chunk is <= 32 counts), total -> *total_out.  cnt[] is readable up to the next multiple of 4 past n.
+// K5s: exclusive scan of the block counts, total -> *total_out.  One CTA walks the array in tiles of 4096 counts: coalesced
+// 128-bit loads, a shuffle scan per warp, the 32 warp totals through shared memory, a running carry, coalesced 128-bit stores.
+// (The first version gave every thread one contiguous chunk: fine while a chunk was <= 32 counts held in registers, but the
+// 65 536 blocks of config 4 and the 83 k cells of K10 on config 3 took its scalar path with a 256-byte stride between
+// neighbouring threads: 121 us.)  cnt[] is readable and prefix[] writable up to the next multiple of 4 past n (+ 1).
 __global__ void __launch_bounds__(1024) k5s_scan_blocks(const uint32_t *cnt, size_t n, uint32_t *prefix, uint32_t *total_out) {
     __shared__ uint32_t red[32];
     bd_pdl_wait();      // (no-ops unless the kernel was launched programmatically dependent)
     bd_pdl_trigger();
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const size_t per = (((n + 1023) / 1024) + 3) & ~(size_t)3, i0 = (size_t)tid * per, i1 = i0 + per < n ? i0 + per : n;
-    const bool in_regs = per <= 32;
-    uint4 v[8];
-    uint32_t local = 0;
-    if (in_regs) {
-#pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            v[k] = make_uint4(0, 0, 0, 0);
-            const size_t i = i0 + 4 * k;
-            if (4 * k < (int)per && i < n) {
-                v[k] = *reinterpret_cast<const uint4 *>(cnt + i);
-                if (i + 1 >= n) v[k].y = 0;
-                if (i + 2 >= n) v[k].z = 0;
-                if (i + 3 >= n) v[k].w = 0;
-            }
-            local += v[k].x + v[k].y + v[k].z + v[k].w;
+    uint32_t carry = 0;
+    for (size_t base = 0; base < n; base += 4096) {
+        const size_t i = base + 4 * (size_t)tid;
+        uint4 v = make_uint4(0, 0, 0, 0);
+        if (i < n) {
+            v = *reinterpret_cast<const uint4 *>(cnt + i);
+            if (i + 1 >= n) v.y = 0;
+            if (i + 2 >= n) v.z = 0;
+            if (i + 3 >= n) v.w = 0;
         }
-    } else {
-        for (size_t i = i0; i < i1; ++i) local += cnt[i];
-    }
-    uint32_t incl = local;
+        const uint32_t local = v.x + v.y + v.z + v.w;
+        uint32_t incl = local;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
-    if (lane == 31) red[warp] = incl;
-    __syncthreads();
-    uint32_t run = incl - local, tot = 0;
-    for (int w = 0; w < 32; ++w) { if (w < warp) run += red[w]; tot += red[w]; }
-    if (in_regs) {
+        for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
+        if (lane == 31) red[warp] = incl;
+        __syncthreads();
+        uint32_t mine = red[lane], wincl = mine;   // every warp scans the 32 warp totals itself
 #pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            const size_t i = i0 + 4 * k;
-            if (4 * k < (int)per && i < n) {
-                uint4 o;
-                o.x = run; run += v[k].x; o.y = run; run += v[k].y; o.z = run; run += v[k].z; o.w = run; run += v[k].w;
-                *reinterpret_cast<uint4 *>(prefix + i) = o;   // prefix[] has room up to the next multiple of 4 past n + 1
-            }
+        for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, wincl, o); if (lane >= o) wincl += t; }
+        const uint32_t wbase = __shfl_sync(0xffffffffu, wincl - mine, warp), tot = __shfl_sync(0xffffffffu, wincl, 31);
+        if (i < n) {
+            uint4 o;
+            uint32_t run = carry + wbase + incl - local;
+            o.x = run; run += v.x; o.y = run; run += v.y; o.z = run; run += v.z; o.w = run;
+            *reinterpret_cast<uint4 *>(prefix + i) = o;
         }
-    } else {
-        for (size_t i = i0; i < i1; ++i) { const uint32_t c = cnt[i]; prefix[i] = run; run += c; }
+        carry += tot;
+        __syncthreads();
     }
-    __syncthreads();
-    if (tid == 0) { prefix[n] = tot; *total_out = tot; }
+    if (tid == 0) { prefix[n] = carry; *total_out = carry; }
 }
 
 // number of kept roots with global pixel index < g: block prefix + popcount of the block's bitmap words below g
