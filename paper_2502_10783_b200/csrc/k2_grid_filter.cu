@@ -64,6 +64,44 @@ __global__ void __launch_bounds__(K2_NT) k2a_window_median(const double *bkg_raw
     }
 }
 
+// Windows of at most 9 cells (the 3 x 3 filter of configs 1, 2, 4, 5): one THREAD per (frame, grid, cell), the window in
+// registers, the same rank rule.  (A warp per cell is 131 072 warps for the 64 frames of config 4: 53 us.)
+__global__ void __launch_bounds__(K2_NT) k2a_window_median_small(const double *bkg_raw, const double *rms_raw, int B, int ny,
+                                                                 int nx, int fh, int fw, float *bkg_mesh, float *rms_mesh,
+                                                                 double *bkg_work, double *rms_work) {
+    const int cells = ny * nx;
+    const long long item = (long long)blockIdx.x * K2_NT + threadIdx.x;   // (frame, which, cell)
+    if (item >= 2ll * B * cells) return;
+    const int c = (int)(item % cells);
+    const int which = (int)((item / cells) & 1);
+    const int frame = (int)(item / (2ll * cells));
+    const size_t goff = (size_t)frame * cells;
+    const int j = c / nx, i = c - j * nx;
+    const int j0 = max(0, j - fh / 2), j1 = min(ny - 1, j + fh / 2);
+    const int i0 = max(0, i - fw / 2), i1 = min(nx - 1, i + fw / 2);
+    const int ww = i1 - i0 + 1, n = (j1 - j0 + 1) * ww;
+    bd_pdl_wait();
+    bd_pdl_trigger();
+    const double *g = (which ? rms_raw : bkg_raw) + goff;
+    double w[9];
+#pragma unroll
+    for (int a = 0; a < 9; ++a) w[a] = a < n ? __ldg(g + (size_t)(j0 + a / ww) * nx + i0 + a % ww) : 0.0;
+    const int k_lo = (n - 1) / 2, k_hi = n / 2;
+    double lo = 0.0, hi = 0.0;
+#pragma unroll
+    for (int a = 0; a < 9; ++a) {
+        int rank = 0;
+#pragma unroll
+        for (int b = 0; b < 9; ++b) rank += (b < n && (w[b] < w[a] || (w[b] == w[a] && b < a))) ? 1 : 0;
+        if (a < n && rank == k_lo) lo = w[a];
+        if (a < n && rank == k_hi) hi = w[a];
+    }
+    const double med = (n & 1) ? lo : 0.5 * (lo + hi);
+    (which ? rms_work : bkg_work)[goff + c] = med;
+    float *mesh = which ? rms_mesh : bkg_mesh;
+    if (mesh) mesh[goff + c] = (float)med;
+}
+
 // ---- K2f: invalid cells (NaN: background variants, reading B3) take the median of the VALID cells of the smallest square
 // window (2r+1)^2, r = 1, 2, ..., truncated at the grid border, that holds one; both grids, read from the unfilled grids.
 // One thread per cell: an invalid cell is rare and its window is a handful of cells (rank counting, as in K2a).
@@ -208,8 +246,12 @@ int k2_launch(bd_ctx *ctx, const double *d_bkg_raw, const double *d_rms_raw, int
               cudaStream_t st) {
     const long long items = 2ll * B * ny * nx;
     const unsigned nblk = (unsigned)((items + K2_NT / 32 - 1) / (K2_NT / 32));
-    BD_CUDA_CHECK(ctx, bd_launch_pdl(k2a_window_median, dim3(nblk), dim3(K2_NT), 0, st, d_bkg_raw, d_rms_raw, B, ny, nx, fh, fw, d_bkg_mesh,
-                                     d_rms_mesh, d_bkg_coef, d_rms_coef));
+    if (fh * fw <= 9)
+        BD_CUDA_CHECK(ctx, bd_launch_pdl(k2a_window_median_small, dim3((unsigned)((items + K2_NT - 1) / K2_NT)), dim3(K2_NT), 0, st, d_bkg_raw,
+                                         d_rms_raw, B, ny, nx, fh, fw, d_bkg_mesh, d_rms_mesh, d_bkg_coef, d_rms_coef));
+    else
+        BD_CUDA_CHECK(ctx, bd_launch_pdl(k2a_window_median, dim3(nblk), dim3(K2_NT), 0, st, d_bkg_raw, d_rms_raw, B, ny, nx, fh, fw, d_bkg_mesh,
+                                         d_rms_mesh, d_bkg_coef, d_rms_coef));
     dim3 grid(B, 2);
     const size_t smem_b = k2b_in_smem(ny, nx) ? (size_t)ny * (nx | 1) * sizeof(double) : 0;
     BD_CUDA_CHECK(ctx, cudaFuncSetAttribute(k2b_spline_prefilter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(K2_SMEM_DOUBLES * sizeof(double))));
