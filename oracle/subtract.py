@@ -80,28 +80,35 @@ def stamp_kernel(p: ConvParams, kcoef: np.ndarray, H: int, W: int, sx: int, sy: 
     return np.tensordot(a, basis, axes=1)
 
 
-def subtract(ref: np.ndarray, img: np.ndarray, p: ConvParams, kcoef: np.ndarray, bgcoef: np.ndarray):
+def subtract(ref: np.ndarray, img: np.ndarray, p: ConvParams, kcoef: np.ndarray, bgcoef: np.ndarray, only=None):
     """O9 for one frame pair.  ref, img float32 [H, W]; kcoef [N, n_poly(ds)], bgcoef [n_poly(db)] float64.
+    `only`: optional iterable of stamps (sy, sx); the other stamps are not computed (their pixels stay 0 in both outputs) --
+    a sampling facility for full-size frames, the arithmetic of a computed stamp is the same.
     -> (diff float64 [H, W], conv float64 [H, W])."""
-    ref = np.asarray(ref, dtype=np.float64)
-    img = np.asarray(img, dtype=np.float64)
+    ref = np.asarray(ref, dtype=np.float64) if only is None else ref
+    img = np.asarray(img, dtype=np.float64) if only is None else img
     H, W = ref.shape
     hw = p.half_width
     S = 2 * hw + 1
     basis = basis_kernels(p)
-    pad = np.zeros((H + 2 * hw, W + 2 * hw))
-    pad[hw:hw + H, hw:hw + W] = ref                          # C4: R = 0 outside the frame
+    stamps = [(sy, sx) for sy in range((H + S - 1) // S) for sx in range((W + S - 1) // S)] if only is None else [(int(a), int(b)) for a, b in only]
     conv = np.zeros((H, W))
-    for sy in range((H + S - 1) // S):
-        for sx in range((W + S - 1) // S):
-            K = stamp_kernel(p, kcoef, H, W, sx, sy, basis)
-            y0, y1, x0, x1 = sy * S, min((sy + 1) * S, H), sx * S, min((sx + 1) * S, W)
-            acc = np.zeros((y1 - y0, x1 - x0))
-            for v in range(-hw, hw + 1):
-                for u in range(-hw, hw + 1):
-                    # R(x - u, y - v) for the pixels of the stamp, in padded coordinates
-                    acc += K[v + hw, u + hw] * pad[y0 - v + hw:y1 - v + hw, x0 - u + hw:x1 - u + hw]
-            conv[y0:y1, x0:x1] = acc
-    yy, xx = np.mgrid[:H, :W].astype(np.float64)
-    bg = poly_eval(np.asarray(bgcoef, dtype=np.float64), p.bg_order, (2.0 * xx - (W - 1)) / W, (2.0 * yy - (H - 1)) / H)
-    return img + bg - conv, conv
+    diff = np.zeros((H, W))
+    bgc = np.asarray(bgcoef, dtype=np.float64)
+    for sy, sx in stamps:
+        K = stamp_kernel(p, kcoef, H, W, sx, sy, basis)
+        y0, y1, x0, x1 = sy * S, min((sy + 1) * S, H), sx * S, min((sx + 1) * S, W)
+        # the template around the stamp, padded with zeros where it leaves the frame (C4: R = 0 outside the frame)
+        pad = np.zeros((y1 - y0 + 2 * hw, x1 - x0 + 2 * hw))
+        ya, yb, xa, xb = max(y0 - hw, 0), min(y1 + hw, H), max(x0 - hw, 0), min(x1 + hw, W)
+        pad[ya - (y0 - hw):yb - (y0 - hw), xa - (x0 - hw):xb - (x0 - hw)] = ref[ya:yb, xa:xb]
+        acc = np.zeros((y1 - y0, x1 - x0))
+        for v in range(-hw, hw + 1):
+            for u in range(-hw, hw + 1):
+                # R(x - u, y - v) for the pixels of the stamp, in the coordinates of the padded patch
+                acc += K[v + hw, u + hw] * pad[hw - v:hw - v + (y1 - y0), hw - u:hw - u + (x1 - x0)]
+        conv[y0:y1, x0:x1] = acc
+        yy, xx = np.mgrid[y0:y1, x0:x1].astype(np.float64)
+        bg = poly_eval(bgc, p.bg_order, (2.0 * xx - (W - 1)) / W, (2.0 * yy - (H - 1)) / H)
+        diff[y0:y1, x0:x1] = np.asarray(img[y0:y1, x0:x1], dtype=np.float64) + bg - acc
+    return diff, conv

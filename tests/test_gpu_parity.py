@@ -844,6 +844,37 @@ def test_k8_stamp_convolution_against_oracle(bd, ctx, H, W, B, kw):
     assert o2["conv"] is None and torch.equal(o2["diff"], out["diff"])
 
 
+def test_k8_full_size_config3_sampled(bd, ctx):
+    """K8 on the full 9216 x 9232 frame of config 3 (the launch configuration bench.py times, default 21 x 21 stamps with
+    spatially varying kernels): 60 seeded stamps plus the four corner stamps, the last (partial) stamp row and column, against
+    the oracle computed for those stamps only."""
+    cfg = CONFIGS[3]
+    ref = make_frames(cfg)
+    B, H, W = ref.shape
+    p = bd.ConvParams()
+    op = osub.ConvParams()
+    rng = np.random.default_rng(77)
+    img = (ref * np.float32(1.02) + rng.normal(5, 3, size=ref.shape).astype(np.float32)).astype(np.float32)
+    kc = rng.normal(0, 0.01, size=(B, p.n_basis, p.n_sp))
+    kc[:, 0, 0] += 0.7
+    bc = rng.normal(0, 3, size=(B, p.n_bg))
+    out = bd.image_subtract(ctx, dev(ref), dev(img), p, dev(kc), dev(bc), want_conv=True)
+    torch.cuda.synchronize()
+    S = 2 * p.half_width + 1
+    nsy, nsx = (H + S - 1) // S, (W + S - 1) // S
+    stamps = {(0, 0), (0, nsx - 1), (nsy - 1, 0), (nsy - 1, nsx - 1), (nsy - 1, nsx // 2), (nsy // 2, nsx - 1)}
+    stamps |= {(int(a), int(b)) for a, b in zip(rng.integers(0, nsy, 60), rng.integers(0, nsx, 60))}
+    diff, conv = osub.subtract(ref[0], img[0], op, kc[0], bc[0], only=sorted(stamps))
+    g_conv, g_diff = out["conv"][0].cpu().numpy(), out["diff"][0].cpu().numpy()
+    rmax = float(np.abs(ref[0]).max())
+    for sy, sx in sorted(stamps):
+        sl = (slice(sy * S, min((sy + 1) * S, H)), slice(sx * S, min((sx + 1) * S, W)))
+        tol = 3e-6 * np.abs(osub.stamp_kernel(op, kc[0], H, W, sx, sy)).sum() * rmax
+        e1, e2 = np.abs(g_conv[sl] - conv[sl]), np.abs(g_diff[sl] - diff[sl])
+        assert np.all(e1 <= tol), f"stamp {(sy, sx)} conv: worst {e1.max() / tol:.2f} x tol"
+        assert np.all(e2 <= tol + 1e-6 * np.abs(diff[sl]) + 1e-4), f"stamp {(sy, sx)} diff"
+
+
 def test_k8_impulse_and_identity(bd, ctx):
     """Properties through the GPU path alone: a delta template returns the stamp's kernel (orientation: convolution, not
     correlation); a delta KERNEL (a_0 = 1 on a very narrow Gaussian) returns the template, so diff = I + B - R exactly."""
