@@ -794,6 +794,31 @@ def test_bkg_iterate_stage_parity(bd, ctx, cid, H, W, mesh, grow, n_iter):
     assert np.max(np.abs(bm[0].cpu().numpy() - ob["bkg_grid"]) / np.abs(ob["bkg_grid"])) < 1e-4
 
 
+def test_bkg_iterate_full_size_config3(bd, ctx):
+    """NEXT-3 at BASELINE.json's full size (9216 x 9232, mesh 256, filter 5 x 5) with a bad-pixel mask (1 % random pixels and
+    blobs): one re-estimation.  (i) the exclusion mask equals oracle.dilate(the library's own first mask) | bad0, bit for bit;
+    (ii) validity flags, filtered grids and spline coefficients equal the oracle's masked estimate under that mask."""
+    cfg = CONFIGS[3]
+    rng = np.random.default_rng(43)
+    img = make_frames(cfg)
+    bad0 = _bad_mask(rng, img.shape, 0.01, blobs=6)
+    p = params_for(bd, cfg)
+    px, opx = bd.BkgXParams(grow=1), oracle.BkgXParams(grow=1)
+    d_img, d_bad = dev(img), dev(bad0)
+    bm, rm, cb, cr, valid, bad_out = bd.bkg_iterate(ctx, d_img, d_bad, p, px, cfg.detect_k, 1)
+    _, _, cb0, cr0, _ = bd.bkg_estimate_masked(ctx, d_img, d_bad, p, px)
+    m0 = bd.bkg_subtract(ctx, d_img, p.mesh_h, p.mesh_w, cb0, cr0, cfg.detect_k, want_bkg=False)["mask"][0].cpu().numpy()
+    torch.cuda.synchronize()
+    bad_g = bad_out[0].cpu().numpy()
+    assert np.array_equal(bad_g, obv.dilate(m0, 1) | (bad0[0] != 0))
+    b = obv.background_masked(img[0], bad_g, to_oracle_params(p), opx)
+    assert np.array_equal(valid[0].cpu().numpy(), b["valid"])
+    assert np.max(np.abs(bm[0].cpu().numpy() - b["bkg_grid"]) / np.abs(b["bkg_grid"])) < 1e-6
+    assert np.max(np.abs(rm[0].cpu().numpy() - b["rms_grid"]) / np.abs(b["rms_grid"])) < 1e-6
+    assert np.max(np.abs(cb[0].cpu().numpy() - b["bkg_coef"])) <= 1e-9 * np.max(np.abs(b["bkg_coef"]))
+    assert np.max(np.abs(cr[0].cpu().numpy() - b["rms_coef"])) <= 1e-9 * np.max(np.abs(b["rms_coef"]))
+
+
 # ------------------------------------------------------------------------------------------- NEXT-4: stamp convolution (K8)
 from oracle import subtract as osub  # noqa: E402
 
