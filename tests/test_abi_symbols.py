@@ -48,6 +48,8 @@ def test_struct_layouts_match_header():
     assert m.SOURCE_DTYPE.itemsize == 88 and m.SOURCE_DTYPE.fields["flux"][1] == 40
     assert ctypes.sizeof(m._CParams) == 48   # 4 x i32, f64, 2 x i32, 2 x f64
     assert m.PHOT_DTYPE.itemsize == 56 and m.PHOT_DTYPE.fields["npix_auto"][1] == 48 and ctypes.sizeof(m._CPhotParams) == 40
+    assert ctypes.sizeof(m._CDeblendParams) == 32 and m._CDeblendParams.min_cont.offset == 8      # i32, pad, 3 x f64
+    assert ctypes.sizeof(m._CBkgXParams) == 24 and ctypes.sizeof(m._CConvParams) == 64            # bd_bkgx_params, bd_conv_params
 
 
 def test_no_gpu_no_fallback():
