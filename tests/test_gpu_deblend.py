@@ -372,3 +372,29 @@ def test_k9_workspace_tier_in_a_batch_and_reproducibility(bd, ctx):
     assert np.array_equal(lab_a, lab_b) and np.array_equal(n_a, n_b)
     for k in ("frame", "label", "npix", "xmin", "xmax", "ymin", "ymax", "xpeak", "ypeak", "peak"):
         assert np.array_equal(cat_a[k], cat_b[k]), k
+
+
+def test_k9_k10_empty_and_tiny_inputs(bd, ctx):
+    """Degenerate inputs: an empty catalogue (nothing detected), a zero capacity, a frame of one tile row; labels untouched,
+    zero counts, no fault."""
+    H, W = 32, 64
+    sub = np.zeros((2, H, W), np.float32)
+    rms = np.ones_like(sub)
+    labels = np.zeros((2, H, W), np.int32)
+    cat = np.zeros(0, dtype=bd.SOURCE_DTYPE)
+    n0 = dev(np.zeros(2, np.int64))
+    for cap in (0, 16):
+        d_lab = dev(labels.copy())
+        out = bd.deblend_sources(ctx, dev(sub), dev(rms), d_lab, cat_to_dev(bd, cat, cap), n0, cap, 1.5, 5, out_capacity=cap)
+        cl = bd.clean_sources(ctx, dev(rms), d_lab, out["cat"], out["n_sources"], cap, 1.5)
+        ph = bd.photometry(ctx, dev(sub), dev(rms), cl["cat"], cl["n_sources"], cap)
+        torch.cuda.synchronize()
+        assert out["n_sources"].sum().item() == 0 and cl["n_sources"].sum().item() == 0
+        assert not d_lab.any().item() and ph is not None
+    # one small candidate that cannot split (fewer than 2 * min_area pixels) next to one that can
+    sub[1, 10:12, 10:13] = 9.0
+    sub[1, 20:23, 30:40] = 9.0
+    sub[1, 20:23, 34:36] = 2.0
+    labels2, cat2 = labelled(sub, rms, 1.5, 5)
+    stats, lab_g, cat_g, n_out = check_deblend(bd, ctx, sub, rms, labels2, cat2, 1.5, 5)
+    assert n_out[0] == 0 and n_out[1] == 3 and stats["n_split"] == 1
