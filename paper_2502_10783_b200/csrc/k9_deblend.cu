@@ -133,7 +133,9 @@ __global__ void __launch_bounds__(256) k9_classify(DbArgs a) {
         const bd_source s = a.cat[i];
         const double t0 = cand_t0(a, s);
         a.w.state[i] = 0;
-        if (!((double)s.peak > t0) || s.npix < 2 * max(a.min_area, 1)) {   // D2: not deblended (or too small to hold two nodes)
+        // D2: not deblended (or too small to hold two nodes; or a box beyond the 15 + 16 bits of a packed (row, column) entry,
+        // which no frame with H * W < 2^31 and a sane aspect ratio produces)
+        if (!((double)s.peak > t0) || s.npix < 2 * max(a.min_area, 1) || s.xmax - s.xmin >= 65535 || s.ymax - s.ymin >= 32767) {
             mark_kept(a.w, (size_t)s.frame * HW + (size_t)(s.label - 1));
             continue;
         }
