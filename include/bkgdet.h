@@ -214,7 +214,8 @@ int photometry(bd_ctx *ctx, const float *d_sub, const float *d_rms, int B, int H
  * (frame, label), the first min(n, cap_out) records; d_n_out int64 [B] true counts.  cap_out also bounds the number of NEW
  * objects whose records can be formed: a candidate that cannot reserve its records still gets its new labels and is counted
  * in d_n_out, so sum(d_n_out) > cap_out or missing records tell the caller to retry with more room.  d_cat_out must not
- * alias d_cat_in.  Label maps are bit-reproducible; flux sums are float64 atomics (tree decisions within 1e-9 relative of
+ * alias d_cat_in.  A candidate whose bounding box is 65 535 or more pixels wide or 32 767 or more tall is left whole.
+ * Label maps are bit-reproducible; flux sums are float64 atomics (tree decisions within 1e-9 relative of
  * the contrast limit may differ from the float64 definition).
  * clean_sources: d_cat_in / d_n_in are a catalogue of d_labels (normally deblend_sources' output); d_flags (uint8
  * [cap_in], may be NULL) receives 1 for every false detection.  Decisions use float64 pow(): pairs within 1e-9 relative of
