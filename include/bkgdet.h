@@ -123,6 +123,31 @@ int bd_grid_filter_spline(bd_ctx *ctx, const double *d_bkg_raw, const double *d_
                           double *d_bkg_coef, double *d_rms_coef, void *d_ws, size_t ws_bytes,
                           void *cuda_stream);
 
+/* ---- a2 for callers that cannot allocate device memory.  PAPER.md:80, same operation and same kernels as
+ * bd_grid_filter_spline, but without the d_ws / ws_bytes pair.
+ * Who needs it: code that gets its device buffers handed to it and has no allocator of its own -- a plug-in inside
+ * an application that owns all of the GPU's memory, a real-time loop that may not enter cudaMalloc (it can block and
+ * synchronises the device), a process whose memory is fully committed by the time this step runs.  Such a caller can
+ * still pass the inputs and outputs it was given, but has nowhere to get the scratch from.
+ * Here the scratch (the Thomas factors of the spline prefilter, 4*B*(ny+nx) doubles) is an array compiled into the
+ * library: BD_GRID_STATIC_MAX_DOUBLES doubles (256 KiB) of device memory that every GPU which loads libbkgdet holds
+ * from module load until the process exits, whether or not this call is ever made.  The call makes no cudaMalloc,
+ * cudaFree or other allocating call.
+ * Limit: 4*B*(ny+nx) <= BD_GRID_STATIC_MAX_DOUBLES, else BD_EWORKSPACE with the numbers in bd_last_error() and
+ * nothing is launched (e.g. B = 64 frames of 32 x 32 meshes, or one frame with ny + nx <= 8192).
+ * First call on a device: looks up the array's device address (cudaGetSymbolAddress with ctx's device current) and
+ * keeps it for later calls; make that first call outside any stream capture.
+ * Sharing: there is ONE array per GPU, used by every call, context and stream.  Nothing in it has to be zero at
+ * entry (the kernel writes each factor before reading it) and the last call's contents stay behind.  Two calls
+ * whose kernels overlap on the same GPU (different streams, or different host threads) race on the array and
+ * produce garbage: keep calls on one stream, or order them with events.  Grids that fit the kernel's shared memory
+ * (ny, nx <= 160 and ny*(nx|1) <= 20880) do not touch the array at all.
+ * Outputs are bit-identical to bd_grid_filter_spline's. */
+#define BD_GRID_STATIC_MAX_DOUBLES 32768
+int bd_grid_filter_spline_static(bd_ctx *ctx, const double *d_bkg_raw, const double *d_rms_raw, int B, int ny, int nx,
+                                 int filt_h, int filt_w, float *d_bkg_mesh, float *d_rms_mesh,
+                                 double *d_bkg_coef, double *d_rms_coef, void *cuda_stream);
+
 /* ---- bkg_estimate = a1 + a2.  PAPER.md:67-80. -------------------------------------------------------
  * d_bkg_mesh, d_rms_mesh: filtered mesh grids, float32 [B, ny, nx] (may be NULL).
  * d_bkg_coef, d_rms_coef: spline coefficients, float64 [B, ny, nx] (required).

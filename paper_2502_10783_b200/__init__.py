@@ -16,10 +16,11 @@ import torch
 from . import _build
 
 __all__ = ["BkgParams", "Context", "SOURCE_DTYPE", "bkg_estimate", "bkg_subtract", "detect_sources", "mesh_stats",
-           "grid_filter_spline", "bkg_subtract_detect", "photometry", "PhotParams", "PHOT_DTYPE", "deblend_sources", "clean_sources", "DeblendParams", "run_host", "grid_shape", "load_library", "EXPORTS"]
+           "grid_filter_spline", "grid_filter_spline_static", "GRID_STATIC_MAX_DOUBLES", "bkg_subtract_detect", "photometry", "PhotParams", "PHOT_DTYPE", "deblend_sources", "clean_sources", "DeblendParams", "run_host", "grid_shape", "load_library", "EXPORTS"]
 
 EXPORTS = ["bd_create", "bd_destroy", "bd_last_error", "bd_default_bkg_params", "bd_grid_shape",
            "bd_bkg_workspace_bytes", "bd_detect_workspace_bytes", "bd_mesh_stats", "bd_grid_filter_spline",
+           "bd_grid_filter_spline_static",
            "bkg_estimate", "bkg_subtract", "detect_sources", "bkg_subtract_detect", "bd_default_phot_params", "bd_phot_workspace_bytes", "photometry",
            "bd_run_host", "bd_default_bkgx_params", "bd_mesh_stats_masked", "bkg_estimate_masked",
            "bd_bkg_iterate_workspace_bytes", "bkg_iterate", "bd_default_conv_params", "bd_conv_num_basis",
@@ -292,6 +293,34 @@ def grid_filter_spline(ctx: Context, bkg_raw: torch.Tensor, rms_raw: torch.Tenso
     ws = torch.empty(4 * B * (ny + nx) + 32, dtype=torch.float64, device=dev)
     ctx.check(ctx.lib.bd_grid_filter_spline(ctx.h, _ptr(bkg_raw), _ptr(rms_raw), B, ny, nx, filt_h, filt_w, _ptr(bm),
                                             _ptr(rm), _ptr(cb), _ptr(cr), _ptr(ws), C.c_size_t(ws.numel() * 8), _stream(ctx)))
+    return bm, rm, cb, cr
+
+
+GRID_STATIC_MAX_DOUBLES = 32768   # BD_GRID_STATIC_MAX_DOUBLES of bkgdet.h
+
+
+def grid_filter_spline_static(ctx: Context, bkg_raw: torch.Tensor, rms_raw: torch.Tensor, filt_h: int, filt_w: int, out=None):
+    """a2 (K2) through bd_grid_filter_spline_static: the call for code that cannot allocate device memory.
+
+    Same inputs and results as grid_filter_spline, but no workspace is allocated or passed: the kernel's scratch is a
+    256 KiB array built into libbkgdet (one per GPU, shared by every call, so calls must not overlap on the GPU).
+    Meant for callers that work inside someone else's memory budget -- a plug-in given a fixed set of buffers, a
+    real-time loop that must stay out of the CUDA allocator -- who pass their own output tensors as
+    out = (bkg_mesh f32, rms_mesh f32, bkg_coef f64, rms_coef f64), each [B,ny,nx]; with out=None the four outputs are
+    made with torch.empty here (which does allocate: convenience for tests).  Raises BkgdetError when
+    4*B*(ny+nx) > GRID_STATIC_MAX_DOUBLES."""
+    _chk(ctx, bkg_raw, torch.float64, "bkg_raw"); _chk(ctx, rms_raw, torch.float64, "rms_raw", bkg_raw.shape)
+    B, ny, nx = bkg_raw.shape
+    if out is None:
+        dev = _dev(ctx)
+        bm = torch.empty((B, ny, nx), dtype=torch.float32, device=dev); rm = torch.empty_like(bm)
+        cb = torch.empty((B, ny, nx), dtype=torch.float64, device=dev); cr = torch.empty_like(cb)
+    else:
+        bm, rm, cb, cr = out
+        _chk(ctx, bm, torch.float32, "bkg_mesh", bkg_raw.shape); _chk(ctx, rm, torch.float32, "rms_mesh", bkg_raw.shape)
+        _chk(ctx, cb, torch.float64, "bkg_coef", bkg_raw.shape); _chk(ctx, cr, torch.float64, "rms_coef", bkg_raw.shape)
+    ctx.check(ctx.lib.bd_grid_filter_spline_static(ctx.h, _ptr(bkg_raw), _ptr(rms_raw), B, ny, nx, filt_h, filt_w, _ptr(bm),
+                                                   _ptr(rm), _ptr(cb), _ptr(cr), _stream(ctx)))
     return bm, rm, cb, cr
 
 

@@ -259,3 +259,61 @@ int k2_launch(bd_ctx *ctx, const double *d_bkg_raw, const double *d_rms_raw, int
     BD_CUDA_CHECK(ctx, cudaGetLastError());
     return BD_OK;
 }
+
+// ---- bd_grid_filter_spline_static: step a2 for callers that may not allocate device memory --------------------------
+// bd_grid_filter_spline takes its Thomas-factor scratch from a workspace the caller cudaMalloc'ed.  Some callers have no
+// allocator to ask: a plug-in running inside a host application that handed it a fixed set of device buffers and forbids
+// further allocation, a real-time acquisition loop that must not enter the driver's allocator (it can block for
+// milliseconds and synchronise the device), or code running after the application has committed all of its memory.  For
+// them the same two kernels run with the scratch in the array below, which is part of the library's image: the driver
+// reserves it on every GPU that loads libbkgdet, when the module is loaded, and releases it at process exit.
+//
+// The array name is only a handle on the host; the device address comes from cudaGetSymbolAddress, asked once per device
+// with that device current (the entry point binds ctx's device first) and kept in k2_static_addr[].
+constexpr size_t K2_STATIC_DOUBLES = BD_GRID_STATIC_MAX_DOUBLES;   // bkgdet.h: 32768 doubles = 256 KiB
+constexpr int K2_STATIC_MAX_DEVICES = 64;
+static __device__ __align__(256) double k2_static_scratch[K2_STATIC_DOUBLES];
+
+#include <mutex>
+static std::mutex k2_static_mutex;
+static double *k2_static_addr[K2_STATIC_MAX_DEVICES];   // device address of k2_static_scratch on device i, or null: not asked yet
+
+// Device address of the array on ctx's device (which must be current).  The first call per device asks the runtime.
+static int k2_static_scratch_ptr(bd_ctx *ctx, double **out) {
+    if (ctx->device < 0 || ctx->device >= K2_STATIC_MAX_DEVICES)
+        return bd_set_error(ctx, BD_EUNSUPPORTED, "bd_grid_filter_spline_static: device ordinal %d is beyond the %d the table holds",
+                            ctx->device, K2_STATIC_MAX_DEVICES);
+    std::lock_guard<std::mutex> lock(k2_static_mutex);
+    if (!k2_static_addr[ctx->device]) {
+        double *p = nullptr;
+        BD_CUDA_CHECK(ctx, cudaGetSymbolAddress((void **)&p, k2_static_scratch));
+        if (!p) return bd_set_error(ctx, BD_ECUDA, "cudaGetSymbolAddress returned a null address for the static scratch array");
+        k2_static_addr[ctx->device] = p;
+    }
+    *out = k2_static_addr[ctx->device];
+    return BD_OK;
+}
+
+extern "C" int bd_grid_filter_spline_static(bd_ctx *ctx, const double *d_bkg_raw, const double *d_rms_raw, int B, int ny, int nx,
+                                            int filt_h, int filt_w, float *d_bkg_mesh, float *d_rms_mesh, double *d_bkg_coef,
+                                            double *d_rms_coef, void *cuda_stream) {
+    if (!ctx) return BD_EINVAL;
+    if (!d_bkg_raw || !d_rms_raw || !d_bkg_coef || !d_rms_coef) return bd_set_error(ctx, BD_EINVAL, "null pointer");
+    if (B <= 0 || ny <= 0 || nx <= 0 || B > 65535) return bd_set_error(ctx, BD_EINVAL, "bad grid shape");
+    if (filt_h < 1 || filt_w < 1 || !(filt_h & 1) || !(filt_w & 1) || filt_h > 11 || filt_w > 11)
+        return bd_set_error(ctx, BD_EINVAL, "filter size must be odd and in 1..11");
+    const size_t need = 2 * (size_t)B * k2_scratch_per_grid(ny, nx);   // doubles; the same count bd_grid_filter_spline asks for
+    if (need > K2_STATIC_DOUBLES)
+        return bd_set_error(ctx, BD_EWORKSPACE,
+                            "bd_grid_filter_spline_static: B=%d grids of %d x %d cells need 4*B*(ny+nx) = %zu doubles of scratch, the "
+                            "built-in array holds %zu (%zu bytes); split the batch or use bd_grid_filter_spline with a workspace",
+                            B, ny, nx, need, K2_STATIC_DOUBLES, K2_STATIC_DOUBLES * sizeof(double));
+    BD_BIND_DEVICE(ctx);
+    double *scratch = nullptr;
+    const int rc = k2_static_scratch_ptr(ctx, &scratch);
+    if (rc) return rc;
+    // Nothing in the array has to start at zero: every (frame, grid) block of the prefilter writes its own factors
+    // before it reads them, so whatever the previous call left behind is simply overwritten.
+    return k2_launch(ctx, d_bkg_raw, d_rms_raw, B, ny, nx, filt_h, filt_w, d_bkg_mesh, d_rms_mesh, d_bkg_coef, d_rms_coef, scratch,
+                     (cudaStream_t)cuda_stream);
+}
