@@ -136,6 +136,9 @@ __global__ void __launch_bounds__(32) k1w_warp_mesh(const __grid_constant__ CUte
                 const bool ok = i0 + lane < n4;
                 uint4 v = make_uint4(0, 0, 0, 0);
                 if (ok) v = kw_lds128(slab_s + 16u * (uint32_t)(i0 + lane));
+                // L grows over slab words that OTHER lanes load in this same iteration (m <= 4 i0): every lane's load must
+                // have completed before the first store below.  The vote intrinsics order nothing in memory; this does.
+                __syncwarp();
                 const uint32_t raw[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
