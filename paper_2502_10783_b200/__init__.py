@@ -76,6 +76,12 @@ class BkgXParams:
         return _CBkgXParams(self.min_valid_px, self.grow, self.max_masked_frac, self.max_reject_frac)
 
 
+def _chk_cat(cat, cat_capacity):
+    """The kernels read up to cat_capacity records of 88 bytes from `cat`: the tensor must hold them."""
+    if cat_capacity < 0 or cat.numel() < cat_capacity * SOURCE_DTYPE.itemsize:
+        raise BkgdetError(f"cat: {cat.numel()} bytes cannot hold cat_capacity = {cat_capacity} records of {SOURCE_DTYPE.itemsize} bytes")
+
+
 _lib = None
 
 
@@ -532,6 +538,7 @@ def deblend_sources(ctx: Context, sub: torch.Tensor, rms: torch.Tensor, labels: 
     B, H, W = sub.shape
     _chk(ctx, rms, torch.float32, "rms", (B, H, W)); _chk(ctx, labels, torch.int32, "labels", (B, H, W))
     _chk(ctx, cat, torch.uint8, "cat"); _chk(ctx, n_sources, torch.int64, "n_sources", (B,)); _chk(ctx, ws, torch.uint8, "ws", optional=True)
+    _chk_cat(cat, cat_capacity)
     p = p or DeblendParams()
     cap_out = cat_capacity if out_capacity is None else out_capacity
     dev = _dev(ctx)
@@ -556,6 +563,7 @@ def clean_sources(ctx: Context, rms: torch.Tensor, labels: torch.Tensor, cat: to
     B, H, W = rms.shape
     _chk(ctx, labels, torch.int32, "labels", (B, H, W)); _chk(ctx, cat, torch.uint8, "cat")
     _chk(ctx, n_sources, torch.int64, "n_sources", (B,)); _chk(ctx, ws, torch.uint8, "ws", optional=True)
+    _chk_cat(cat, cat_capacity)
     p = p or DeblendParams()
     dev = _dev(ctx)
     cat_out = torch.empty(max(cat_capacity, 1) * SOURCE_DTYPE.itemsize, dtype=torch.uint8, device=dev)
@@ -596,3 +604,4 @@ def run_host(ctx: Context, img: np.ndarray, p: BkgParams, detect_k: float, min_a
                                   C.c_int32(min_area), C.c_void_p(cat.ctypes.data), C.c_int64(cat_capacity),
                                   C.c_void_p(n.ctypes.data)))
     return cat[: min(int(n.sum()), cat_capacity)], n
+

@@ -220,6 +220,7 @@ int bkg_estimate_masked(bd_ctx *ctx, const float *d_img, const uint8_t *d_bad, i
 }
 
 int bd_bkg_iterate_workspace_bytes(const bd_ctx *ctx, int B, int H, int W, const bd_bkg_params *p, size_t *bytes) {
+    if (!bytes) return BD_EINVAL;
     size_t b = 0;
     int rc = bd_bkg_workspace_bytes(ctx, B, H, W, p, &b);
     if (rc) return rc;
@@ -442,6 +443,21 @@ int image_subtract(bd_ctx *ctx, const float *d_ref, const float *d_img, int B, i
     return k8_launch(ctx, d_ref, d_img, B, H, W, p, d_kcoef, d_bgcoef, d_diff, d_conv, d_ws, (cudaStream_t)cuda_stream);
 }
 
+// bd_run_host returns early on any error; by then copies on the copy stream may still be reading the caller's h_img and
+// writing h_n_sources / h_cat.  The guard waits for both streams on every such path (the caller may free its buffers as
+// soon as the call returns); the successful path has already synchronised and disarms it.
+struct BdHostDrain {
+    bd_ctx *ctx;
+    bool armed = true;
+    explicit BdHostDrain(bd_ctx *c) : ctx(c) {}
+    ~BdHostDrain() {
+        if (!armed) return;
+        if (ctx->copy_stream) cudaStreamSynchronize(ctx->copy_stream);
+        if (ctx->host_stream) cudaStreamSynchronize(ctx->host_stream);
+        cudaGetLastError();   // the error that brought us here is already recorded in ctx->err
+    }
+};
+
 int bd_run_host(bd_ctx *ctx, const float *h_img, int B, int H, int W, const bd_bkg_params *p, double detect_k,
                 int32_t min_area, bd_source *h_cat, int64_t cat_capacity, int64_t *h_n_sources) {
     int rc = check_frame(ctx, B, H, W);
@@ -476,6 +492,8 @@ int bd_run_host(bd_ctx *ctx, const float *h_img, int B, int H, int W, const bd_b
     if (!ctx->copy_stream) BD_CUDA_CHECK(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
     for (int c = 0; c < BD_HOST_CHUNKS; ++c)
         if (!ctx->host_ev[c]) BD_CUDA_CHECK(ctx, cudaEventCreateWithFlags(&ctx->host_ev[c], cudaEventDisableTiming));
+    BdHostDrain drain(ctx);
+    drain.armed = false;
     {
         const size_t stride = bd_align_up(cells * sizeof(double), 256);
         char *base = (char *)bd_align_up((size_t)(d + o_wsb), 256);
@@ -485,6 +503,7 @@ int bd_run_host(bd_ctx *ctx, const float *h_img, int B, int H, int W, const bd_b
         const int units = B > 1 ? B : ny;
         const int nch = units < BD_HOST_CHUNKS ? units : BD_HOST_CHUNKS;
         // (the copy stream must not overwrite the frame while work of the previous call still reads it)
+        drain.armed = true;   // from the first enqueue on, an early return waits for the streams
         BD_CUDA_CHECK(ctx, cudaEventRecord(ctx->host_ev[BD_HOST_CHUNKS - 1], st));
         BD_CUDA_CHECK(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->host_ev[BD_HOST_CHUNKS - 1], 0));
         for (int c = 0; c < nch; ++c) {
@@ -519,6 +538,7 @@ int bd_run_host(bd_ctx *ctx, const float *h_img, int B, int H, int W, const bd_b
         BD_CUDA_CHECK(ctx, cudaMemcpyAsync(h_cat, d + o_cat, (size_t)total * sizeof(bd_source), cudaMemcpyDeviceToHost, st));
         BD_CUDA_CHECK(ctx, cudaStreamSynchronize(st));
     }
+    drain.armed = false;   // both streams are idle here: st was synchronised after the last copy it waited for
     return BD_OK;
 }
 

@@ -104,20 +104,32 @@ __global__ void __launch_bounds__(K2_NT) k2a_window_median_small(const double *b
 
 // ---- K2f: invalid cells (NaN: background variants, reading B3) take the median of the VALID cells of the smallest square
 // window (2r+1)^2, r = 1, 2, ..., truncated at the grid border, that holds one; both grids, read from the unfilled grids.
-// One thread per cell: an invalid cell is rare and its window is a handful of cells (rank counting, as in K2a).
-__device__ double k2f_window_median(const double *g, const double *gv, int nx, int j0, int j1, int i0, int i1, int n) {
-    const int ww = i1 - i0 + 1, tot = (j1 - j0 + 1) * ww;
+// One thread per cell.  The window of radius r - 1 held no valid cell, so the valid cells of the window of radius r all lie
+// on its outer RING (Chebyshev distance exactly r, 8r cells before truncation): only the ring is scanned, and the rank
+// counting (as in K2a) runs over the ring's valid cells.  A grid that is mostly or wholly invalid therefore costs
+// O(max(ny, nx)^2) loads per cell, not the O(max(ny, nx)^3) + O(window^2) of rescanning whole windows.
+// Ring cell t in [0, 8r): top row, bottom row (2r + 1 cells each), then the left and right columns without their corners.
+__device__ __forceinline__ bool k2f_ring_cell(int t, int r, int j, int i, int ny, int nx, int *jj, int *ii) {
+    const int w = 2 * r + 1;
+    int dj, di;
+    if (t < 2 * w) { dj = t < w ? -r : r; di = (t < w ? t : t - w) - r; }
+    else { const int u = t - 2 * w, h = w - 2; di = u < h ? -r : r; dj = (u < h ? u : u - h) - r + 1; }
+    *jj = j + dj; *ii = i + di;
+    return *jj >= 0 && *jj < ny && *ii >= 0 && *ii < nx;
+}
+// median of g over the valid (gv not NaN) cells of the ring, n > 0 of them; ties: any order gives the same value
+__device__ double k2f_ring_median(const double *g, const double *gv, int ny, int nx, int j, int i, int r, int n) {
     const int k_lo = (n - 1) / 2, k_hi = n / 2;
     double lo = 0.0, hi = 0.0;
-    for (int a = 0; a < tot; ++a) {
-        const size_t ia = (size_t)(j0 + a / ww) * nx + i0 + a % ww;
-        if (isnan(gv[ia])) continue;
-        const double va = g[ia];
+    for (int a = 0; a < 8 * r; ++a) {
+        int ja, ia;
+        if (!k2f_ring_cell(a, r, j, i, ny, nx, &ja, &ia) || isnan(gv[(size_t)ja * nx + ia])) continue;
+        const double va = g[(size_t)ja * nx + ia];
         int rank = 0;
-        for (int b = 0; b < tot; ++b) {
-            const size_t ib = (size_t)(j0 + b / ww) * nx + i0 + b % ww;
-            if (isnan(gv[ib])) continue;
-            const double vb = g[ib];
+        for (int b = 0; b < 8 * r; ++b) {
+            int jb, ib;
+            if (!k2f_ring_cell(b, r, j, i, ny, nx, &jb, &ib) || isnan(gv[(size_t)jb * nx + ib])) continue;
+            const double vb = g[(size_t)jb * nx + ib];
             rank += (vb < va || (vb == va && b < a)) ? 1 : 0;
         }
         if (rank == k_lo) lo = va;
@@ -125,36 +137,44 @@ __device__ double k2f_window_median(const double *g, const double *gv, int nx, i
     }
     return (n & 1) ? lo : 0.5 * (lo + hi);
 }
+// grid = (ceil(cells / K2_NT), B): a block's cells belong to one frame.  A block that holds an invalid cell first scans its
+// frame's grid for ANY valid cell (cells / K2_NT loads per thread, from L2): a frame without one is written as 0 straight
+// away instead of every cell walking all its rings to the far corner.
 __global__ void __launch_bounds__(K2_NT) k2f_fill_invalid(const double *bkg_raw, const double *rms_raw, int B, int ny, int nx,
                                                           double *bkg_out, double *rms_out, uint8_t *valid) {
-    const long long idx = (long long)blockIdx.x * K2_NT + threadIdx.x;
     const int cells = ny * nx;
-    if (idx >= (long long)B * cells) return;
-    const int c = (int)(idx % cells);
-    const size_t goff = (size_t)(idx / cells) * cells;
+    const int c = blockIdx.x * K2_NT + threadIdx.x;
+    const size_t goff = (size_t)blockIdx.y * cells;
     const double *gb = bkg_raw + goff, *gr = rms_raw + goff;
-    const double vb = gb[c];
-    if (!isnan(vb)) {
-        bkg_out[idx] = vb; rms_out[idx] = gr[c];
-        if (valid) valid[idx] = 1;
-        return;
+    const bool mine = c < cells;
+    const double vb = mine ? gb[c] : 0.0;
+    const bool inv = mine && isnan(vb);
+    if (mine && !inv) {
+        bkg_out[goff + c] = vb; rms_out[goff + c] = gr[c];
+        if (valid) valid[goff + c] = 1;
     }
-    if (valid) valid[idx] = 0;
+    if (!__syncthreads_or(inv ? 1 : 0)) return;
+    int any = 0;
+    for (int k = threadIdx.x; k < cells; k += K2_NT) any |= isnan(gb[k]) ? 0 : 1;
+    any = __syncthreads_or(any);
+    if (!inv) return;
+    if (valid) valid[goff + c] = 0;
     const int j = c / nx, i = c - j * nx;
     double fb = 0.0, fr = 0.0;
-    const int rmax = max(ny, nx);
+    const int rmax = any ? max(max(j, ny - 1 - j), max(i, nx - 1 - i)) : 0;   // the ring of this radius reaches the farthest corner
     for (int r = 1; r <= rmax; ++r) {
-        const int j0 = max(j - r, 0), j1 = min(j + r, ny - 1), i0 = max(i - r, 0), i1 = min(i + r, nx - 1);
         int n = 0;
-        for (int jj = j0; jj <= j1; ++jj)
-            for (int ii = i0; ii <= i1; ++ii) n += isnan(gb[(size_t)jj * nx + ii]) ? 0 : 1;
+        for (int t = 0; t < 8 * r; ++t) {
+            int jj, ii;
+            if (k2f_ring_cell(t, r, j, i, ny, nx, &jj, &ii)) n += isnan(gb[(size_t)jj * nx + ii]) ? 0 : 1;
+        }
         if (n > 0) {
-            fb = k2f_window_median(gb, gb, nx, j0, j1, i0, i1, n);
-            fr = k2f_window_median(gr, gb, nx, j0, j1, i0, i1, n);
+            fb = k2f_ring_median(gb, gb, ny, nx, j, i, r, n);
+            fr = k2f_ring_median(gr, gb, ny, nx, j, i, r, n);
             break;
         }
     }
-    bkg_out[idx] = fb; rms_out[idx] = fr;
+    bkg_out[goff + c] = fb; rms_out[goff + c] = fr;
 }
 
 // ---- K2b: cubic-B-spline prefilter ------------------------------------------------------------------------
@@ -234,9 +254,8 @@ __global__ void __launch_bounds__(K2_NT) k2b_spline_prefilter(int ny, int nx, do
 
 int k2f_launch(bd_ctx *ctx, const double *d_bkg_raw, const double *d_rms_raw, int B, int ny, int nx, double *d_bkg_filled,
                double *d_rms_filled, uint8_t *d_valid, cudaStream_t st) {
-    const long long n = (long long)B * ny * nx;
-    k2f_fill_invalid<<<(unsigned)((n + K2_NT - 1) / K2_NT), K2_NT, 0, st>>>(d_bkg_raw, d_rms_raw, B, ny, nx, d_bkg_filled,
-                                                                          d_rms_filled, d_valid);
+    const dim3 grid((unsigned)((ny * nx + K2_NT - 1) / K2_NT), (unsigned)B);   // B <= 65535 (check_frame)
+    k2f_fill_invalid<<<grid, K2_NT, 0, st>>>(d_bkg_raw, d_rms_raw, B, ny, nx, d_bkg_filled, d_rms_filled, d_valid);
     BD_CUDA_CHECK(ctx, cudaGetLastError());
     return BD_OK;
 }

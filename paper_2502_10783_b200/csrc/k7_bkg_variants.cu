@@ -16,9 +16,10 @@ __global__ void __launch_bounds__(256) k7_dilate_or_kernel(const uint8_t *det, c
                                                            uint8_t *out) {
     const int w4 = W >> 2;
     const int x4 = blockIdx.x * blockDim.x + threadIdx.x;
-    const int y = blockIdx.y, frame = blockIdx.z;
+    const int frame = blockIdx.z;
     if (x4 >= w4) return;
     const size_t fbase = (size_t)frame * H * W;
+  for (int y = blockIdx.y; y < H; y += gridDim.y) {   // gridDim.y = min(H, 65535): one row per block unless the frame is taller
     uint32_t any = 0;   // bit q: pixel 4 x4 + q has a detection in its window
     if (det) {
         const int y0 = max(y - grow, 0), y1 = min(y + grow, H - 1);
@@ -38,13 +39,14 @@ __global__ void __launch_bounds__(256) k7_dilate_or_kernel(const uint8_t *det, c
         o |= (nb & 1u) | (nb & 2u) << 7 | (nb & 4u) << 14 | (nb & 8u) << 21;
     }
     reinterpret_cast<uint32_t *>(out + fbase + (size_t)y * W)[x4] = o;
+  }
 }
 
 }  // namespace
 
 int k7_dilate_or(bd_ctx *ctx, const uint8_t *d_det, const uint8_t *d_bad0, int B, int H, int W, int grow, uint8_t *d_out,
                  cudaStream_t st) {
-    dim3 grid((W / 4 + 255) / 256, H, B);
+    dim3 grid((W / 4 + 255) / 256, H < 65535 ? H : 65535, B);
     k7_dilate_or_kernel<<<grid, 256, 0, st>>>(d_det, d_bad0, H, W, grow, d_out);
     BD_CUDA_CHECK(ctx, cudaGetLastError());
     return BD_OK;

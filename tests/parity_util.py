@@ -85,7 +85,11 @@ def assert_catalogue_equal(got, want, frame=None, exempt_labels=(), peak_pos_exa
     for k in ("x2", "y2", "xy"):
         # a moment can be ~0 by symmetry (xy, or x2 of a one-column component): the error it inherits from a
         # relative perturbation eps of the pixel values is <= eps * (x2 + y2), so the scale has that floor
-        scale = np.maximum(np.abs(want[k]), 1e-3 * (want["x2"] + want["y2"]) + 1e-9)
+        # -- CHAIN comparison (each side reduces its own sub map, ~1e-6 ADU apart): floor 1e-3 (x2 + y2), DESIGN.md section 8.
+        # -- STAGE comparison (peak_pos_exact: both sides read the SAME float32 sub; only the summation order differs):
+        #    the tight floor 1e-6 (1 + x2 + y2), i.e. 1e-9 (1 + x2 + y2) absolute.
+        floor = 1e-6 * (1.0 + want["x2"] + want["y2"]) if peak_pos_exact else 1e-3 * (want["x2"] + want["y2"]) + 1e-9
+        scale = np.maximum(np.abs(want[k]), floor)
         err = np.abs(got[k] - want[k]) / scale
         assert np.all(err <= REL_MOM), f"{k}: worst rel {err.max():.3e}"
         worst[k] = float(err.max())

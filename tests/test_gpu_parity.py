@@ -748,6 +748,80 @@ def test_bkg_estimate_masked_and_fill(bd, ctx, cid, H, W, mesh):
     assert int(valid.sum()) == 0 and float(bm.abs().max()) == 0.0 and float(cb.abs().max()) == 0.0
 
 
+def _time_ms(fn, reps=3):
+    fn(); torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record(); torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+@pytest.mark.parametrize("keep", ["5%", "one corner cell", "all but a right strip", "none"])
+def test_k2f_mostly_invalid_grid_of_config3_size(bd, ctx, keep):
+    """B3 on a 144 x 145 mesh grid (the grid of config 3; 8 x 8 meshes keep the frame small) of which almost every cell is
+    invalid: the fill scans rings, not whole windows, and a frame without a valid cell is written as 0 at once, so the
+    stage stays in milliseconds where rescanning windows took seconds (about cells x grid loads).  Parity with O8's
+    fill on every cell, plus a time bound for the whole masked estimate."""
+    mesh, ny, nx = 8, 144, 145
+    H, W = ny * mesh, nx * mesh
+    rng = np.random.default_rng(31)
+    img = rng.normal(500, 10, size=(1, H, W)).astype(np.float32)
+    img[0] += np.linspace(0, 80, W, dtype=np.float32)[None, :]
+    good = np.zeros((ny, nx), bool)
+    if keep == "5%":
+        good = rng.uniform(size=(ny, nx)) < 0.05
+    elif keep == "one corner cell":
+        good[ny - 1, 0] = True
+    elif keep == "all but a right strip":      # rings that hold many valid cells
+        good[:, : nx - 12] = True
+    bad = np.repeat(np.repeat((~good).astype(np.uint8), mesh, axis=0), mesh, axis=1)[None]
+    p = bd.BkgParams(mesh_h=mesh, mesh_w=mesh)
+    px = bd.BkgXParams(min_valid_px=32)
+    d_img, d_bad = dev(img), dev(bad)
+    bm, rm, cb, cr, valid = bd.bkg_estimate_masked(ctx, d_img, d_bad, p, px)
+    torch.cuda.synchronize()
+    assert np.array_equal(valid[0].cpu().numpy() != 0, good)
+    if keep == "none":
+        assert float(bm.abs().max()) == 0.0 and float(rm.abs().max()) == 0.0 and float(cb.abs().max()) == 0.0
+    else:
+        st = oracle.mesh_stats_masked(img[0], bad[0], to_oracle_params(p), oracle.BkgXParams(min_valid_px=32))
+        assert np.array_equal(~np.isnan(st["bkg"]), good)
+        for raw, got in ((st["bkg"], bm), (st["rms"], rm)):
+            if keep == "one corner cell":   # every window that holds a valid cell holds exactly this one: B3 gives its value
+                filled = np.full((ny, nx), raw[ny - 1, 0])   # (O8's loop would sort ~2e6 windows here)
+            else:
+                filled = obv.fill_invalid(raw)
+            want = oracle.grid_median(filled, p.filt_h, p.filt_w)
+            assert np.max(np.abs(got[0].cpu().numpy() - want) / np.abs(want)) < 1e-6
+    ms = _time_ms(lambda: bd.bkg_estimate_masked(ctx, d_img, d_bad, p, px))
+    assert ms < 50.0, f"masked estimate with a {keep} valid grid took {ms:.1f} ms"
+
+
+def test_k7_frame_taller_than_the_grid_limit(bd, ctx):
+    """bkg_iterate on a frame of more than 65 535 rows: the dilation kernel folds the rows into its y blocks."""
+    H, W = 65600, 8
+    rng = np.random.default_rng(9)
+    img = rng.normal(100, 1, size=(1, H, W)).astype(np.float32)
+    img[0, 65590:65593, 2:5] += 50.0                       # a detection in the rows beyond the limit
+    bad0 = (rng.uniform(size=img.shape) < 0.05).astype(np.uint8) * 3
+    p = bd.BkgParams(mesh_h=64, mesh_w=8)
+    px = bd.BkgXParams(min_valid_px=100, grow=1)
+    out = bd.bkg_iterate(ctx, dev(img), dev(bad0), p, px, 1.5, 0)
+    torch.cuda.synchronize()
+    assert np.array_equal(out[5].cpu().numpy(), (bad0 != 0).astype(np.uint8))
+    # one iteration: the exclusion mask is the dilated mask of the first estimate, OR bad0 (stage check, as in
+    # test_bkg_iterate_stage_parity (i))
+    first = bd.bkg_estimate_masked(ctx, dev(img), dev((bad0 != 0).astype(np.uint8)), p, px)
+    m0 = bd.bkg_subtract(ctx, dev(img), p.mesh_h, p.mesh_w, first[2], first[3], 1.5)["mask"][0].cpu().numpy()
+    out = bd.bkg_iterate(ctx, dev(img), dev(bad0), p, px, 1.5, 1)
+    torch.cuda.synchronize()
+    got = out[5][0].cpu().numpy()
+    assert np.array_equal(got, obv.dilate(m0, 1) | (bad0[0] != 0))
+    assert got[65589:65594, 1:6].all()
+
+
 def test_k7_dilate_or_exhaustive_window(bd, ctx):
     """B5 through bkg_iterate's exclusion mask with n_iter = 0 / the dilation kernel against scipy-pinned oracle dilation:
     every grow, frame edges, bad0 with arbitrary non-zero bytes."""
@@ -765,10 +839,14 @@ def test_k7_dilate_or_exhaustive_window(bd, ctx):
 @pytest.mark.parametrize("cid,H,W,mesh,grow,n_iter", [(1, 512, 512, 64, 1, 1), (3, 528, 768, 256, 2, 2), (5, 384, 512, 64, 0, 1), (2, 300, 340, 50, 3, 1)])
 def test_bkg_iterate_stage_parity(bd, ctx, cid, H, W, mesh, grow, n_iter):
     """NEXT-3, B4.  The threshold inside the iteration is the library's float32 rule, the oracle's is float64:
-    masks may differ on fragile pixels, so the comparison is stage-wise and exact: (i) with n_iter = 1 the exclusion mask
-    equals oracle.dilate(bkg_subtract's mask of the first estimate) | bad0; (ii) the final grids equal the oracle's masked
-    estimate under the library's own final exclusion mask; (iii) against the oracle's own iteration the exclusion masks
-    differ on at most a handful of pixels (those grown from fragile detections)."""
+    masks may differ on fragile pixels, so the comparison is stage-wise and exact, EVERY round k = 1..n_iter:
+    (i) the library's detection mask of round k (its estimate under its exclusion mask of round k - 1, thresholded by
+    bkg_subtract) equals the oracle's threshold of the oracle's masked estimate under that SAME exclusion mask, except on
+    the oracle's fragile set of that round; (ii) the exclusion mask of round k is oracle.dilate(that library mask) | bad0, bit
+    for bit, and the last one is what bkg_iterate returns; (iii) the final grids equal the oracle's masked estimate under the
+    library's final exclusion mask.  (iv) Against the oracle's own free-running iteration: with one round every differing
+    pixel lies within `grow` of a fragile pixel; from the second round on a pixel that differed in round 1 moves a mesh's
+    statistics by ~1e-4 sigma, more than the fragile band, so there the difference is bounded by count."""
     cfg = CONFIGS[cid]
     rng = np.random.default_rng(cid + 40)
     img = make_frames(cfg, H=H, W=W, B=1)
@@ -780,17 +858,27 @@ def test_bkg_iterate_stage_parity(bd, ctx, cid, H, W, mesh, grow, n_iter):
     torch.cuda.synchronize()
     bad_g = bad_out[0].cpu().numpy()
     assert set(np.unique(bad_g)) <= {0, 1}
-    if n_iter == 1:
-        _, _, cb0, cr0, _ = bd.bkg_estimate_masked(ctx, d_img, dev(bad0), p, px)
-        m0 = bd.bkg_subtract(ctx, d_img, p.mesh_h, p.mesh_w, cb0, cr0, cfg.detect_k)["mask"][0].cpu().numpy()
-        assert np.array_equal(bad_g, obv.dilate(m0, grow) | (bad0[0] != 0))
-    b = obv.background_masked(img[0], bad_g, to_oracle_params(p), opx)
+    bad_k = (bad0[0] != 0).astype(np.uint8)
+    frag1 = None
+    for k in range(1, n_iter + 1):
+        _, _, cbk, crk, _ = bd.bkg_estimate_masked(ctx, d_img, dev(bad_k[None]), p, px)
+        m_k = bd.bkg_subtract(ctx, d_img, p.mesh_h, p.mesh_w, cbk, crk, cfg.detect_k)["mask"][0].cpu().numpy()
+        ok = obv.background_masked(img[0], bad_k, to_oracle_params(p), opx)
+        _, _, det_k, frag_k = oracle.subtract_threshold(img[0], ok["bkg"], ok["rms"], cfg.detect_k)
+        assert_mask_parity(m_k, det_k, frag_k)                                   # (i)
+        frag1 = frag_k if k == 1 else frag1
+        bad_k = (obv.dilate(m_k, grow) | (bad0[0] != 0)).astype(np.uint8)        # (ii)
+    assert np.array_equal(bad_g, bad_k)
+    b = obv.background_masked(img[0], bad_g, to_oracle_params(p), opx)           # (iii)
     assert np.array_equal(valid[0].cpu().numpy(), b["valid"])
     assert np.max(np.abs(bm[0].cpu().numpy() - b["bkg_grid"]) / np.abs(b["bkg_grid"])) < 1e-6
     assert np.max(np.abs(cb[0].cpu().numpy() - b["bkg_coef"])) <= 1e-9 * np.max(np.abs(b["bkg_coef"]))
     assert np.max(np.abs(cr[0].cpu().numpy() - b["rms_coef"])) <= 1e-9 * np.max(np.abs(b["rms_coef"]))
-    ob, obad = obv.iterate(img[0], bad0[0], to_oracle_params(p), opx, cfg.detect_k, n_iter)
-    assert (obad != bad_g).sum() <= 1e-4 * bad_g.size
+    ob, obad = obv.iterate(img[0], bad0[0], to_oracle_params(p), opx, cfg.detect_k, n_iter)   # (iv)
+    diff = obad != bad_g
+    if n_iter == 1:
+        assert not (diff & ~(obv.dilate(frag1.astype(np.uint8), grow) != 0)).any()
+    assert diff.sum() <= 1e-4 * bad_g.size
     assert np.max(np.abs(bm[0].cpu().numpy() - ob["bkg_grid"]) / np.abs(ob["bkg_grid"])) < 1e-4
 
 

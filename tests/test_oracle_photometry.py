@@ -109,3 +109,40 @@ def test_aperture_weights_are_fractions():
     assert w.min() == 0.0 and w.max() == 1.0 and np.array_equal(w, w[::-1, ::-1]) and np.array_equal(w, w.T)
     assert w[8, 8] == 1.0 and w[8, 8 + 4] == 1.0 and w[8, 8 + 6] == 0.0 and 0.0 < w[8, 8 + 5] < 1.0
     assert w[8, 8 + 5] == pytest.approx(0.5, abs=0.11)     # the rim pixel on the axis is cut in half
+
+
+def test_a28_records_without_an_ellipse_are_not_measured():
+    """Reading A28 (PAPER.md:159 names the methods only): a record whose centroid or moments are not finite, or whose
+    moments still define no ellipse after the 1/12 rule (A24), is not measured -- every sum 0, flags = 4 -- while the
+    1/12 rule itself keeps measuring.  Expected values written out by hand: a spike of 100 at (40, 50) on zeros, rms = 1,
+    so s1 = 0, the Kron radius is the minimum 3.5 and the auto ellipse is a circle of 3.5 sqrt(x2) pixels about (40, 50)."""
+    sub = np.zeros((90, 110), np.float32); sub[50, 40] = 100.0
+    rms = np.ones_like(sub)
+    p = ph.PhotParams()
+    zeros = (0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0, 4)
+    nan, inf = float("nan"), float("inf")
+    not_measured = [(nan, 50.0, 2.0, 2.0, 0.0), (40.0, nan, 2.0, 2.0, 0.0),        # centroid
+                    (40.0, 50.0, inf, 2.0, 0.0), (40.0, 50.0, 2.0, -inf, 0.0), (40.0, 50.0, 2.0, 2.0, nan),   # moments
+                    (40.0, 50.0, -3.0, -3.0, 0.0),      # D = 9 > 0 but both variances negative
+                    (40.0, 50.0, -0.5, 2.0, 0.0),       # D = -1: the 1/12 rule gives (-0.4167, 2.0833), D still < 0
+                    (40.0, 50.0, 1.0, 1.0, 1.5),        # |xy| > sqrt(x2 y2): D = -1.25, after 1/12: 1.1736 - 2.25 < 0
+                    (40.0, 50.0, -1.0 / 12.0, 1.0, 0.0)]  # the rule lifts x2 to exactly 0: no ellipse
+    for r in not_measured:
+        o = ph.photometry(sub, rms, rec(*r), p)[0]
+        assert tuple(o) == zeros, (r, tuple(o))
+    # D = x2 y2 - xy^2 just BELOW 0.00694 (0.083^2 = 0.006889): 1/12 is added, radius 3.5 sqrt(0.083 + 1/12) = 1.427 px:
+    # the centre, its 4 neighbours (1 px) and the 4 diagonals (1.414 px) = 9 pixels
+    lo = ph.photometry(sub, rms, rec(40.0, 50.0, 0.083, 0.083, 0.0), p)[0]
+    assert (lo["flags"], lo["npix_auto"], lo["kron_radius"], lo["flux_auto"]) == (0, 9, 3.5, 100.0)
+    assert lo["fluxerr_auto"] == pytest.approx(3.0, rel=1e-12)
+    # just ABOVE (0.0834^2 = 0.006956): measured as it stands, radius 3.5 sqrt(0.0834) = 1.011 px: centre + 4 neighbours
+    hi = ph.photometry(sub, rms, rec(40.0, 50.0, 0.0834, 0.0834, 0.0), p)[0]
+    assert (hi["flags"], hi["npix_auto"], hi["kron_radius"], hi["flux_auto"]) == (0, 5, 3.5, 100.0)
+    assert hi["fluxerr_auto"] == pytest.approx(np.sqrt(5.0), rel=1e-12)
+    # the aperture sums of a measured record do not depend on the moments: circle of r = 5 about the spike
+    for o in (lo, hi):
+        assert o["flux_aper"] == 100.0 and o["area_aper"] == pytest.approx(np.pi * 25.0, rel=0.01)
+    # a degenerate record between two good ones leaves them alone (records are independent)
+    cat = np.concatenate([rec(40.0, 50.0, 0.0834, 0.0834, 0.0), rec(nan, 50.0, 2.0, 2.0, 0.0), rec(40.0, 50.0, 0.083, 0.083, 0.0)])
+    o3 = ph.photometry(sub, rms, cat, p)
+    assert list(o3["flags"]) == [0, 4, 0] and list(o3["npix_auto"]) == [5, 0, 9]
