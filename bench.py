@@ -18,7 +18,7 @@ collective); value = all ranks' pixels / max-over-ranks time.
 `--impl reference` times the CPU oracle, as it stands, on a bounded crop of the same workload.
 The default run (config 3, N = 1) also reports, outside the timed region: `configs` -- the same step on configs 1, 2, 4, 5
 (inputs of configs 1-2 rotated through > 256 MB of distinct copies so that L2 cannot serve them), each with its own clock
-sample -- and `next_stages_ms` -- deblend_sources, clean_sources, photometry and image_subtract on config 3.
+sample -- and `next_stages_ms` -- deblend_sources, clean_sources, photometry, image_subtract and image_reproject on config 3.
 """
 from __future__ import annotations
 
@@ -276,8 +276,8 @@ class Workload:
         self.torch.cuda.empty_cache()
 
 
-def time_next_stages(bd, torch, ctx, wl, reps=5):
-    """deblend_sources, clean_sources, photometry and image_subtract on the maps of the last step (outside the timed region)."""
+def time_next_stages(bd, torch, ctx, wl, reps=5, sm_mhz=None, hbm_peak=None):
+    """deblend_sources, clean_sources, photometry, image_subtract and image_reproject on the maps of the last step (outside the timed region)."""
     cfg, cap = wl.cfg, wl.cap
     sub, rms = wl.o3["sub"], wl.o3["rms"]
     ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
@@ -319,10 +319,26 @@ def time_next_stages(bd, torch, ctx, wl, reps=5):
     out["image_subtract_gflops"] = 2.0 * 441 * wl.npx / (out["image_subtract"] * 1e-3) / 1e9
     # K8 is bound by the float32 FMA pipe (K8): peak = SMs x 128 FMA/clk x 2 flop x the SM clock of the run
     prop = torch.cuda.get_device_properties(sub.device)
-    peak_tf = prop.multi_processor_count * 128 * 2 * 1.965e9 / 1e12
+    clk_mhz = float(sm_mhz) if sm_mhz else 1965.0    # the SM clock sampled under load during the timed steps
+    peak_tf = prop.multi_processor_count * 128 * 2 * clk_mhz * 1e6 / 1e12
     out["roofline_image_subtract"] = {"kernel": "k8_stamp_conv<10>", "bound": "alu", "achieved": out["image_subtract_gflops"] / 1e3, "peak": peak_tf,
                                       "unit": "TFLOP/s", "frac": out["image_subtract_gflops"] / 1e3 / peak_tf,
-                                      "peak_source": "SMs x 128 FP32 FMA/clk x 2 x 1.965 GHz (B200_PROFILING.md unit counts and clocks)", "traffic": None}
+                                      "peak_source": f"SMs x 128 FP32 FMA/clk x 2 x {clk_mhz:.0f} MHz (B200_PROFILING.md unit counts; SM clock sampled under load)", "traffic": None}
+    # K11: bilinear reprojection through a small rotation + shear + shift; 4 B/px read + 4 B/px written
+    A = torch.tensor([[1.0007 * np.cos(0.004), -1.0007 * np.sin(0.004) + 0.0006, 3.37, 1.0007 * np.sin(0.004), 1.0007 * np.cos(0.004), -2.81]] * wl.B,
+                     dtype=torch.float64, device=sub.device)
+    tr = []
+    for _ in range(reps + 1):
+        e0, e1 = ev(), ev()
+        e0.record()
+        bd.image_reproject(ctx, wl.imgs[0], A, None, 0.0, out=diff)
+        e1.record()
+        torch.cuda.synchronize()
+        tr.append(e0.elapsed_time(e1))
+    out["image_reproject"] = float(np.median(tr[1:]))
+    gbs = 8.0 * wl.npx / (out["image_reproject"] * 1e-3) / 1e9
+    out["roofline_image_reproject"] = {"kernel": "k11_reproject", "bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s",
+                                       "frac": gbs / hbm_peak if hbm_peak else None, "bytes_per_px": 8.0, "traffic": None}
     return out
 
 
@@ -473,7 +489,7 @@ def main():
     extras = not args.no_extras and world == 1 and args.config == 3 and not args.unfused
     if extras:
         # SURVEY 8(f) stages on this config, then the other configs (parity-test cases; reported, not the headline)
-        line["next_stages_ms"] = time_next_stages(bd, torch, ctx, wl)
+        line["next_stages_ms"] = time_next_stages(bd, torch, ctx, wl, sm_mhz=(clocks or {}).get("sm_mhz"), hbm_peak=peak)
         wl.free()
         others = []
         for c in (1, 2, 4, 5):

@@ -340,6 +340,23 @@ int image_subtract(bd_ctx *ctx, const float *d_ref, const float *d_img, int B, i
                    const double *d_kcoef, const double *d_bgcoef, float *d_diff, float *d_conv, void *d_ws,
                    size_t ws_bytes, void *cuda_stream);
 
+/* ---- SURVEY 8(f) NEXT-4, second half: bilinear reprojection through an affine matrix (kernel K11).
+ * PAPER.md:114 ("we use the affine matrix to obtain the coordinate mapping between the source image and the resulting image.
+ * For each pixel in the source image, the pixel value in the resulting image is calculated through bilinear interpolation
+ * based on the four neighboring pixels").  The FIT of the matrix is out of scope: the matrix is an input.  Readings R1-R6:
+ *   R1  d_affine: float64 [B][6] on the device, one row-major 2 x 3 matrix per frame, the FORWARD map source pixel (x, y) ->
+ *       result pixel (x', y') = (a0 x + a1 y + a2, a3 x + a4 y + a5).  The result pulls: result(x', y') is the source
+ *       sampled at A^-1 (x', y');   R2  pixel centres at integers, x = column, y = row, 0-based;
+ *   R3  neighbours (x0, y0) .. (x0+1, y0+1), x0 = floor(xs), y0 = floor(ys), weights (1-fx)(1-fy), fx(1-fy), (1-fx)fy, fx fy;
+ *   R4  a neighbour outside the source frame has the value `fill` and is interpolated like any other;
+ *   R5  a matrix without an inverse (det = 0, or non-finite entries) gives a result frame of `fill`;
+ *   R6  A^-1 and the source coordinates are float64, fx, fy and the blend float32 (within 1e-6 max|src| of the float64
+ *       definition).
+ * d_src: float32 [B,Hs,Ws]; d_out: float32 [B,Hd,Wd] (its own shape; Ws and Wd multiples of 4), must not alias d_src.
+ * No workspace.  Deterministic. */
+int image_reproject(bd_ctx *ctx, const float *d_src, int B, int Hs, int Ws, const double *d_affine, double fill,
+                    float *d_out, int Hd, int Wd, void *cuda_stream);
+
 /* ---- whole chain from HOST buffers (pinned or pageable), synchronous. ----------------------------------
  * Copies h_img to the device in up to 8 chunks (whole frames of a batch, strips of mesh rows of a single frame) on a
  * copy stream of its own and runs the statistics kernel of step a1 on every chunk as it arrives, then a2 and

@@ -67,6 +67,9 @@ def reproject(src: np.ndarray, A, out_shape=None, fill: float = 0.0, only=None) 
     xd = xd.astype(np.float64); yd = yd.astype(np.float64)
     xs = inv[0] * xd + inv[1] * yd + inv[2]
     ys = inv[3] * xd + inv[4] * yd + inv[5]
+    # (coordinates far outside the frame, up to the overflow of a huge translation: all four neighbours are outside, R4;
+    #  clamped to two pixels beyond the frame so that the integer cast below is defined -- the weights are then irrelevant)
+    xs = np.clip(xs, -3.0, W + 2.0); ys = np.clip(ys, -3.0, H + 2.0)
     x0 = np.floor(xs); y0 = np.floor(ys)
     fx, fy = xs - x0, ys - y0
     x0 = x0.astype(np.int64); y0 = y0.astype(np.int64)

@@ -16,7 +16,7 @@ import torch
 from . import _build
 
 __all__ = ["BkgParams", "Context", "SOURCE_DTYPE", "bkg_estimate", "bkg_subtract", "detect_sources", "mesh_stats",
-           "grid_filter_spline", "grid_filter_spline_static", "GRID_STATIC_MAX_DOUBLES", "bkg_subtract_detect", "photometry", "PhotParams", "PHOT_DTYPE", "deblend_sources", "clean_sources", "DeblendParams", "run_host", "grid_shape", "load_library", "EXPORTS"]
+           "grid_filter_spline", "grid_filter_spline_static", "image_reproject", "GRID_STATIC_MAX_DOUBLES", "bkg_subtract_detect", "photometry", "PhotParams", "PHOT_DTYPE", "deblend_sources", "clean_sources", "DeblendParams", "run_host", "grid_shape", "load_library", "EXPORTS"]
 
 EXPORTS = ["bd_create", "bd_destroy", "bd_last_error", "bd_default_bkg_params", "bd_grid_shape",
            "bd_bkg_workspace_bytes", "bd_detect_workspace_bytes", "bd_mesh_stats", "bd_grid_filter_spline",
@@ -25,7 +25,7 @@ EXPORTS = ["bd_create", "bd_destroy", "bd_last_error", "bd_default_bkg_params", 
            "bd_run_host", "bd_default_bkgx_params", "bd_mesh_stats_masked", "bkg_estimate_masked",
            "bd_bkg_iterate_workspace_bytes", "bkg_iterate", "bd_default_conv_params", "bd_conv_num_basis",
            "bd_subtract_workspace_bytes", "image_subtract", "bd_default_deblend_params", "bd_deblend_workspace_bytes",
-           "deblend_sources", "bd_clean_workspace_bytes", "clean_sources"]
+           "deblend_sources", "bd_clean_workspace_bytes", "clean_sources", "image_reproject"]
 DEBUG_EXPORTS = ["bd_debug_k1_slow_meshes", "bd_debug_k1_reasons", "bd_debug_k1_force_slow", "bd_debug_tile_kernel_events"]
 
 
@@ -605,3 +605,18 @@ def run_host(ctx: Context, img: np.ndarray, p: BkgParams, detect_k: float, min_a
                                   C.c_void_p(n.ctypes.data)))
     return cat[: min(int(n.sum()), cat_capacity)], n
 
+
+def image_reproject(ctx: Context, src: torch.Tensor, affine: torch.Tensor, out_shape=None, fill: float = 0.0, out: torch.Tensor | None = None):
+    """NEXT-4, second half (K11): bilinear reprojection.  src float32 [B,Hs,Ws]; affine float64 [B,6] (or [B,2,3]) on the
+    device, the forward map source -> result (R1); out_shape (Hd, Wd), default the source's.  -> float32 [B,Hd,Wd]."""
+    _chk(ctx, src, torch.float32, "src")
+    B, Hs, Ws = src.shape
+    _chk(ctx, affine, torch.float64, "affine")
+    if affine.numel() != B * 6:
+        raise BkgdetError(f"affine: expected {B} x 6 numbers, got {tuple(affine.shape)}")
+    Hd, Wd = (Hs, Ws) if out_shape is None else out_shape
+    if out is None:
+        out = torch.empty((B, Hd, Wd), dtype=torch.float32, device=_dev(ctx))
+    _chk(ctx, out, torch.float32, "out", (B, Hd, Wd))
+    ctx.check(ctx.lib.image_reproject(ctx.h, _ptr(src), B, Hs, Ws, _ptr(affine), C.c_double(fill), _ptr(out), Hd, Wd, _stream(ctx)))
+    return out

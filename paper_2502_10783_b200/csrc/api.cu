@@ -443,6 +443,19 @@ int image_subtract(bd_ctx *ctx, const float *d_ref, const float *d_img, int B, i
     return k8_launch(ctx, d_ref, d_img, B, H, W, p, d_kcoef, d_bgcoef, d_diff, d_conv, d_ws, (cudaStream_t)cuda_stream);
 }
 
+int image_reproject(bd_ctx *ctx, const float *d_src, int B, int Hs, int Ws, const double *d_affine, double fill, float *d_out,
+                    int Hd, int Wd, void *cuda_stream) {
+    int rc = check_frame(ctx, B, Hs, Ws);
+    if (rc) return rc;
+    if ((rc = check_frame(ctx, B, Hd, Wd))) return rc;
+    if (Hd > 65535 * 16) return bd_set_error(ctx, BD_EUNSUPPORTED, "result frames taller than 1 048 560 rows are not supported");
+    BD_BIND_DEVICE(ctx);
+    if (!d_src || !d_affine || !d_out) return bd_set_error(ctx, BD_EINVAL, "null pointer");
+    if (!aligned16(d_out) || ((uintptr_t)d_affine & 7)) return bd_set_error(ctx, BD_EINVAL, "d_out must be 16-byte, d_affine 8-byte aligned");
+    if (d_src == d_out) return bd_set_error(ctx, BD_EINVAL, "d_out must not alias d_src");
+    return k11_launch(ctx, d_src, B, Hs, Ws, d_affine, (float)fill, d_out, Hd, Wd, (cudaStream_t)cuda_stream);
+}
+
 // bd_run_host returns early on any error; by then copies on the copy stream may still be reading the caller's h_img and
 // writing h_n_sources / h_cat.  The guard waits for both streams on every such path (the caller may free its buffers as
 // soon as the call returns); the successful path has already synchronised and disarms it.

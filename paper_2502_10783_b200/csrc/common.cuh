@@ -130,6 +130,10 @@ size_t k8_workspace_bytes(int B, const bd_conv_params *p);
 int k8_launch(bd_ctx *ctx, const float *d_ref, const float *d_img, int B, int H, int W, const bd_conv_params *p,
               const double *d_kcoef, const double *d_bgcoef, float *d_diff, float *d_conv, void *d_ws, cudaStream_t st);
 
+// K11: bilinear reprojection through a per-frame affine matrix (d_affine: float64 [B][6], source -> result)
+int k11_launch(bd_ctx *ctx, const float *d_src, int B, int Hs, int Ws, const double *d_affine, float fill, float *d_out, int Hd,
+               int Wd, cudaStream_t st);
+
 // ---- programmatic dependent launch (the small kernels that follow a large one on the same stream) ------------------
 // A kernel launched with bd_launch_pdl may become resident while its predecessor is still draining; it must call
 // bd_pdl_wait() before it touches anything the predecessor wrote (the wait returns when the whole predecessor grid has
