@@ -429,7 +429,8 @@ def main():
     e2e = None
     if not args.no_e2e:
         pinned = torch.from_numpy(img_h).pin_memory()
-        cat_h = np.empty(cap, dtype=bd.SOURCE_DTYPE)
+        cat_pin = torch.empty(cap * bd.SOURCE_DTYPE.itemsize, dtype=torch.uint8).pin_memory()   # (a pageable buffer is staged by the driver: ~1 ms more for 15 MB)
+        cat_h = cat_pin.numpy().view(bd.SOURCE_DTYPE)
         host_img = pinned.numpy()
         for _ in range(2):
             bd.run_host(ctx, host_img, wl.p, cfg.detect_k, cfg.min_area, cap, cat=cat_h)
@@ -443,8 +444,8 @@ def main():
         dt = shard.max_over_ranks(dt, dist, dev)
         e2e = {"value": world * npx / dt / 1e6, "unit": "Mpix/s", "h2d_bytes_per_step": int(npx * 4),
                "d2h_bytes_per_step": int(len(recs) * bd.SOURCE_DTYPE.itemsize + B * 8), "ms_per_step": dt * 1e3,
-               "api": "bd_run_host (pinned host frame -> catalogue on host)"}
-        del pinned, host_img
+               "api": "bd_run_host (pinned host frame -> catalogue in a pinned host buffer)"}
+        del pinned, host_img, cat_h, cat_pin
 
     if rank != 0:
         if dist: dist.destroy_process_group()

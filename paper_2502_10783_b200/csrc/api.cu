@@ -448,10 +448,9 @@ int image_reproject(bd_ctx *ctx, const float *d_src, int B, int Hs, int Ws, cons
     int rc = check_frame(ctx, B, Hs, Ws);
     if (rc) return rc;
     if ((rc = check_frame(ctx, B, Hd, Wd))) return rc;
-    if (Hd > 65535 * 16) return bd_set_error(ctx, BD_EUNSUPPORTED, "result frames taller than 1 048 560 rows are not supported");
     BD_BIND_DEVICE(ctx);
     if (!d_src || !d_affine || !d_out) return bd_set_error(ctx, BD_EINVAL, "null pointer");
-    if (!aligned16(d_out) || ((uintptr_t)d_affine & 7)) return bd_set_error(ctx, BD_EINVAL, "d_out must be 16-byte, d_affine 8-byte aligned");
+    if (!aligned16(d_out) || !aligned16(d_src) || ((uintptr_t)d_affine & 7)) return bd_set_error(ctx, BD_EINVAL, "d_src, d_out must be 16-byte, d_affine 8-byte aligned");
     if (d_src == d_out) return bd_set_error(ctx, BD_EINVAL, "d_out must not alias d_src");
     return k11_launch(ctx, d_src, B, Hs, Ws, d_affine, (float)fill, d_out, Hd, Wd, (cudaStream_t)cuda_stream);
 }

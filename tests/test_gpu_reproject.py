@@ -37,7 +37,8 @@ def rot(th, s=1.0, sh=0.0, tx=0.0, ty=0.0):
 def test_k11_every_pixel(bd, ctx, Hs, Ws, out_shape, fill):
     rng = np.random.default_rng(Hs + Ws)
     mats = [rot(0.0), rot(0.0, tx=3.0, ty=-2.0), rot(0.2, 1.0, 0.0, 2.3, -1.7), rot(-0.7, 0.9, 0.15, 10.0, 6.5), rot(2.5, 1.3, -0.2, 0.6 * Ws, 0.5 * Hs),
-            rot(0.001, 1.0005, 0.0, -0.37, 0.81), [1, 2, 0, 2, 4, 0], rot(0.3, 40.0), rot(0.3, 0.02, 0.0, 0.4 * Ws, 0.4 * Hs), [1, 0, 1e300, 0, 1, 0]]
+            rot(0.001, 1.0005, 0.0, -0.37, 0.81), [1, 2, 0, 2, 4, 0], rot(0.3, 40.0), rot(0.3, 0.02, 0.0, 0.4 * Ws, 0.4 * Hs), [1, 0, 1e300, 0, 1, 0],
+            rot(-0.003, 0.9995, 0.0, 1.25, 2.5), [1, 0, 0.3, 0.01, 1, -0.2], [1, 0, -0.6, -0.02, 1.0, 0.7], rot(0.004, 1.0007, 0.0006, 3.37, -2.81)]
     B = len(mats)
     src = rng.normal(1000, 200, size=(B, Hs, Ws)).astype(np.float32)
     out = bd.image_reproject(ctx, dev(src), dev(np.array(mats, dtype=np.float64)), out_shape, fill)
